@@ -1,0 +1,166 @@
+"""Pins for oracle/planner.py: hand traces, brute-force optimum + Graham's LPT bound on tiny
+inputs, list-scheduling bound for ROLE_GREEDY, conservation / layout invariants.
+The paper prints no assignment, so nothing here is a paper value; the
+comparison against the *paper's own* planner stays "parity unpinned"."""
+import itertools
+import random
+
+import pytest
+
+from oracle import planner as P
+
+
+def mat(block, rows, cols, dtype=1, flags=0):
+    return (block, 2, rows, cols, dtype, flags)
+
+
+def vec(block, n, dtype=1, flags=0):
+    return (block, 1, n, 1, dtype, flags)
+
+
+def test_roles_one_per_matrix_one_tail_per_block():
+    params = [vec(0, 8), mat(0, 4, 4), vec(0, 3), mat(0, 2, 6), mat(1, 5, 5), vec(2, 7), (2, 3, 6, 2, 1, 0)]
+    roles = P.build_roles(params)
+    kinds = [(r["kind"], r["block"], r["index"], r["numel"]) for r in roles]
+    assert kinds == [(P.ROLE_TAIL, 0, 0, 11), (P.ROLE_MATRIX, 0, 1, 16), (P.ROLE_MATRIX, 0, 3, 12),
+                     (P.ROLE_MATRIX, 1, 4, 25), (P.ROLE_TAIL, 2, 5, 19)]
+    assert roles[0]["members"] == [0, 2]
+
+
+def test_skip_flag_removes_parameter():
+    params = [mat(0, 4, 4, flags=P.PARAM_SKIP), mat(0, 2, 2), vec(0, 5, flags=P.PARAM_SKIP)]
+    roles = P.build_roles(params)
+    assert len(roles) == 1 and roles[0]["index"] == 1
+
+
+def test_seven_equal_roles_two_ranks_hand_trace():
+    params = [mat(0, 8, 8) for _ in range(7)]
+    for policy in (P.POLICY_ROLE_GREEDY, P.POLICY_SCOPE_GREEDY):
+        out = P.plan(params, 2, policy, P.METRIC_NUMEL, rank=0)
+        assert out["owner"] == [0, 1, 0, 1, 0, 1, 0]
+        assert out["loads"][0] == [256, 192]
+
+
+def test_role_vs_scope_hand_trace():
+    # block 0: 10, 1 ; block 1: 9, 2 ; two ranks, numel metric
+    params = [mat(0, 10, 1), mat(0, 1, 1), mat(1, 9, 1), mat(1, 2, 1)]
+    role = P.plan(params, 2, P.POLICY_ROLE_GREEDY, P.METRIC_NUMEL)
+    # block 0: 10 -> r0, 1 -> r1 ; block 1 (loads 10, 1): 9 -> r1 (10), 2 -> r0 (tie 10/10 -> lowest id)
+    assert role["owner"] == [0, 1, 1, 0] and role["loads"][0] == [12, 10]
+    scope = P.plan(params, 2, P.POLICY_SCOPE_GREEDY, P.METRIC_NUMEL)
+    # pooled: 10 (idx0) -> r0, 9 (idx2) -> r1, 2 (idx3) -> r1 (11), 1 (idx1) -> r0 (11)
+    assert scope["owner"] == [0, 0, 1, 1] and scope["loads"][0] == [11, 11]
+
+
+def test_ns_flops_metric_and_separate_tail_vector():
+    params = [vec(0, 100), mat(0, 4, 16), mat(0, 16, 4), mat(0, 8, 8), vec(1, 50), mat(1, 2, 2)]
+    out = P.plan(params, 2, P.POLICY_SCOPE_GREEDY, P.METRIC_NS_FLOPS)
+    # loads: 4x16 and 16x4 -> 16*(32+4) = 576 ; 8x8 -> 64*24 = 1536 ; 2x2 -> 4*6 = 24
+    # sorted: 1536 (idx3) -> r0 ; 576 (idx1) -> r1 ; 576 (idx2) -> r1 (576 < 1536) ; 24 -> r1 (1152 < 1536)
+    # tails on their own vector: 100 -> r0 ; 50 -> r1
+    assert out["owner"] == [0, 1, 1, 0, 1, 1]
+    assert out["loads"] == [[1536, 1176], [100, 50]]
+
+
+def test_world_one_puts_everything_on_rank_zero():
+    params = [vec(0, 3), mat(0, 4, 5), mat(1, 6, 7)]
+    out = P.plan(params, 1, P.POLICY_ROLE_GREEDY, P.METRIC_NUMEL)
+    assert out["owner"] == [0, 0, 0] and len(out["desc"]) == 3
+
+
+def test_heaviest_rank_selection_and_tie():
+    params = [mat(0, 4, 4), mat(0, 4, 4), mat(0, 2, 2)]
+    out = P.plan(params, 2, P.POLICY_SCOPE_GREEDY, P.METRIC_NUMEL, rank=-1)
+    # 16 -> r0, 16 -> r1, 4 -> r0 : heaviest is rank 0
+    assert out["rank"] == 0
+    out = P.plan([mat(0, 4, 4), mat(0, 4, 4)], 3, P.POLICY_SCOPE_GREEDY, P.METRIC_NUMEL, rank=-1)
+    assert out["rank"] == 0   # tie between ranks 0 and 1 -> lowest id
+
+
+def brute_force_makespan(loads, world):
+    best = None
+    for assign in itertools.product(range(world), repeat=len(loads)):
+        per = [0] * world
+        for l, r in zip(loads, assign):
+            per[r] += l
+        mk = max(per)
+        best = mk if best is None else min(best, mk)
+    return best
+
+
+@pytest.mark.parametrize("seed", range(25))
+def test_scope_greedy_within_graham_lpt_bound(seed):
+    rnd = random.Random(seed)
+    world = rnd.choice([2, 3])
+    n = rnd.randint(1, 8)
+    params = [mat(rnd.randint(0, 2), rnd.randint(1, 9), rnd.randint(1, 9)) for _ in range(n)]
+    params.sort(key=lambda p: p[0])
+    out = P.plan(params, world, P.POLICY_SCOPE_GREEDY, P.METRIC_NUMEL)
+    loads = [r["numel"] for r in out["roles"]]
+    opt = brute_force_makespan(loads, world)
+    assert opt <= max(out["loads"][0])
+    assert max(out["loads"][0]) * 3 * world <= (4 * world - 1) * opt      # LPT: <= (4/3 - 1/(3W)) OPT
+    # ROLE_GREEDY is list scheduling in some order: <= (2 - 1/W) OPT
+    role = P.plan(params, world, P.POLICY_ROLE_GREEDY, P.METRIC_NUMEL)
+    assert opt <= max(role["loads"][0])
+    assert max(role["loads"][0]) * world <= (2 * world - 1) * opt
+
+
+@pytest.mark.parametrize("seed", range(10))
+@pytest.mark.parametrize("policy", [P.POLICY_ROLE_GREEDY, P.POLICY_SCOPE_GREEDY])
+@pytest.mark.parametrize("metric", [P.METRIC_NUMEL, P.METRIC_NS_FLOPS])
+def test_invariants_random_models(seed, policy, metric):
+    rnd = random.Random(1000 + seed)
+    world = rnd.randint(1, 6)
+    params = []
+    for b in range(rnd.randint(1, 6)):
+        for _ in range(rnd.randint(1, 7)):
+            if rnd.random() < 0.6:
+                params.append(mat(b, rnd.choice([1, 3, 64, 100, 128]), rnd.choice([1, 5, 64, 96, 256])))
+            else:
+                params.append(vec(b, rnd.randint(1, 300)))
+    out = P.plan(params, world, policy, metric, rank=-1)
+    roles, owner = out["roles"], out["owner"]
+    assert all(0 <= o < world for o in owner)                       # every role exactly one owner
+    per = [[0] * world, [0] * world]
+    for r, o in zip(roles, owner):
+        vecid, load = P.role_load(r, metric)
+        per[vecid][o] += load
+    assert per == out["loads"]                                      # loads conserved
+    covered = sorted(i for r in roles for i in r["members"])
+    assert covered == list(range(len(params)))                      # every parameter in exactly one role
+    # descriptor tables of all ranks partition the roles; offsets aligned, disjoint, ordered
+    seen = 0
+    for k in range(world):
+        d = P.plan(params, world, policy, metric, rank=k)["desc"]
+        seen += len(d)
+        P.validate_desc(d)
+        assert [x["param_id"] for x in d] == sorted(x["param_id"] for x in d)
+        for x in d:
+            if x["role"] == P.ROLE_MATRIX:
+                assert (x["flags"] & P.DESC_TRANSPOSED) == (1 if x["rows"] > x["cols"] else 0)
+            else:
+                assert x["cols"] == 1
+    assert seen == len(roles)
+    assert out["rank"] == max(range(world), key=lambda k: (out["loads"][0][k], -k))
+
+
+def test_validate_rejects_bad_tables():
+    good = [dict(role=0, param_id=0, block_id=0, rows=4, cols=16, dtype=1, flags=0, elem_off=0),
+            dict(role=0, param_id=1, block_id=0, rows=4, cols=16, dtype=1, flags=0, elem_off=64)]
+    assert P.validate_desc(good)
+    for bad in ([dict(good[0], elem_off=8)], [good[0], dict(good[1], elem_off=0)],
+                [dict(good[0], rows=0)], [dict(good[0], role=7)]):
+        with pytest.raises(ValueError):
+            P.validate_desc(bad)
+
+
+def test_transformer_shaped_balance_is_in_the_papers_range():
+    """Sanity only (PAPER.md:174, 219-222 report max/avg 1.02-1.39 on other models)."""
+    params = []
+    for b in range(16):
+        params += [vec(b, 4096), mat(b, 4096, 4096), mat(b, 4096, 4096), mat(b, 4096, 4096), mat(b, 4096, 4096),
+                   vec(b, 4096), mat(b, 16384, 4096), mat(b, 4096, 16384)]
+    for policy in (P.POLICY_ROLE_GREEDY, P.POLICY_SCOPE_GREEDY):
+        out = P.plan(params, 8, policy, P.METRIC_NUMEL)
+        assert 1.0 <= P.balance(out["loads"][0]) <= 1.4
