@@ -1,0 +1,204 @@
+/* mfsdp.h -- C ABI of the owner-local optimizer step of MatrixFSDP (arxiv/paper_2607_05895), B200 / sm_100a.
+ *
+ * What the library computes (PAPER.md = /root/reference/PAPER.md, the paper text):
+ *   PAPER.md:45   each DP-sharded 2D weight lives whole on one owner rank; the non-2D tensors of an FSDP unit
+ *                 are packed into one tail role on a tail owner and stay on AdamW.
+ *   PAPER.md:47   "The owner applies the Newton-Schulz update to the full matrix and updates its local parameter
+ *                 and Muon state, so the optimizer step contains no matrix all-gather, broadcast, or
+ *                 redistribute.  Tail owners apply AdamW to their packed non-matrix tensors."
+ *   PAPER.md:97   optimizer routing: Muon sees a matrix only on its owner, tail-owner shards go to AdamW.
+ *   PAPER.md:101-107 (Algorithm 1) + PAPER.md:65-71: the balance-aware owner planner.
+ * The Muon arithmetic itself (the paper never prints it) is fixed by BASELINE.json's north_star and the readings
+ * listed in DESIGN.md section 4: EMA Nesterov momentum, Frobenius normalisation with eps clamp, K-step quintic
+ * Newton-Schulz (A = X X^T, B = bA + cA^2, X <- aX + BX, tall matrices transposed), scaled decoupled-decay update.
+ *
+ * Conventions
+ *   * Plain C, POD structs with fixed-width fields, no torch / C++ types.  Every pointer is annotated HOST or DEVICE.
+ *   * Ownership: the caller owns every buffer.  The library never allocates or frees caller-visible device memory
+ *     and keeps no state except a small per-process cache of host-built launch tables (tensor maps, tile tables).
+ *   * Asynchrony: the *_step functions enqueue work on `cuda_stream` (a cudaStream_t passed as void*, NULL = the
+ *     legacy default stream) and return without synchronising.  G is read-only; W, M (P, m, v) are updated in place.
+ *   * Errors: 0 on success, a negative MFSDP_E* code otherwise; nothing is printed, nothing throws or aborts.
+ *   * Determinism: fixed reduction order and a static tile schedule -> same inputs give bit-identical outputs.
+ *   * There is NO CPU fallback: on a machine without an sm_100 device the step functions return MFSDP_EARCH.
+ */
+#ifndef MFSDP_H_
+#define MFSDP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- enums (plain ints in the ABI) ------------------------------------------------------------------------- */
+enum { MFSDP_BF16 = 0, MFSDP_F32 = 1 };                       /* storage dtype of W / G (tails: P / G)            */
+enum { MFSDP_ROLE_MATRIX = 0, MFSDP_ROLE_TAIL = 1 };          /* PAPER.md:103 Alg. 1 line 1                       */
+enum { MFSDP_POLICY_ROLE_GREEDY = 0,                          /* PAPER.md:104 Alg. 1 line 2                       */
+       MFSDP_POLICY_SCOPE_GREEDY = 1 };                       /* PAPER.md:105 Alg. 1 line 3                       */
+enum { MFSDP_METRIC_NUMEL = 0,                                /* PAPER.md:65 "greedy load is owner-resident numel" */
+       MFSDP_METRIC_NS_FLOPS = 1 };                           /* BASELINE.json C4/C5: m^2 (2n + m), m=min n=max    */
+enum { MFSDP_SCALE_MATCH_RMS_ADAMW = 0,                       /* 0.2 sqrt(max(rows, cols))       */
+       MFSDP_SCALE_ORIGINAL = 1,                              /* sqrt(max(1, rows / cols))                        */
+       MFSDP_SCALE_NONE = 2 };
+enum { MFSDP_NS_BF16 = 0,                                     /* bf16 operands, fp32 accumulate (tcgen05)         */
+       MFSDP_NS_FP32 = 1 };                                   /* fp32 operands and accumulate (FFMA), no TF32     */
+enum { MFSDP_PARAM_SKIP = 1u };                               /* mfsdp_param_t.flags bit0 (PAPER.md:45 TP skip)   */
+enum { MFSDP_DESC_TRANSPOSED = 1u };                          /* mfsdp_desc_t.flags bit0: rows > cols (NS runs on X^T) */
+enum { MFSDP_SEG_ALIGN = 64 };                                /* every segment starts on a 64-element boundary    */
+
+enum { MFSDP_OK = 0, MFSDP_EINVAL = -1, MFSDP_ECAP = -2, MFSDP_ELAYOUT = -3, MFSDP_EARCH = -4, MFSDP_ECUDA = -5 };
+
+/* ---- records ------------------------------------------------------------------------------------------------ */
+/* One model parameter, in model order (planner input). */
+typedef struct {
+  uint32_t block_id; /* FSDP unit; non-decreasing in model order                                                  */
+  uint32_t ndim;     /* 2 -> matrix role; anything else -> member of the block's tail role                        */
+  uint32_t rows;     /* ndim != 2: rows = numel, cols = 1                                                         */
+  uint32_t cols;
+  uint32_t dtype;    /* MFSDP_BF16 | MFSDP_F32                                                                    */
+  uint32_t flags;    /* MFSDP_PARAM_SKIP                                                                          */
+} mfsdp_param_t;
+
+/* One resident segment of one rank (planner output, step input): the analogue of the paper's MatrixShard layout
+ * entry: "one full segment per 2D matrix, one packed tail segment per block".
+ * Matrices live in one rank-flat element space (W, G, M share offsets), tails in another (P, G, m, v). */
+typedef struct {
+  uint32_t role;     /* MFSDP_ROLE_MATRIX | MFSDP_ROLE_TAIL                                                       */
+  uint32_t param_id; /* index into params[] (a tail: index of its first member)                                   */
+  uint32_t block_id;
+  uint32_t rows;     /* as stored, row-major, cols contiguous.  tail: rows = packed numel, cols = 1               */
+  uint32_t cols;
+  uint32_t dtype;
+  uint32_t flags;    /* MFSDP_DESC_TRANSPOSED                                                                     */
+  uint32_t reserved; /* 0                                                                                         */
+  uint64_t elem_off; /* offset in ELEMENTS into the rank-flat buffers of its element space; multiple of 64        */
+} mfsdp_desc_t;
+
+/* Hyper-parameters are doubles so that derived constants (1 - mu, 1 - lr wd, 1 - beta^t) are formed in double on
+ * the host and rounded once to the kernels' fp32. */
+typedef struct {
+  double  lr;            /* eta                                                                                   */
+  double  weight_decay;  /* lambda, decoupled: W <- W (1 - eta lambda) - eta s O                                  */
+  double  momentum;      /* mu: M <- mu M + (1 - mu) G                                                            */
+  double  a, b, c;       /* quintic coefficients (north_star fallback 3.4445, -4.7750, 2.0315)                    */
+  double  eps;           /* X0 = U / max(||U||_F, eps), 1e-7                                                      */
+  int32_t nesterov;      /* != 0: U = (1 - mu) G + mu M ; 0: U = M                                                */
+  int32_t ns_steps;      /* K >= 1 (north_star: 5; the paper's runs: 2)                             */
+  int32_t scale_mode;    /* MFSDP_SCALE_*                                                                         */
+  int32_t precision;     /* MFSDP_NS_BF16 | MFSDP_NS_FP32                                                         */
+} mfsdp_muon_hparams_t;
+
+typedef struct {
+  double  lr, beta1, beta2, eps, weight_decay;
+  int64_t step;          /* 1-based step count t used for bias correction                                         */
+} mfsdp_adamw_hparams_t;
+
+/* ---- planner (HOST only, no CUDA) -----------------------------------------------------------------------------
+ * Algorithm 1, lines 1-3 and 5.  Roles are built from params[] (line 1), assigned greedily
+ * ("largest roles to the currently lightest ranks", ties: load desc, block asc, parameter index asc; lightest rank
+ * ties -> lowest rank id), and the resident set of `rank` (rank < 0: the heaviest rank by primary load, ties ->
+ * lowest id) is emitted as a descriptor table in (block, parameter) order and validated (line 5: one contiguous,
+ * aligned, non-overlapping segment per resident parameter).
+ *   params, n_params    HOST in.   model parameters in model order.
+ *   owner_out           HOST out.  [n_roles] owner rank per role, roles in model order; may be NULL.
+ *   n_roles             HOST out.  number of roles; may be NULL.
+ *   rank_load_out       HOST out.  [2 * world_size]: primary load vector then tail load vector (the latter is all
+ *                                  zero under MFSDP_METRIC_NUMEL, where one vector carries both); may be NULL.
+ *   desc_out, desc_cap  HOST out.  descriptor table of the chosen rank; desc_out == NULL -> size query only.
+ *   n_desc              HOST out.  number of descriptors of the chosen rank (always written).
+ *   rank_out            HOST out.  the rank actually chosen; may be NULL.
+ * Returns MFSDP_EINVAL (null params with n_params > 0, world_size < 1, rank >= world_size, unknown policy/metric,
+ * zero-sized parameter, decreasing block ids, tail members of one block with different dtypes), MFSDP_ECAP
+ * (desc_cap < *n_desc; *n_desc holds the required count), MFSDP_ELAYOUT (validation failed). */
+int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int world_size, int policy, int metric, int rank,
+               int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
+               mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out);
+
+/* Validate a descriptor table against PAPER.md:71 / Alg. 1 line 5 (HOST).  0 or MFSDP_ELAYOUT / MFSDP_EINVAL. */
+int mfsdp_validate_desc(const mfsdp_desc_t* desc, size_t n_desc);
+
+/* Elements spanned by the rank-flat matrix space and tail space of a descriptor table (HOST): what the caller
+ * must allocate for W/G/M (matrix_elems) and P/G/m/v (tail_elems).  Either out pointer may be NULL. */
+int mfsdp_flat_elems(const mfsdp_desc_t* desc, size_t n_desc, uint64_t* matrix_elems, uint64_t* tail_elems);
+
+/* ---- Muon step (DEVICE work, HOST call) ----------------------------------------------------------------------- */
+/* Bytes of DEVICE workspace mfsdp_muon_step needs for this table and precision (HOST). */
+int mfsdp_workspace_bytes(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t* bytes);
+
+/* Where the step leaves its per-matrix intermediates inside the workspace (HOST; for tests and callers that
+ * consume the orthogonalised update): for the `index`-th MATRIX descriptor of the table,
+ *   *o_byte_off   byte offset of O = X_K, stored rows x cols row-major exactly like the parameter (tall matrices
+ *                 are NOT physically transposed: the kernels iterate X <- X (aI + bA' + cA'^2), A' = X^T X, which
+ *                 is the transposed problem of the north_star read through the tensor-core operand descriptors),
+ *                 row pitch *o_pitch elements of bf16 (MFSDP_NS_BF16) or float (MFSDP_NS_FP32);
+ *   *ssq_byte_off byte offset of a double holding ||U||_F^2.
+ * Any out pointer may be NULL. */
+int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision, int ns_steps, size_t index,
+                         size_t* o_byte_off, size_t* o_pitch, size_t* ssq_byte_off);
+
+/* One owner-local Muon step on every MATRIX descriptor of the table (tail descriptors are ignored: routing,
+ * PAPER.md:97).  For each matrix (SURVEY.md 8(c) O-2 / DESIGN.md section 2):
+ *   M <- mu M + (1-mu) G ; U = (1-mu) G + mu M (Nesterov) or M ; X0 = U^(T if tall) / max(||U||_F, eps) ;
+ *   K x { A = X X^T ; B = b A + c A A ; X <- a X + B X } ; O = X_K ; W <- W (1 - lr wd) - lr s(rows, cols) O.
+ *   desc, n_desc   HOST in.    descriptor table (as returned by mfsdp_plan).  All matrix descriptors must share
+ *                              one dtype.
+ *   W              DEVICE i/o. rank-flat weights, dtype of the descriptors, 128-byte aligned base.
+ *   G              DEVICE in.  rank-flat gradients, same dtype and offsets as W.
+ *   M              DEVICE i/o. rank-flat momentum, always float, same element offsets.
+ *   workspace      DEVICE.     >= mfsdp_workspace_bytes, 1024-byte aligned; contents need not be preserved
+ *                              between calls; after the call it holds O and ||U||^2 (mfsdp_workspace_view).
+ *                              The library caches, per (table, workspace pointer, precision), a few KB..MB of
+ *                              launch tables (TMA tensor maps, tile lists) in device memory of its own.
+ *   hp             HOST in.
+ * Returns MFSDP_EINVAL (null / misaligned pointer, bad hyper-parameter, mixed dtypes), MFSDP_ECAP (ws_bytes too
+ * small), MFSDP_ELAYOUT, MFSDP_EARCH (current device is not compute capability 10.x), MFSDP_ECUDA. */
+int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
+                    void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+
+/* Individual passes of the step, exposed so tests can check each kernel against the oracle and bench.py can time
+ * them.  Same arguments and errors as mfsdp_muon_step.
+ *   momentum pass: M, X~ = cast(U) in the workspace, ||U||^2.
+ *   ns pass:       X_K from X~ and ||U||^2 (a2 + a3).
+ *   update pass:   W from O (a4). */
+int mfsdp_muon_momentum_pass(const mfsdp_desc_t* desc, size_t n_desc, const void* G, void* M,
+                             void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+int mfsdp_muon_ns_pass(const mfsdp_desc_t* desc, size_t n_desc, void* workspace, size_t ws_bytes,
+                       const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, void* W, void* workspace, size_t ws_bytes,
+                           const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+
+/* The same step with HOST buffers (pinned or pageable): copies G (and W, M when `upload_state` != 0) to the
+ * caller's device staging buffers dW/dG/dM, runs mfsdp_muon_step, copies W and M back, all on `cuda_stream`, and
+ * synchronises the stream before returning.  Used for the end-to-end measurement. */
+int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, const void* hG, void* hM,
+                         void* dW, void* dG, void* dM, int upload_state,
+                         void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+
+/* ---- AdamW on packed tails (DEVICE work, HOST call) ------------------------------------------------------------
+ * For every TAIL descriptor (matrix descriptors are ignored), element-wise:
+ *   p <- p (1 - lr wd) ; m <- b1 m + (1-b1) g ; v <- b2 v + (1-b2) g^2 ;
+ *   p <- p - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps).
+ *   P, G   DEVICE. rank-flat tail parameters / gradients, dtype of the descriptors (one dtype for all tails).
+ *   m, v   DEVICE. rank-flat first / second moments, always float, same element offsets.
+ * Returns as mfsdp_muon_step (hp->step < 1 is MFSDP_EINVAL). */
+int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, const void* G, void* m, void* v,
+                          const mfsdp_adamw_hparams_t* hp, void* cuda_stream);
+
+/* Debug / test aid (HOST): byte offsets inside the workspace of the `index`-th matrix' NS buffers:
+ * out[0], out[1] = X ping-pong buffers (X~ = cast(U) is written to out[0]; rows x cols like the parameter),
+ * out[2] = A (d x d, d = min(rows, cols)), out[3] = P = aI + bA + cA^2 (d x d),
+ * out[4] = X row pitch in elements, out[5] = A/P row pitch in elements. */
+int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t index, size_t out[6]);
+
+/* ---- misc ----------------------------------------------------------------------------------------------------- */
+const char* mfsdp_strerror(int code);      /* static string; for MFSDP_ECUDA the last CUDA error text            */
+int mfsdp_version(void);                   /* ABI version, currently 1                                            */
+/* Number of kernels the library launched since process start (for bench.py's gpu_launches claim). */
+uint64_t mfsdp_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MFSDP_H_ */

@@ -1,0 +1,316 @@
+// C-ABI entry points of the step (include/mfsdp.h): argument checks, workspace layout, the per-table cache of
+// device launch tables, and the launch sequence.  No compute happens here and there is no CPU fallback.
+#include <cstring>
+#include <mutex>
+#include <string>
+
+#include "mfsdp_internal.h"
+
+namespace mfsdp {
+
+// ---- bookkeeping ------------------------------------------------------------------------------------------------
+namespace {
+std::mutex g_mu;
+uint64_t g_launches = 0;
+std::string g_cuda_err = "no CUDA error recorded";
+std::vector<Plan*> g_plans;
+std::vector<std::vector<uint8_t>> g_plan_keys;
+}  // namespace
+
+void count_launch(uint64_t n) { g_launches += n; }
+int cuda_fail(cudaError_t e) {
+  g_cuda_err = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e);
+  return MFSDP_ECUDA;
+}
+int check_last_launch() {
+  const cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? MFSDP_OK : cuda_fail(e);
+}
+
+// ---- workspace layout -----------------------------------------------------------------------------------------------
+int build_ws_layout(const mfsdp_desc_t* desc, size_t n_desc, int precision, WsLayout& out) {
+  if (n_desc && !desc) return MFSDP_EINVAL;
+  if (precision != MFSDP_NS_BF16 && precision != MFSDP_NS_FP32) return MFSDP_EINVAL;
+  const int rc = mfsdp_validate_desc(desc, n_desc);
+  if (rc) return rc;
+  out = WsLayout();
+  const size_t es = precision == MFSDP_NS_BF16 ? 2 : 4;
+  const uint32_t pad = 8;                               // row pitches are multiples of 8 elements (16 B for bf16)
+  for (size_t i = 0; i < n_desc; ++i) {
+    const mfsdp_desc_t& q = desc[i];
+    if (q.role == MFSDP_ROLE_MATRIX) {
+      if (out.mat_dtype >= 0 && out.mat_dtype != (int)q.dtype) return MFSDP_EINVAL;
+      out.mat_dtype = (int)q.dtype;
+      MatLayout L;
+      std::memset(&L, 0, sizeof L);
+      L.elem_off = q.elem_off; L.rows = q.rows; L.cols = q.cols;
+      L.numel = (uint64_t)q.rows * q.cols;
+      L.tall = q.rows > q.cols;
+      L.d = L.tall ? q.cols : q.rows; L.n_long = L.tall ? q.rows : q.cols;
+      L.pitch_x = (uint32_t)align_up_u64(q.cols, pad);
+      L.pitch_a = (uint32_t)align_up_u64(L.d, pad);
+      L.chunk_begin = out.n_chunks;
+      const uint64_t nch = (L.numel + kChunk - 1) / kChunk;
+      if (nch + out.n_chunks > 0x7fffffffull) return MFSDP_EINVAL;
+      out.n_chunks += (uint32_t)nch;
+      out.mats.push_back(L);
+    } else {
+      if (out.tail_dtype >= 0 && out.tail_dtype != (int)q.dtype) return MFSDP_EINVAL;
+      out.tail_dtype = (int)q.dtype;
+      TailLayout T;
+      T.elem_off = q.elem_off; T.numel = (uint64_t)q.rows * q.cols; T.chunk_begin = out.n_tail_chunks; T.pad = 0;
+      out.n_tail_chunks += (uint32_t)((T.numel + kChunk - 1) / kChunk);
+      out.tails.push_back(T);
+    }
+  }
+  size_t off = 0;
+  const size_t n_mat = out.mats.size();
+  out.ssq_off = off;     off = align_up_u64(off + n_mat * sizeof(double), kBufAlign);
+  out.invn_off = off;    off = align_up_u64(off + n_mat * sizeof(float), kBufAlign);
+  out.partial_off = off; off = align_up_u64(off + (size_t)out.n_chunks * sizeof(double), kBufAlign);
+  for (MatLayout& L : out.mats) {
+    const size_t xb = align_up_u64((size_t)L.rows * L.pitch_x * es, kBufAlign);
+    const size_t ab = align_up_u64((size_t)L.d * L.pitch_a * es, kBufAlign);
+    L.x_off[0] = off; off += xb;
+    L.x_off[1] = off; off += xb;
+    L.a_off = off; off += ab;
+    L.p_off = off; off += ab;
+  }
+  out.total_bytes = off;
+  return MFSDP_OK;
+}
+
+// ---- plan cache ---------------------------------------------------------------------------------------------------------
+namespace {
+template <typename T>
+int upload(T** dptr, const T* h, size_t n) {
+  *dptr = nullptr;
+  if (n == 0) n = 1;
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dptr), n * sizeof(T));
+  if (e != cudaSuccess) return cuda_fail(e);
+  if (h) {
+    e = cudaMemcpy(*dptr, h, n * sizeof(T), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(e);
+  }
+  return MFSDP_OK;
+}
+}  // namespace
+
+int get_plan(const mfsdp_desc_t* desc, size_t n_desc, int precision, void* workspace, bool need_ws, Plan** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e == cudaErrorNoDevice || e == cudaErrorInsufficientDriver ? MFSDP_EARCH : cuda_fail(e);
+  int major = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) return e == cudaErrorNoDevice || e == cudaErrorInsufficientDriver ? MFSDP_EARCH : cuda_fail(e);
+  if (major != 10) return MFSDP_EARCH;
+
+  std::vector<uint8_t> key(sizeof(int) * 2 + sizeof(void*) + n_desc * sizeof(mfsdp_desc_t));
+  {
+    uint8_t* k = key.data();
+    std::memcpy(k, &dev, sizeof(int)); k += sizeof(int);
+    std::memcpy(k, &precision, sizeof(int)); k += sizeof(int);
+    void* wsk = need_ws ? workspace : nullptr;
+    std::memcpy(k, &wsk, sizeof(void*)); k += sizeof(void*);
+    if (n_desc) std::memcpy(k, desc, n_desc * sizeof(mfsdp_desc_t));
+  }
+  std::lock_guard<std::mutex> lock(g_mu);
+  for (size_t i = 0; i < g_plans.size(); ++i)
+    if (g_plan_keys[i] == key) { *out = g_plans[i]; return MFSDP_OK; }
+
+  Plan* pl = new Plan();
+  int rc = build_ws_layout(desc, n_desc, precision, pl->lay);
+  if (rc) { delete pl; return rc; }
+  pl->precision = precision;
+  pl->workspace = need_ws ? workspace : nullptr;
+  pl->device = dev;
+  const WsLayout& lay = pl->lay;
+  std::vector<uint32_t> cb(lay.mats.size() + 1), tcb(lay.tails.size() + 1);
+  for (size_t i = 0; i < lay.mats.size(); ++i) cb[i] = lay.mats[i].chunk_begin;
+  cb[lay.mats.size()] = lay.n_chunks;
+  for (size_t i = 0; i < lay.tails.size(); ++i) tcb[i] = lay.tails[i].chunk_begin;
+  tcb[lay.tails.size()] = lay.n_tail_chunks;
+  if ((rc = upload(&pl->d_mats, lay.mats.data(), lay.mats.size())) ||
+      (rc = upload(&pl->d_tails, lay.tails.data(), lay.tails.size())) ||
+      (rc = upload(&pl->d_chunk_begin, cb.data(), cb.size())) ||
+      (rc = upload(&pl->d_tail_chunk_begin, tcb.data(), tcb.size()))) {
+    return rc;   // a failed cudaMalloc on a tiny table: leave the partial plan to process teardown
+  }
+  if (g_plans.size() >= 64) {          // bound the cache: drop the oldest entry
+    Plan* old = g_plans.front();
+    cudaFree(old->d_mats); cudaFree(old->d_tails); cudaFree(old->d_chunk_begin); cudaFree(old->d_tail_chunk_begin);
+    destroy_ns_tc(old->tc);
+    delete old;
+    g_plans.erase(g_plans.begin());
+    g_plan_keys.erase(g_plan_keys.begin());
+  }
+  g_plans.push_back(pl);
+  g_plan_keys.push_back(std::move(key));
+  *out = pl;
+  return MFSDP_OK;
+}
+
+namespace {
+
+bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int check_hp(const mfsdp_muon_hparams_t* hp) {
+  if (!hp) return MFSDP_EINVAL;
+  if (hp->ns_steps < 1 || hp->ns_steps > 64) return MFSDP_EINVAL;
+  if (!(hp->momentum >= 0.0 && hp->momentum < 1.0)) return MFSDP_EINVAL;
+  if (!(hp->eps > 0.0) || !(hp->lr == hp->lr) || !(hp->weight_decay == hp->weight_decay)) return MFSDP_EINVAL;
+  if (hp->scale_mode < MFSDP_SCALE_MATCH_RMS_ADAMW || hp->scale_mode > MFSDP_SCALE_NONE) return MFSDP_EINVAL;
+  if (hp->precision != MFSDP_NS_BF16 && hp->precision != MFSDP_NS_FP32) return MFSDP_EINVAL;
+  return MFSDP_OK;
+}
+
+// Common front end of the Muon passes: validates, finds the plan, checks the workspace.
+int muon_front(const mfsdp_desc_t* desc, size_t n_desc, void* workspace, size_t ws_bytes,
+               const mfsdp_muon_hparams_t* hp, Plan** pl) {
+  int rc = check_hp(hp);
+  if (rc) return rc;
+  if (n_desc && !desc) return MFSDP_EINVAL;
+  if (!workspace || !aligned(workspace, kBufAlign)) return MFSDP_EINVAL;
+  rc = get_plan(desc, n_desc, hp->precision, workspace, true, pl);
+  if (rc) return rc;
+  if (ws_bytes < (*pl)->lay.total_bytes) return MFSDP_ECAP;
+  return MFSDP_OK;
+}
+
+int ns_dispatch(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
+  return hp.precision == MFSDP_NS_BF16 ? launch_ns_tc(pl, hp, st) : launch_ns_fp32(pl, hp, st);
+}
+
+}  // namespace
+}  // namespace mfsdp
+
+using namespace mfsdp;
+
+extern "C" int mfsdp_workspace_bytes(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t* bytes) {
+  if (!bytes) return MFSDP_EINVAL;
+  WsLayout lay;
+  const int rc = build_ws_layout(desc, n_desc, precision, lay);
+  if (rc) return rc;
+  *bytes = lay.total_bytes;
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision, int ns_steps,
+                                    size_t index, size_t* o_byte_off, size_t* o_pitch, size_t* ssq_byte_off) {
+  WsLayout lay;
+  const int rc = build_ws_layout(desc, n_desc, precision, lay);
+  if (rc) return rc;
+  if (index >= lay.mats.size() || ns_steps < 1) return MFSDP_EINVAL;
+  if (o_byte_off) *o_byte_off = lay.mats[index].x_off[ns_steps & 1];
+  if (o_pitch) *o_pitch = lay.mats[index].pitch_x;
+  if (ssq_byte_off) *ssq_byte_off = lay.ssq_off + index * sizeof(double);
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t index,
+                                      size_t out[6]) {
+  WsLayout lay;
+  const int rc = build_ws_layout(desc, n_desc, precision, lay);
+  if (rc) return rc;
+  if (index >= lay.mats.size() || !out) return MFSDP_EINVAL;
+  const MatLayout& L = lay.mats[index];
+  out[0] = L.x_off[0]; out[1] = L.x_off[1]; out[2] = L.a_off; out[3] = L.p_off; out[4] = L.pitch_x; out[5] = L.pitch_a;
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_muon_momentum_pass(const mfsdp_desc_t* desc, size_t n_desc, const void* G, void* M,
+                                        void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,
+                                        void* cuda_stream) {
+  Plan* pl = nullptr;
+  const int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
+  if (rc) return rc;
+  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!G || !M || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
+  return launch_momentum(*pl, G, M, *hp, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int mfsdp_muon_ns_pass(const mfsdp_desc_t* desc, size_t n_desc, void* workspace, size_t ws_bytes,
+                                  const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
+  Plan* pl = nullptr;
+  const int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
+  if (rc) return rc;
+  if (pl->lay.mats.empty()) return MFSDP_OK;
+  return ns_dispatch(*pl, *hp, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, void* W, void* workspace,
+                                      size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
+  Plan* pl = nullptr;
+  const int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
+  if (rc) return rc;
+  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!W || !aligned(W, 128)) return MFSDP_EINVAL;
+  return launch_update(*pl, W, *hp, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
+                               void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
+  Plan* pl = nullptr;
+  int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
+  if (rc) return rc;
+  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!W || !G || !M || !aligned(W, 128) || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if ((rc = launch_momentum(*pl, G, M, *hp, st))) return rc;
+  if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
+  return launch_update(*pl, W, *hp, st);
+}
+
+extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, const void* hG, void* hM,
+                                    void* dW, void* dG, void* dM, int upload_state, void* workspace,
+                                    size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
+  Plan* pl = nullptr;
+  int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
+  if (rc) return rc;
+  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!hW || !hG || !hM || !dW || !dG || !dM) return MFSDP_EINVAL;
+  uint64_t elems = 0;
+  if ((rc = mfsdp_flat_elems(desc, n_desc, &elems, nullptr))) return rc;
+  const size_t es = pl->lay.mat_dtype == MFSDP_BF16 ? 2 : 4;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaError_t e = cudaMemcpyAsync(dG, hG, elems * es, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  if (upload_state) {
+    if ((e = cudaMemcpyAsync(dW, hW, elems * es, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaMemcpyAsync(dM, hM, elems * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
+  }
+  if ((rc = mfsdp_muon_step(desc, n_desc, dW, dG, dM, workspace, ws_bytes, hp, cuda_stream))) return rc;
+  if ((e = cudaMemcpyAsync(hW, dW, elems * es, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+  if ((e = cudaMemcpyAsync(hM, dM, elems * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, const void* G, void* m,
+                                     void* v, const mfsdp_adamw_hparams_t* hp, void* cuda_stream) {
+  if (!hp || hp->step < 1 || (n_desc && !desc)) return MFSDP_EINVAL;
+  if (!(hp->beta1 >= 0.0 && hp->beta1 < 1.0) || !(hp->beta2 >= 0.0 && hp->beta2 < 1.0) || !(hp->eps >= 0.0))
+    return MFSDP_EINVAL;
+  Plan* pl = nullptr;
+  const int rc = get_plan(desc, n_desc, MFSDP_NS_BF16, nullptr, false, &pl);
+  if (rc) return rc;
+  if (pl->lay.tails.empty()) return MFSDP_OK;
+  if (!P || !G || !m || !v || !aligned(P, 128) || !aligned(G, 128) || !aligned(m, 128) || !aligned(v, 128))
+    return MFSDP_EINVAL;
+  return launch_adamw(*pl, P, G, m, v, *hp, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" const char* mfsdp_strerror(int code) {
+  switch (code) {
+    case MFSDP_OK: return "ok";
+    case MFSDP_EINVAL: return "invalid argument";
+    case MFSDP_ECAP: return "capacity too small";
+    case MFSDP_ELAYOUT: return "descriptor table violates the one-contiguous-segment layout";
+    case MFSDP_EARCH: return "no compute-capability-10.x (sm_100) device; there is no CPU fallback";
+    case MFSDP_ECUDA: return g_cuda_err.c_str();
+    default: return "unknown error code";
+  }
+}
+
+extern "C" int mfsdp_version(void) { return 1; }
+extern "C" uint64_t mfsdp_launch_count(void) { return g_launches; }

@@ -1,0 +1,179 @@
+// Balance-aware owner planner, host side (no CUDA).
+// PAPER.md:101-107 Algorithm 1 lines 1-3 and 5; PAPER.md:65 (greedy load), :71 (contiguity validation),
+// :97 (routing by role).  Readings P1-P6 of DESIGN.md section 4 fix what the paper leaves open
+// (tie-breaks, NS-flops metric, separate tail load vector, heaviest rank).
+#include <algorithm>
+#include <cstring>
+#include <vector>
+
+#include "mfsdp.h"
+
+namespace {
+
+struct Role {
+  uint32_t kind;       // MFSDP_ROLE_*
+  uint32_t block;
+  uint32_t first;      // parameter index (tail: first member)
+  uint32_t rows, cols; // tail: rows = packed numel, cols = 1
+  uint32_t dtype;
+  uint64_t numel;
+};
+
+inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+// Alg. 1 line 1: "each 2D matrix is one role; non-2D tensors form one tail role per block".
+int build_roles(const mfsdp_param_t* p, size_t n, std::vector<Role>& roles) {
+  roles.clear();
+  long tail_slot = -1;           // index in roles[] of the current block's tail role
+  bool have_block = false;
+  uint32_t cur_block = 0;
+  for (size_t i = 0; i < n; ++i) {
+    const mfsdp_param_t& q = p[i];
+    if (have_block && q.block_id < cur_block) return MFSDP_EINVAL;
+    if (!have_block || q.block_id != cur_block) { tail_slot = -1; cur_block = q.block_id; have_block = true; }
+    if (q.flags & MFSDP_PARAM_SKIP) continue;
+    if (q.rows == 0 || q.cols == 0) return MFSDP_EINVAL;
+    if (q.dtype != MFSDP_BF16 && q.dtype != MFSDP_F32) return MFSDP_EINVAL;
+    const uint64_t numel = (uint64_t)q.rows * q.cols;
+    if (q.ndim == 2) {
+      roles.push_back(Role{MFSDP_ROLE_MATRIX, q.block_id, (uint32_t)i, q.rows, q.cols, q.dtype, numel});
+    } else {
+      if (tail_slot < 0) {
+        tail_slot = (long)roles.size();
+        roles.push_back(Role{MFSDP_ROLE_TAIL, q.block_id, (uint32_t)i, 0, 1, q.dtype, 0});
+      }
+      Role& t = roles[(size_t)tail_slot];
+      if (t.dtype != q.dtype) return MFSDP_EINVAL;
+      t.numel += numel;
+      if (t.numel > 0xffffffffull) return MFSDP_EINVAL;
+      t.rows = (uint32_t)t.numel;
+    }
+  }
+  return MFSDP_OK;
+}
+
+// PAPER.md:65 numel load; BASELINE.json C4/C5 NS-flops load m^2 (2n + m) with tails on their own vector (P3).
+inline void role_load(const Role& r, int metric, int& vec, uint64_t& load) {
+  if (metric == MFSDP_METRIC_NUMEL) { vec = 0; load = r.numel; return; }
+  if (r.kind == MFSDP_ROLE_MATRIX) {
+    const uint64_t m = std::min(r.rows, r.cols), n = std::max(r.rows, r.cols);
+    vec = 0; load = m * m * (2 * n + m);
+  } else { vec = 1; load = r.numel; }
+}
+
+// "assign largest roles to the currently lightest ranks" over the role ids in `ids` (P1 tie-breaks).
+void greedy(std::vector<uint32_t>& ids, const std::vector<Role>& roles, int metric, int world,
+            std::vector<uint64_t>* loads, std::vector<int32_t>& owner) {
+  std::vector<uint64_t> key(roles.size());
+  for (uint32_t id : ids) { int v; role_load(roles[id], metric, v, key[id]); }
+  std::stable_sort(ids.begin(), ids.end(), [&](uint32_t x, uint32_t y) {
+    if (key[x] != key[y]) return key[x] > key[y];
+    if (roles[x].block != roles[y].block) return roles[x].block < roles[y].block;
+    return roles[x].first < roles[y].first;
+  });
+  for (uint32_t id : ids) {
+    int v; uint64_t l; role_load(roles[id], metric, v, l);
+    std::vector<uint64_t>& L = loads[v];
+    int best = 0;
+    for (int r = 1; r < world; ++r) if (L[r] < L[best]) best = r;
+    owner[id] = best;
+    L[best] += l;
+  }
+}
+
+}  // namespace
+
+extern "C" int mfsdp_validate_desc(const mfsdp_desc_t* d, size_t n) {
+  if (n && !d) return MFSDP_EINVAL;
+  uint64_t end[2] = {0, 0};
+  for (size_t i = 0; i < n; ++i) {
+    const uint32_t k = d[i].role;
+    if (k != MFSDP_ROLE_MATRIX && k != MFSDP_ROLE_TAIL) return MFSDP_EINVAL;
+    if (d[i].rows == 0 || d[i].cols == 0) return MFSDP_EINVAL;
+    if (d[i].dtype != MFSDP_BF16 && d[i].dtype != MFSDP_F32) return MFSDP_EINVAL;
+    if (k == MFSDP_ROLE_TAIL && d[i].cols != 1) return MFSDP_EINVAL;
+    if (d[i].elem_off % MFSDP_SEG_ALIGN) return MFSDP_ELAYOUT;
+    if (d[i].elem_off < end[k]) return MFSDP_ELAYOUT;          // overlapping or out of order
+    const bool tall = d[i].rows > d[i].cols;
+    if (k == MFSDP_ROLE_MATRIX && tall != ((d[i].flags & MFSDP_DESC_TRANSPOSED) != 0)) return MFSDP_ELAYOUT;
+    end[k] = d[i].elem_off + (uint64_t)d[i].rows * d[i].cols;
+  }
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_flat_elems(const mfsdp_desc_t* d, size_t n, uint64_t* mat, uint64_t* tail) {
+  if (n && !d) return MFSDP_EINVAL;
+  uint64_t end[2] = {0, 0};
+  for (size_t i = 0; i < n; ++i) {
+    if (d[i].role > 1) return MFSDP_EINVAL;
+    end[d[i].role] = std::max(end[d[i].role],
+                              align_up(d[i].elem_off + (uint64_t)d[i].rows * d[i].cols, MFSDP_SEG_ALIGN));
+  }
+  if (mat) *mat = end[0];
+  if (tail) *tail = end[1];
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int world, int policy, int metric,
+                          int rank, int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
+                          mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out) {
+  if ((n_params && !params) || world < 1 || rank >= world || !n_desc) return MFSDP_EINVAL;
+  if (policy != MFSDP_POLICY_ROLE_GREEDY && policy != MFSDP_POLICY_SCOPE_GREEDY) return MFSDP_EINVAL;
+  if (metric != MFSDP_METRIC_NUMEL && metric != MFSDP_METRIC_NS_FLOPS) return MFSDP_EINVAL;
+
+  std::vector<Role> roles;
+  int rc = build_roles(params, n_params, roles);
+  if (rc) return rc;
+
+  std::vector<int32_t> owner(roles.size(), -1);
+  std::vector<uint64_t> loads[2] = {std::vector<uint64_t>((size_t)world, 0), std::vector<uint64_t>((size_t)world, 0)};
+  std::vector<uint32_t> ids;
+  if (policy == MFSDP_POLICY_ROLE_GREEDY) {           // line 2: per block, carry loads forward
+    size_t i = 0;
+    while (i < roles.size()) {
+      ids.clear();
+      const uint32_t blk = roles[i].block;
+      while (i < roles.size() && roles[i].block == blk) ids.push_back((uint32_t)i++);
+      greedy(ids, roles, metric, world, loads, owner);
+    }
+  } else {                                            // line 3: pool all roles
+    ids.resize(roles.size());
+    for (size_t i = 0; i < roles.size(); ++i) ids[i] = (uint32_t)i;
+    greedy(ids, roles, metric, world, loads, owner);
+  }
+
+  if (rank < 0) {                                     // P6: heaviest by primary load, ties -> lowest id
+    rank = 0;
+    for (int r = 1; r < world; ++r) if (loads[0][r] > loads[0][rank]) rank = r;
+  }
+
+  // Emit the chosen rank's layout in (block, parameter) order = role order (line 5).
+  std::vector<mfsdp_desc_t> out;
+  uint64_t off[2] = {0, 0};
+  for (size_t i = 0; i < roles.size(); ++i) {
+    if (owner[i] != rank) continue;
+    const Role& r = roles[i];
+    mfsdp_desc_t d;
+    std::memset(&d, 0, sizeof d);
+    d.role = r.kind; d.param_id = r.first; d.block_id = r.block; d.rows = r.rows; d.cols = r.cols;
+    d.dtype = r.dtype;
+    d.flags = (r.kind == MFSDP_ROLE_MATRIX && r.rows > r.cols) ? MFSDP_DESC_TRANSPOSED : 0u;
+    d.elem_off = off[r.kind];
+    off[r.kind] = align_up(off[r.kind] + r.numel, MFSDP_SEG_ALIGN);
+    out.push_back(d);
+  }
+  rc = mfsdp_validate_desc(out.data(), out.size());
+  if (rc) return MFSDP_ELAYOUT;
+
+  if (n_roles) *n_roles = roles.size();
+  if (rank_out) *rank_out = rank;
+  if (owner_out) for (size_t i = 0; i < roles.size(); ++i) owner_out[i] = owner[i];
+  if (rank_load_out)
+    for (int r = 0; r < world; ++r) { rank_load_out[r] = loads[0][r]; rank_load_out[world + r] = loads[1][r]; }
+  *n_desc = out.size();
+  if (desc_out) {
+    if (desc_cap < out.size()) return MFSDP_ECAP;
+    if (!out.empty()) std::memcpy(desc_out, out.data(), out.size() * sizeof(mfsdp_desc_t));
+  }
+  return MFSDP_OK;
+}
