@@ -1,0 +1,272 @@
+"""ctypes marshalling for libmfsdp.so.  Same names as include/mfsdp.h; no arithmetic of the method lives here."""
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+PKG = os.path.dirname(os.path.abspath(__file__))
+
+BF16, F32 = 0, 1
+ROLE_MATRIX, ROLE_TAIL = 0, 1
+POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY = 0, 1
+METRIC_NUMEL, METRIC_NS_FLOPS = 0, 1
+SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE = 0, 1, 2
+NS_BF16, NS_FP32 = 0, 1
+OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA = 0, -1, -2, -3, -4, -5
+
+
+class Param(C.Structure):            # mfsdp_param_t
+    _fields_ = [("block_id", C.c_uint32), ("ndim", C.c_uint32), ("rows", C.c_uint32), ("cols", C.c_uint32),
+                ("dtype", C.c_uint32), ("flags", C.c_uint32)]
+
+
+class Desc(C.Structure):             # mfsdp_desc_t
+    _fields_ = [("role", C.c_uint32), ("param_id", C.c_uint32), ("block_id", C.c_uint32), ("rows", C.c_uint32),
+                ("cols", C.c_uint32), ("dtype", C.c_uint32), ("flags", C.c_uint32), ("reserved", C.c_uint32),
+                ("elem_off", C.c_uint64)]
+
+    def as_dict(self):
+        return dict(role=self.role, param_id=self.param_id, block_id=self.block_id, rows=self.rows, cols=self.cols,
+                    dtype=self.dtype, flags=self.flags, elem_off=self.elem_off)
+
+
+class MuonHParams(C.Structure):      # mfsdp_muon_hparams_t
+    _fields_ = [("lr", C.c_double), ("weight_decay", C.c_double), ("momentum", C.c_double), ("a", C.c_double),
+                ("b", C.c_double), ("c", C.c_double), ("eps", C.c_double), ("nesterov", C.c_int32),
+                ("ns_steps", C.c_int32), ("scale_mode", C.c_int32), ("precision", C.c_int32)]
+
+    def __init__(self, lr=0.02, weight_decay=0.01, momentum=0.95, a=3.4445, b=-4.7750, c=2.0315, eps=1e-7,
+                 nesterov=1, ns_steps=5, scale_mode=SCALE_MATCH_RMS_ADAMW, precision=NS_BF16):
+        super().__init__(lr, weight_decay, momentum, a, b, c, eps, int(nesterov), ns_steps, scale_mode, precision)
+
+
+class AdamWHParams(C.Structure):     # mfsdp_adamw_hparams_t
+    _fields_ = [("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("eps", C.c_double),
+                ("weight_decay", C.c_double), ("step", C.c_int64)]
+
+    def __init__(self, lr=1e-3, beta1=0.9, beta2=0.95, eps=1e-8, weight_decay=0.01, step=1):
+        super().__init__(lr, beta1, beta2, eps, weight_decay, step)
+
+
+class MfsdpError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        super().__init__("%s failed: %d (%s)" % (what, code, mfsdp_strerror(code)))
+
+
+@dataclass
+class PlanResult:
+    owner: list          # owner rank per role, roles in model order
+    n_roles: int
+    rank_load: list      # [2 * world]: primary loads then tail loads
+    desc: object         # ctypes array of Desc (the chosen rank's resident set)
+    rank: int
+
+
+_SYMBOLS = ["mfsdp_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
+            "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
+            "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
+            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count"]
+_lib = None
+
+
+def lib_path():
+    return os.path.join(PKG, "libmfsdp.so")
+
+
+def exported_symbols():
+    return list(_SYMBOLS)
+
+
+def load():
+    """dlopen libmfsdp.so (built in-tree by paper_2607_05895_b200.build).  Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise RuntimeError("libmfsdp.so is not built (%s); run `python -m paper_2607_05895_b200.build` -- there is "
+                           "no CPU fallback" % path)
+    lib = C.CDLL(path)
+    vp, sz, i32 = C.c_void_p, C.c_size_t, C.c_int
+    pD, pP = C.POINTER(Desc), C.POINTER(Param)
+    psz = C.POINTER(C.c_size_t)
+    lib.mfsdp_plan.argtypes = [pP, sz, i32, i32, i32, i32, C.POINTER(C.c_int32), psz, C.POINTER(C.c_uint64), pD, sz,
+                               psz, C.POINTER(C.c_int)]
+    lib.mfsdp_validate_desc.argtypes = [pD, sz]
+    lib.mfsdp_flat_elems.argtypes = [pD, sz, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    lib.mfsdp_workspace_bytes.argtypes = [pD, sz, i32, psz]
+    lib.mfsdp_workspace_view.argtypes = [pD, sz, i32, i32, sz, psz, psz, psz]
+    lib.mfsdp_debug_ws_offsets.argtypes = [pD, sz, i32, sz, psz]
+    pMH, pAH = C.POINTER(MuonHParams), C.POINTER(AdamWHParams)
+    lib.mfsdp_muon_step.argtypes = [pD, sz, vp, vp, vp, vp, sz, pMH, vp]
+    lib.mfsdp_muon_momentum_pass.argtypes = [pD, sz, vp, vp, vp, sz, pMH, vp]
+    lib.mfsdp_muon_ns_pass.argtypes = [pD, sz, vp, sz, pMH, vp]
+    lib.mfsdp_muon_update_pass.argtypes = [pD, sz, vp, vp, sz, pMH, vp]
+    lib.mfsdp_muon_step_host.argtypes = [pD, sz, vp, vp, vp, vp, vp, vp, i32, vp, sz, pMH, vp]
+    lib.mfsdp_adamw_tail_step.argtypes = [pD, sz, vp, vp, vp, vp, pAH, vp]
+    lib.mfsdp_strerror.argtypes = [i32]
+    lib.mfsdp_strerror.restype = C.c_char_p
+    lib.mfsdp_version.restype = i32
+    lib.mfsdp_launch_count.restype = C.c_uint64
+    for name in _SYMBOLS:
+        getattr(lib, name)          # AttributeError if the library does not export what the header declares
+    _lib = lib
+    return lib
+
+
+# ---- marshalling helpers ----------------------------------------------------------------------------------------
+def _ptr(x):
+    """Device/host pointer of a torch tensor, an int address, or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return C.c_void_p(x)
+    return C.c_void_p(x.data_ptr())
+
+
+def _nbytes(x):
+    return x.numel() * x.element_size()
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        if torch.cuda.is_available():
+            return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+        return None
+    if isinstance(stream, int):
+        return C.c_void_p(stream)
+    return C.c_void_p(stream.cuda_stream)
+
+
+def make_desc_array(desc):
+    """ctypes Desc array from a Desc array (returned as is), a list of Desc, or a list of dicts."""
+    if isinstance(desc, C.Array):
+        return desc
+    arr = (Desc * max(1, len(desc)))()
+    for i, d in enumerate(desc):
+        if isinstance(d, Desc):
+            arr[i] = d
+        else:
+            arr[i] = Desc(d["role"], d["param_id"], d["block_id"], d["rows"], d["cols"], d["dtype"], d["flags"], 0,
+                          d["elem_off"])
+    arr._n = len(desc)
+    return arr
+
+
+def _dn(desc):
+    arr = make_desc_array(desc)
+    return arr, getattr(arr, "_n", len(arr))
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise MfsdpError(rc, what)
+
+
+# ---- the C ABI, same names ----------------------------------------------------------------------------------------
+def mfsdp_strerror(code):
+    return load().mfsdp_strerror(code).decode()
+
+
+def mfsdp_version():
+    return load().mfsdp_version()
+
+
+def mfsdp_launch_count():
+    return int(load().mfsdp_launch_count())
+
+
+def mfsdp_plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0):
+    """params: list of (block_id, ndim, rows, cols, dtype, flags) tuples or Param.  Returns PlanResult."""
+    lib = load()
+    n = len(params)
+    arr = (Param * max(1, n))()
+    for i, p in enumerate(params):
+        arr[i] = p if isinstance(p, Param) else Param(*p)
+    n_roles, n_desc, rank_out = C.c_size_t(0), C.c_size_t(0), C.c_int(0)
+    rc = lib.mfsdp_plan(arr, n, world_size, policy, metric, rank, None, C.byref(n_roles), None, None, 0,
+                        C.byref(n_desc), C.byref(rank_out))
+    _check(rc, "mfsdp_plan(size query)")
+    owner = (C.c_int32 * max(1, n_roles.value))()
+    loads = (C.c_uint64 * (2 * world_size))()
+    desc = (Desc * max(1, n_desc.value))()
+    cap = n_desc.value
+    rc = lib.mfsdp_plan(arr, n, world_size, policy, metric, rank, owner, C.byref(n_roles), loads, desc, cap,
+                        C.byref(n_desc), C.byref(rank_out))
+    _check(rc, "mfsdp_plan")
+    desc._n = n_desc.value
+    return PlanResult(list(owner[:n_roles.value]), n_roles.value, list(loads), desc, rank_out.value)
+
+
+def mfsdp_validate_desc(desc):
+    arr, n = _dn(desc)
+    return load().mfsdp_validate_desc(arr, n)
+
+
+def mfsdp_flat_elems(desc):
+    arr, n = _dn(desc)
+    a, b = C.c_uint64(0), C.c_uint64(0)
+    _check(load().mfsdp_flat_elems(arr, n, C.byref(a), C.byref(b)), "mfsdp_flat_elems")
+    return a.value, b.value
+
+
+def mfsdp_workspace_bytes(desc, precision=NS_BF16):
+    arr, n = _dn(desc)
+    out = C.c_size_t(0)
+    _check(load().mfsdp_workspace_bytes(arr, n, precision, C.byref(out)), "mfsdp_workspace_bytes")
+    return out.value
+
+
+def mfsdp_workspace_view(desc, precision, ns_steps, index):
+    """(o_byte_off, o_pitch_elems, ssq_byte_off) of the index-th matrix descriptor."""
+    arr, n = _dn(desc)
+    a, b, c = C.c_size_t(0), C.c_size_t(0), C.c_size_t(0)
+    _check(load().mfsdp_workspace_view(arr, n, precision, ns_steps, index, C.byref(a), C.byref(b), C.byref(c)),
+           "mfsdp_workspace_view")
+    return a.value, b.value, c.value
+
+
+def mfsdp_debug_ws_offsets(desc, precision, index):
+    arr, n = _dn(desc)
+    out = (C.c_size_t * 6)()
+    _check(load().mfsdp_debug_ws_offsets(arr, n, precision, index, out), "mfsdp_debug_ws_offsets")
+    return list(out)
+
+
+def mfsdp_muon_step(desc, W, G, M, workspace, hp, stream=None):
+    arr, n = _dn(desc)
+    _check(load().mfsdp_muon_step(arr, n, _ptr(W), _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
+                                  C.byref(hp), _stream(stream)), "mfsdp_muon_step")
+
+
+def mfsdp_muon_momentum_pass(desc, G, M, workspace, hp, stream=None):
+    arr, n = _dn(desc)
+    _check(load().mfsdp_muon_momentum_pass(arr, n, _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
+                                           C.byref(hp), _stream(stream)), "mfsdp_muon_momentum_pass")
+
+
+def mfsdp_muon_ns_pass(desc, workspace, hp, stream=None):
+    arr, n = _dn(desc)
+    _check(load().mfsdp_muon_ns_pass(arr, n, _ptr(workspace), _nbytes(workspace), C.byref(hp), _stream(stream)),
+           "mfsdp_muon_ns_pass")
+
+
+def mfsdp_muon_update_pass(desc, W, workspace, hp, stream=None):
+    arr, n = _dn(desc)
+    _check(load().mfsdp_muon_update_pass(arr, n, _ptr(W), _ptr(workspace), _nbytes(workspace), C.byref(hp),
+                                         _stream(stream)), "mfsdp_muon_update_pass")
+
+
+def mfsdp_muon_step_host(desc, hW, hG, hM, dW, dG, dM, upload_state, workspace, hp, stream=None):
+    """HOST buffers hW/hG/hM (pinned torch CPU tensors), device staging dW/dG/dM.  Synchronises the stream."""
+    arr, n = _dn(desc)
+    _check(load().mfsdp_muon_step_host(arr, n, _ptr(hW), _ptr(hG), _ptr(hM), _ptr(dW), _ptr(dG), _ptr(dM),
+                                       int(upload_state), _ptr(workspace), _nbytes(workspace), C.byref(hp),
+                                       _stream(stream)), "mfsdp_muon_step_host")
+
+
+def mfsdp_adamw_tail_step(desc, P, G, m, v, hp, stream=None):
+    arr, n = _dn(desc)
+    _check(load().mfsdp_adamw_tail_step(arr, n, _ptr(P), _ptr(G), _ptr(m), _ptr(v), C.byref(hp), _stream(stream)),
+           "mfsdp_adamw_tail_step")

@@ -18,6 +18,13 @@ def pytest_collection_modifyitems(config, items):
     pass
 
 
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """Build libmfsdp.so in-tree if it is missing or stale (nvcc cross-compiles without a GPU)."""
+    from paper_2607_05895_b200 import build as _build
+    _build.build()
+
+
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")

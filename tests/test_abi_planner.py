@@ -1,0 +1,164 @@
+"""Host-side checks that need no GPU: the C-ABI library loads and exports every symbol include/mfsdp.h declares,
+the host planner (mfsdp_plan, C++) matches the oracle planner BIT-EXACTLY, layout validation, workspace sizing and
+error codes.  No compute entry point is exercised beyond its argument checks."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2607_05895_b200 as mf
+import workloads
+from oracle import planner as oplan
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "mfsdp.h")).read()
+    declared = set(re.findall(r"\b(mfsdp_[a-z_0-9]+)\s*\(", header))
+    assert declared, "no declarations found in mfsdp.h"
+    lib = ctypes.CDLL(mf.lib_path())
+    for name in sorted(declared):
+        assert hasattr(lib, name), "libmfsdp.so does not export %s" % name
+    assert declared == set(mf.exported_symbols()), "binding and header disagree on the entry points"
+    assert mf.mfsdp_version() == 1
+
+
+def test_struct_sizes_match_header_layout():
+    assert ctypes.sizeof(mf.Param) == 24
+    assert ctypes.sizeof(mf.Desc) == 40
+    assert ctypes.sizeof(mf.MuonHParams) == 7 * 8 + 4 * 4
+    assert ctypes.sizeof(mf.AdamWHParams) == 5 * 8 + 8
+
+
+def _compare_plan(params, world, policy, metric, rank):
+    want = oplan.plan(params, world, policy, metric, rank)
+    got = mf.mfsdp_plan(params, world, policy, metric, rank)
+    assert got.n_roles == len(want["roles"])
+    assert got.owner == want["owner"]
+    assert got.rank == want["rank"]
+    assert got.rank_load[:world] == want["loads"][0]
+    assert got.rank_load[world:] == want["loads"][1]
+    gd = [got.desc[i].as_dict() for i in range(got.desc._n)]
+    assert gd == want["desc"]
+    return got, want
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4", "c5", "small"])
+@pytest.mark.parametrize("policy", [mf.POLICY_ROLE_GREEDY, mf.POLICY_SCOPE_GREEDY])
+@pytest.mark.parametrize("metric", [mf.METRIC_NUMEL, mf.METRIC_NS_FLOPS])
+def test_planner_matches_oracle_bit_exact_on_configs(name, policy, metric):
+    wl = workloads.get(name)
+    ranks = sorted({0, wl.world - 1, -1, wl.world // 2})
+    for rank in ranks:
+        _compare_plan(wl.params, wl.world, policy, metric, rank)
+
+
+def test_planner_matches_oracle_on_random_models():
+    rng = np.random.default_rng(123)
+    for trial in range(200):
+        n_blocks = int(rng.integers(1, 6))
+        params = []
+        for b in range(n_blocks):
+            for _ in range(int(rng.integers(0, 6))):
+                if rng.random() < 0.6:
+                    params.append((b, 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)), 0, int(rng.random() < 0.1)))
+                else:
+                    params.append((b, 1, int(rng.integers(1, 300)), 1, 0, int(rng.random() < 0.1)))
+        world = int(rng.integers(1, 7))
+        policy = int(rng.integers(0, 2))
+        metric = int(rng.integers(0, 2))
+        rank = int(rng.integers(-1, world))
+        _compare_plan(params, world, policy, metric, rank)
+
+
+def test_configured_resident_sets():
+    """The sets bench.py and the GPU tests run (regenerated, not trusted from the survey)."""
+    wl = workloads.get("c2")
+    got, _ = _compare_plan(wl.params, wl.world, wl.policy, wl.metric, wl.rank)
+    assert sum(1 for i in range(got.desc._n) if got.desc[i].role == mf.ROLE_MATRIX) == 48
+    assert sum(1 for i in range(got.desc._n) if got.desc[i].role == mf.ROLE_TAIL) == 12
+    wl = workloads.get("c5")
+    got, want = _compare_plan(wl.params, wl.world, wl.policy, wl.metric, wl.rank)
+    loads = want["loads"][0]
+    assert loads[got.rank] == max(loads)
+    assert 1.0 <= oplan.balance(loads) <= 1.4          # PAPER.md:174, 219-222 sanity range
+    wl = workloads.get("c4")
+    got, want = _compare_plan(wl.params, wl.world, wl.policy, wl.metric, wl.rank)
+    assert 1.0 <= oplan.balance(want["loads"][0]) <= 1.4
+
+
+def test_plan_errors_and_size_query():
+    lib = mf.load()
+    n_desc = ctypes.c_size_t(0)
+    P = (mf.Param * 2)(mf.Param(0, 2, 4, 4, 0, 0), mf.Param(0, 2, 8, 4, 0, 0))
+    assert lib.mfsdp_plan(P, 2, 0, 0, 0, 0, None, None, None, None, 0, ctypes.byref(n_desc), None) == mf.EINVAL
+    assert lib.mfsdp_plan(P, 2, 2, 0, 0, 2, None, None, None, None, 0, ctypes.byref(n_desc), None) == mf.EINVAL
+    assert lib.mfsdp_plan(P, 2, 1, 7, 0, 0, None, None, None, None, 0, ctypes.byref(n_desc), None) == mf.EINVAL
+    assert lib.mfsdp_plan(P, 2, 1, 0, 0, 0, None, None, None, None, 0, ctypes.byref(n_desc), None) == 0
+    assert n_desc.value == 2
+    D = (mf.Desc * 1)()
+    assert lib.mfsdp_plan(P, 2, 1, 0, 0, 0, None, None, None, D, 1, ctypes.byref(n_desc), None) == mf.ECAP
+    assert n_desc.value == 2
+    bad = (mf.Param * 2)(mf.Param(1, 2, 4, 4, 0, 0), mf.Param(0, 2, 8, 4, 0, 0))      # decreasing block ids
+    assert lib.mfsdp_plan(bad, 2, 1, 0, 0, 0, None, None, None, None, 0, ctypes.byref(n_desc), None) == mf.EINVAL
+    zero = (mf.Param * 1)(mf.Param(0, 2, 0, 4, 0, 0))
+    assert lib.mfsdp_plan(zero, 1, 1, 0, 0, 0, None, None, None, None, 0, ctypes.byref(n_desc), None) == mf.EINVAL
+
+
+def test_validate_desc_rejects_bad_layouts():
+    good = [dict(role=0, param_id=0, block_id=0, rows=8, cols=16, dtype=0, flags=0, elem_off=0),
+            dict(role=0, param_id=1, block_id=0, rows=16, cols=8, dtype=0, flags=1, elem_off=128),
+            dict(role=1, param_id=2, block_id=0, rows=5, cols=1, dtype=0, flags=0, elem_off=0)]
+    assert mf.mfsdp_validate_desc(good) == 0
+    overlap = [dict(good[0]), dict(good[1], elem_off=64)]
+    assert mf.mfsdp_validate_desc(overlap) == mf.ELAYOUT
+    misaligned = [dict(good[0], elem_off=8)]
+    assert mf.mfsdp_validate_desc(misaligned) == mf.ELAYOUT
+    wrong_flag = [dict(good[1], flags=0, elem_off=0)]
+    assert mf.mfsdp_validate_desc(wrong_flag) == mf.ELAYOUT
+    assert mf.mfsdp_flat_elems(good) == (256, 64)
+
+
+def test_workspace_sizing_is_consistent():
+    wl = workloads.get("small")
+    pr = mf.mfsdp_plan(wl.params, 1)
+    for prec, es in ((mf.NS_BF16, 2), (mf.NS_FP32, 4)):
+        total = mf.mfsdp_workspace_bytes(pr.desc, prec)
+        n_mat = sum(1 for i in range(pr.desc._n) if pr.desc[i].role == mf.ROLE_MATRIX)
+        spans = []
+        for i in range(n_mat):
+            x0, x1, a, p, px, pa = mf.mfsdp_debug_ws_offsets(pr.desc, prec, i)
+            d = [pr.desc[j] for j in range(pr.desc._n) if pr.desc[j].role == mf.ROLE_MATRIX][i]
+            dmin = min(d.rows, d.cols)
+            assert px >= d.cols and pa >= dmin and px % 8 == 0 and pa % 8 == 0
+            for off, nbytes in ((x0, d.rows * px * es), (x1, d.rows * px * es), (a, dmin * pa * es), (p, dmin * pa * es)):
+                assert off % 1024 == 0 and off + nbytes <= total
+                spans.append((off, off + nbytes))
+            o_off, o_pitch, ssq_off = mf.mfsdp_workspace_view(pr.desc, prec, 5, i)
+            assert o_off == x1 and o_pitch == px and ssq_off == 8 * i          # K = 5 -> O in X buffer 1
+        spans.sort()
+        for (a0, a1), (b0, b1) in zip(spans, spans[1:]):
+            assert a1 <= b0, "workspace buffers overlap"
+
+
+def test_step_entry_points_reject_bad_arguments_without_a_gpu():
+    """Argument checks run before any CUDA call; with valid arguments and no device the answer is MFSDP_EARCH."""
+    lib = mf.load()
+    wl = workloads.get("c1")
+    pr = mf.mfsdp_plan(wl.params, 1)
+    hp = mf.MuonHParams(precision=mf.NS_FP32)
+    n = pr.desc._n
+    assert lib.mfsdp_muon_step(pr.desc, n, None, None, None, None, 0, ctypes.byref(hp), None) == mf.EINVAL
+    assert lib.mfsdp_muon_step(pr.desc, n, 1024, 1024, 1024, 1024, 0, None, None) == mf.EINVAL
+    bad = mf.MuonHParams(ns_steps=0)
+    assert lib.mfsdp_muon_step(pr.desc, n, 1024, 1024, 1024, 1024, 1 << 30, ctypes.byref(bad), None) == mf.EINVAL
+    ah = mf.AdamWHParams(step=0)
+    assert lib.mfsdp_adamw_tail_step(pr.desc, n, 1024, 1024, 1024, 1024, ctypes.byref(ah), None) == mf.EINVAL
+    import torch
+    if not torch.cuda.is_available():
+        rc = lib.mfsdp_muon_step(pr.desc, n, 1024, 1024, 1024, 1024, 1 << 30, ctypes.byref(hp), None)
+        assert rc == mf.EARCH, "no device must mean MFSDP_EARCH, never a CPU fallback"
+        assert "no CPU fallback" in mf.mfsdp_strerror(mf.EARCH)

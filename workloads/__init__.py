@@ -1,0 +1,169 @@
+"""Seeded synthetic owner sets (BASELINE.json configs C1..C5) -- the ONLY module shared by the oracle side and the
+CUDA side.  It holds none of the method's arithmetic: it lists parameter shapes and draws input tensors.
+
+What stands in for what: the paper measures on Qwen-style decoder shapes and a 12-layer
+GPT-2-vocabulary LM trained on a token stream; neither data nor weights are needed for an
+optimizer step, whose cost depends only on shapes and dtypes.  BASELINE.json's five owner sets stand in for the
+paper's models, and seeded Gaussian tensors (weights std 0.02; gradients std 1e-3 with a per-row lognormal(0, 0.5)
+scale to mimic heavy-tailed row norms) stand in for training tensors.
+
+Generator: numpy Philox, key = (seed, 4 * tensor_id + kind), counter offset = step; fp32 normals, rounded RNE to the
+storage dtype by torch.  Both sides consume the stored bytes, so libm differences cannot matter.
+
+A parameter record is the tuple (block_id, ndim, rows, cols, dtype, flags) of oracle.planner / mfsdp_param_t.
+"""
+from concurrent.futures import ThreadPoolExecutor
+from dataclasses import dataclass, field
+
+import numpy as np
+import torch
+
+BF16, F32 = 0, 1
+ROLE_MATRIX, ROLE_TAIL = 0, 1
+POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY = 0, 1
+METRIC_NUMEL, METRIC_NS_FLOPS = 0, 1
+NS_BF16, NS_FP32 = 0, 1
+KIND_W, KIND_G, KIND_ROWSCALE, KIND_SHAPE = 0, 1, 2, 3
+
+TORCH_DTYPE = {BF16: torch.bfloat16, F32: torch.float32}
+
+
+@dataclass
+class Workload:
+    name: str
+    params: list                      # [(block_id, ndim, rows, cols, dtype, flags)]
+    seed: int
+    world: int = 1
+    policy: int = POLICY_ROLE_GREEDY
+    metric: int = METRIC_NUMEL
+    rank: int = 0                     # -1 = heaviest
+    steps: int = 1
+    precision: int = NS_BF16
+    dtype: int = BF16
+    row_lognormal: bool = True        # gradients carry a per-row lognormal(0, 0.5) scale
+    muon: dict = field(default_factory=lambda: dict(lr=0.02, weight_decay=0.01, momentum=0.95, nesterov=1,
+                                                    ns_steps=5, a=3.4445, b=-4.7750, c=2.0315, eps=1e-7,
+                                                    scale_mode=0))
+    adamw: dict = field(default_factory=lambda: dict(lr=1e-3, beta1=0.9, beta2=0.95, eps=1e-8, weight_decay=0.01))
+
+
+def _layers(n_layers, mats, tails, dtype):
+    p = []
+    for blk in range(n_layers):
+        for rows, cols in mats:
+            p.append((blk, 2, rows, cols, dtype, 0))
+        for n in tails:
+            p.append((blk, 1, n, 1, dtype, 0))
+    return p
+
+
+def c1_tiny():
+    """C1: 256x256 and 256x1024 fp32 matrices + one 1-D tail of 1024; NS in fp32; plain Gaussian gradients."""
+    params = [(0, 2, 256, 256, F32, 0), (0, 2, 256, 1024, F32, 0), (0, 1, 1024, 1, F32, 0)]
+    return Workload("c1_tiny", params, seed=0, precision=NS_FP32, dtype=F32, row_lognormal=False)
+
+
+def c2_gpt2_small():
+    """C2: 12 layers x {768x2304, 768x768, 768x3072, 3072x768} bf16, world 1; tails: 6 x 768 + 1 x 3072 per layer."""
+    mats = [(768, 2304), (768, 768), (768, 3072), (3072, 768)]
+    tails = [768, 768, 768, 768, 768, 3072, 768]
+    return Workload("c2_gpt2_small", _layers(12, mats, tails, BF16), seed=1, steps=10)
+
+
+def c3_ragged(n=512):
+    """C3: 512 bf16 matrices, rows and cols independently uniform on {64,128,192,256,384,512}; one block each."""
+    vals = (64, 128, 192, 256, 384, 512)
+    rng = np.random.Generator(np.random.Philox(key=[2, KIND_SHAPE]))
+    draws = rng.integers(0, 6, size=(n, 2))
+    params = [(i, 2, vals[int(draws[i, 0])], vals[int(draws[i, 1])], BF16, 0) for i in range(n)]
+    return Workload("c3_ragged", params, seed=2, row_lognormal=False)
+
+
+def c4_llama8b():
+    """C4: Llama-3-8B shapes, 32 layers, two RMSNorm tails of 4096 per layer; 8 ranks, NS-flops greedy, rank 0."""
+    mats = [(4096, 4096), (1024, 4096), (1024, 4096), (4096, 4096), (14336, 4096), (14336, 4096), (4096, 14336)]
+    return Workload("c4_llama8b_rank0of8", _layers(32, mats, [4096, 4096], BF16), seed=3, world=8,
+                    metric=METRIC_NS_FLOPS, rank=0)
+
+
+def c5_llama70b():
+    """C5: Llama-3-70B shapes, 80 layers, two RMSNorm tails of 8192 per layer; 64 ranks, NS-flops greedy, heaviest."""
+    mats = [(8192, 8192), (1024, 8192), (1024, 8192), (8192, 8192), (28672, 8192), (28672, 8192), (8192, 28672)]
+    return Workload("c5_llama70b_heaviestof64", _layers(80, mats, [8192, 8192], BF16), seed=4, world=64,
+                    metric=METRIC_NS_FLOPS, rank=-1)
+
+
+def small_ragged(seed=7, dtype=BF16, precision=NS_BF16):
+    """Parity-test set the oracle finishes in seconds: several tiles, ragged tails, wide / tall / square, odd pitches."""
+    shapes = [(320, 200), (200, 320), (130, 130), (64, 520), (520, 64), (384, 384), (72, 1000), (257, 129), (8, 24)]
+    params = [(i // 3, 2, r, c, dtype, 0) for i, (r, c) in enumerate(shapes)]
+    params += [(0, 1, 1000, 1, dtype, 0), (0, 1, 7, 1, dtype, 0), (2, 1, 4099, 1, dtype, 0)]
+    params.sort(key=lambda p: p[0])
+    return Workload("small_ragged", params, seed=seed, precision=precision, dtype=dtype)
+
+
+CONFIGS = {"c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
+           "small": small_ragged}
+
+
+def get(name):
+    return CONFIGS[name]()
+
+
+# ---- tensors -----------------------------------------------------------------------------------------------------
+def _rng(seed, tensor_id, kind, step):
+    return np.random.Generator(np.random.Philox(key=[seed, 4 * tensor_id + kind], counter=[0, 0, 0, step]))
+
+
+def _normal(seed, tensor_id, kind, step, n):
+    return _rng(seed, tensor_id, kind, step).standard_normal(n, dtype=np.float32)
+
+
+def weight(wl, tensor_id, rows, cols):
+    """W ~ N(0, 0.02), fp32 values before storage rounding, shape (rows, cols)."""
+    return (np.float32(0.02) * _normal(wl.seed, tensor_id, KIND_W, 0, rows * cols)).reshape(rows, cols)
+
+
+def gradient(wl, tensor_id, rows, cols, step, is_tail=False):
+    """G ~ N(0, 1e-3), times exp(0.5 xi_row) per stored row when the workload says so (never for tails)."""
+    g = (np.float32(1e-3) * _normal(wl.seed, tensor_id, KIND_G, step, rows * cols)).reshape(rows, cols)
+    if wl.row_lognormal and not is_tail:
+        xi = _normal(wl.seed, tensor_id, KIND_ROWSCALE, step, rows)
+        g *= np.exp(np.float32(0.5) * xi)[:, None]
+    return g
+
+
+def _fields(d):
+    if isinstance(d, dict):
+        return d["role"], d["param_id"], d["rows"], d["cols"], d["elem_off"]
+    return d.role, d.param_id, d.rows, d.cols, d.elem_off
+
+
+def flat_elems(desc):
+    end = [0, 0]
+    for d in desc:
+        role, _, rows, cols, off = _fields(d)
+        end[role] = max(end[role], (off + rows * cols + 63) // 64 * 64)
+    return end[0], end[1]
+
+
+def fill_flat(wl, desc, kind, step=0, role=ROLE_MATRIX, dtype=None, pin=False, threads=8):
+    """Rank-flat CPU tensor (storage dtype) of `kind` (KIND_W / KIND_G) for all descriptors of `role`;
+    gaps between segments are zero."""
+    n = flat_elems(desc)[role]
+    tdt = TORCH_DTYPE[wl.dtype if dtype is None else dtype]
+    out = torch.zeros(max(n, 1), dtype=tdt, pin_memory=pin)[:n]
+
+    def one(d):
+        r, pid, rows, cols, off = _fields(d)
+        if r != role:
+            return
+        if kind == KIND_W:
+            a = weight(wl, pid, rows, cols)
+        else:
+            a = gradient(wl, pid, rows, cols, step, is_tail=(role == ROLE_TAIL))
+        out[off:off + rows * cols] = torch.from_numpy(a.reshape(-1)).to(tdt)   # RNE to the storage dtype
+
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        list(ex.map(one, list(desc)))
+    return out
