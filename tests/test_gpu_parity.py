@@ -1,0 +1,215 @@
+"""GPU parity tests proper (`-m gpu`): the CUDA path, called through the C ABI, against the fp64 oracle on the same
+seeded inputs, element by element.  Sizes here are ones the oracle finishes in seconds yet span several 128-wide
+tiles, ragged tails, wide / tall / square matrices.  Tolerances are BASELINE.json's: relF(O) <= 3e-2 (bf16 mode),
+<= 1e-4 (fp32 mode), <= 1e-6 on momentum / AdamW state; the update is checked lock-step."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2607_05895_b200 as mf
+import workloads
+from oracle import adamw as oadamw
+from oracle import muon as omuon
+
+import gpu_harness as gh
+from helpers import bf16_rne, bf16_ulp_distance, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+
+def _snapshot(sess):
+    W_old = [sess.seg64(sess.W, d) for d in sess.mats]
+    M_old = [sess.seg64(sess.M, d) for d in sess.mats]
+    return W_old, M_old
+
+
+def _full_step_check(wl, precision=None, hp_over=None, tol_o=None):
+    sess = gh.Session(wl, precision=precision, hp_over=hp_over)
+    sess.load_grads(0)
+    W_old, M_old = _snapshot(sess)
+    sess.muon_step()
+    errs = []
+    for i in range(len(sess.mats)):
+        eo, em = gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i], tol_o=tol_o)
+        errs.append(eo)
+    return sess, errs
+
+
+# ---- a1 / a2: momentum pass --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [mf.BF16, mf.F32])
+@pytest.mark.parametrize("precision", [mf.NS_BF16, mf.NS_FP32])
+@pytest.mark.parametrize("nesterov", [1, 0])
+def test_momentum_pass_matches_oracle(dtype, precision, nesterov):
+    wl = workloads.small_ragged(dtype=dtype, precision=precision)
+    sess = gh.Session(wl, hp_over=dict(nesterov=nesterov))
+    for step in range(3):                         # three consecutive steps: the EMA state carries over
+        sess.load_grads(step)
+        M_old = [sess.seg64(sess.M, d) for d in sess.mats]
+        mf.mfsdp_muon_momentum_pass(sess.desc, sess.G, sess.M, sess.ws, sess.hp)
+        torch.cuda.synchronize()
+        for i, d in enumerate(sess.mats):
+            G = sess.seg(sess.hG, d).to(torch.float64).numpy()
+            M_ref, U_ref = omuon.momentum_update(M_old[i], G, sess.hp.momentum, bool(nesterov))
+            assert rel_fro(sess.seg64(sess.M, d), M_ref) <= gh.TOL_STATE
+            ssq = sess.read_ssq(i)
+            want = float(np.sum(U_ref * U_ref))
+            assert abs(ssq - want) <= gh.TOL_STATE * want
+            x0, _, _, _, px, _ = mf.mfsdp_debug_ws_offsets(sess.desc, sess.precision, i)
+            Xt = sess.ws_matrix(x0, d.rows, d.cols, px)
+            tol = 2.0 ** -8 if precision == mf.NS_BF16 else 1e-6      # X~ = cast(U): one rounding
+            assert np.abs(Xt - U_ref).max() <= tol * np.abs(U_ref).max()
+            assert rel_fro(Xt, U_ref) <= (3e-3 if precision == mf.NS_BF16 else 1e-6)
+
+
+# ---- a5: AdamW on tails ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [mf.BF16, mf.F32])
+def test_adamw_tail_matches_oracle(dtype):
+    wl = workloads.small_ragged(dtype=dtype)
+    sess = gh.Session(wl)
+    assert len(sess.tails) >= 2
+    m_ref = [np.zeros(d.rows) for d in sess.tails]
+    v_ref = [np.zeros(d.rows) for d in sess.tails]
+    for t in (1, 2, 3):
+        sess.load_grads(t - 1)
+        P_old = [sess.seg64(sess.P, d).reshape(-1) for d in sess.tails]
+        m_old = [sess.seg64(sess.m, d).reshape(-1) for d in sess.tails]
+        v_old = [sess.seg64(sess.v, d).reshape(-1) for d in sess.tails]
+        sess.adamw_step(t)
+        # free-running oracle state (from zero) and lock-step oracle (from the GPU's previous state)
+        for j, d in enumerate(sess.tails):
+            g = sess.seg(sess.hGt, d).to(torch.float64).numpy().reshape(-1)
+            _, m_ref[j], v_ref[j] = oadamw.adamw_step(P_old[j], g, m_ref[j], v_ref[j], t, **wl.adamw)
+            p_l, m_l, v_l = oadamw.adamw_step(P_old[j], g, m_old[j], v_old[j], t, **wl.adamw)
+            m_gpu, v_gpu = sess.seg64(sess.m, d).reshape(-1), sess.seg64(sess.v, d).reshape(-1)
+            p_gpu = sess.seg64(sess.P, d).reshape(-1)
+            assert rel_fro(m_gpu, m_ref[j]) <= gh.TOL_STATE and rel_fro(v_gpu, v_ref[j]) <= gh.TOL_STATE
+            assert rel_fro(m_gpu, m_l) <= gh.TOL_STATE and rel_fro(v_gpu, v_l) <= gh.TOL_STATE
+            if dtype == mf.F32:
+                assert rel_fro(p_gpu, p_l) <= gh.TOL_STATE
+            else:
+                ulps = bf16_ulp_distance(p_gpu, bf16_rne(p_l))
+                assert ulps.max() <= 1 and (ulps > 0).mean() <= 2e-3
+
+
+def test_adamw_ignores_matrices_and_muon_ignores_tails():
+    """Routing: each entry point touches only its own role's element space."""
+    wl = workloads.small_ragged()
+    sess = gh.Session(wl)
+    sess.load_grads(0)
+    W0, P0 = sess.W.clone(), sess.P.clone()
+    sess.adamw_step(1)
+    assert torch.equal(sess.W, W0) and not torch.equal(sess.P, P0)
+    P1 = sess.P.clone()
+    sess.muon_step()
+    assert torch.equal(sess.P, P1) and not torch.equal(sess.W, W0)
+
+
+# ---- a3: Newton-Schulz, fp32 mode -----------------------------------------------------------------------------------------
+def test_c1_fp32_mode_full_step():
+    """BASELINE.json config 1 exactly: fp32 W/G, NS in fp32, lr 0.02, wd 0.01, + AdamW on the tail."""
+    wl = workloads.get("c1")
+    sess, errs = _full_step_check(wl)
+    assert max(errs) <= 1e-4
+    sess.adamw_step(1)
+
+
+def test_c1_original_scale_mode():
+    wl = workloads.get("c1")
+    _full_step_check(wl, hp_over=dict(scale_mode=mf.SCALE_ORIGINAL))
+
+
+@pytest.mark.parametrize("dtype", [mf.BF16, mf.F32])
+def test_small_ragged_fp32_mode(dtype):
+    wl = workloads.small_ragged(dtype=dtype, precision=mf.NS_FP32)
+    _full_step_check(wl)
+
+
+# ---- a3: Newton-Schulz, bf16 tensor-core mode --------------------------------------------------------------------------------
+def test_c1_bf16_mode_full_step():
+    wl = workloads.get("c1")
+    _, errs = _full_step_check(wl, precision=mf.NS_BF16)
+    assert max(errs) <= 3e-2
+
+
+@pytest.mark.parametrize("dtype", [mf.BF16, mf.F32])
+def test_small_ragged_bf16_mode(dtype):
+    wl = workloads.small_ragged(dtype=dtype, precision=mf.NS_BF16)
+    sess, errs = _full_step_check(wl)
+    rng = np.random.default_rng(5)
+    for i in range(len(sess.mats)):
+        gh.probe_last_iteration(sess, i, rng, 2e-2)
+
+
+@pytest.mark.parametrize("steps", [1, 2, 3])
+def test_ns_step_counts_bf16(steps):
+    """K is an argument (the paper's runs use K = 2); odd/even K end in different ping-pong buffers."""
+    wl = workloads.small_ragged()
+    _full_step_check(wl, hp_over=dict(ns_steps=steps))
+
+
+def test_zero_gradient_gives_zero_update_no_nan():
+    """Reading M3: zero gradient and zero momentum -> O = 0 exactly; W only decays."""
+    wl = workloads.small_ragged()
+    for precision in (mf.NS_BF16, mf.NS_FP32):
+        sess = gh.Session(wl, precision=precision)
+        sess.load_grads(0)
+        sess.G.zero_()
+        W_old = sess.W.clone()
+        sess.muon_step()
+        for i, d in enumerate(sess.mats):
+            O = sess.read_O(i)
+            assert np.all(O == 0.0)
+            assert sess.read_ssq(i) == 0.0
+        assert torch.isfinite(sess.W.float()).all()
+
+
+def test_run_to_run_determinism():
+    wl = workloads.small_ragged()
+    outs = []
+    for _ in range(2):
+        sess = gh.Session(wl)
+        sess.load_grads(0)
+        sess.muon_step()
+        outs.append((sess.W.clone(), sess.M.clone(), sess.ws.clone()))
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    for i in range(len(sess.mats)):
+        pass
+    o_off, pitch, _ = mf.mfsdp_workspace_view(sess.desc, sess.precision, sess.hp.ns_steps, 0)
+    d = sess.mats[0]
+    n = d.rows * pitch * 2
+    assert torch.equal(outs[0][2][o_off:o_off + n], outs[1][2][o_off:o_off + n])
+
+
+def test_separate_passes_equal_fused_step():
+    wl = workloads.small_ragged()
+    a = gh.Session(wl)
+    a.load_grads(0)
+    a.muon_step()
+    b = gh.Session(wl)
+    b.load_grads(0)
+    mf.mfsdp_muon_momentum_pass(b.desc, b.G, b.M, b.ws, b.hp)
+    mf.mfsdp_muon_ns_pass(b.desc, b.ws, b.hp)
+    mf.mfsdp_muon_update_pass(b.desc, b.W, b.ws, b.hp)
+    torch.cuda.synchronize()
+    assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M)
+
+
+def test_host_buffer_entry_point():
+    wl = workloads.small_ragged()
+    a = gh.Session(wl)
+    a.load_grads(0)
+    hW, hG = a.hW.clone().pin_memory(), a.hG.clone().pin_memory()
+    hM = torch.zeros(a.n_mat_el, dtype=torch.float32).pin_memory()
+    dW, dG, dM = torch.empty_like(a.W), torch.empty_like(a.G), torch.empty_like(a.M)
+    mf.mfsdp_muon_step_host(a.desc, hW, hG, hM, dW, dG, dM, 1, a.ws, a.hp)
+    a.muon_step()
+    assert torch.equal(hW, a.W.cpu()) and torch.equal(hM, a.M.cpu())
+
+
+def test_launch_counter_counts_kernels():
+    wl = workloads.small_ragged()
+    sess = gh.Session(wl)
+    sess.load_grads(0)
+    n0 = mf.mfsdp_launch_count()
+    sess.muon_step()
+    assert mf.mfsdp_launch_count() > n0
