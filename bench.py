@@ -214,6 +214,26 @@ def rank_order_by_load(mf, wl):
     return sorted(range(wl.world), key=lambda r: (-loads[r], r))
 
 
+def choose_plan_rank(order, wl_rank, rank, world):
+    """Which rank of the plan this process runs: at N = 1 the workload's own choice (heaviest when wl_rank < 0); at
+    N > 1 process r takes the r-th heaviest rank (independent resident sets, no collective on the data path)."""
+    if world > 1 or wl_rank < 0:
+        return order[rank % len(order)]
+    return wl_rank
+
+
+def reduce_over_ranks(ms, ms_e2e, f_alg, launches, world, device):
+    """MAX over ranks of the device times, SUM over ranks of flops and launches (the only collective: the report)."""
+    import torch
+    import torch.distributed as dist
+    stats = torch.tensor([ms, ms_e2e, float(f_alg), float(launches)], dtype=torch.float64, device=device)
+    if world > 1:
+        mx = stats.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = stats.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        return mx[0].item(), mx[1].item(), sm[2].item(), int(sm[3].item())
+    return ms, ms_e2e, float(f_alg), int(launches)
+
+
 def ev_time(torch, stream, fn, reps):
     """Mean device time (ms) of fn() over reps, CUDA events recorded on `stream`, synchronised on both sides."""
     torch.cuda.synchronize()
@@ -244,7 +264,7 @@ def run_ours(args):
 
     wl = workloads.get(args.config)
     order = rank_order_by_load(mf, wl)
-    plan_rank = order[rank % len(order)] if (world > 1 or wl.rank < 0) else wl.rank
+    plan_rank = choose_plan_rank(order, wl.rank, rank, world)
     pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, plan_rank)
     desc = pr.desc
     descs = [desc[i] for i in range(desc._n)]
@@ -329,15 +349,7 @@ def run_ours(args):
     b_upd = sum(elementwise_bytes(d.rows, d.cols, wbytes)["upd"] for d in mats)
     b_adam = sum(d.rows * d.cols for d in tails) * (3 * wbytes + 16)
 
-    # max over ranks / sums over ranks
-    stats = torch.tensor([ms, ms_e2e, float(f_alg), float(launches)],
-                         dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = stats.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = stats.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        ms_all, ms_e2e_all, f_all, launches_all = mx[0].item(), mx[1].item(), sm[2].item(), int(sm[3].item())
-    else:
-        ms_all, ms_e2e_all, f_all, launches_all = ms, stats[1].item(), float(f_alg), int(launches)
+    ms_all, ms_e2e_all, f_all, launches_all = reduce_over_ranks(ms, ms_e2e, f_alg, launches, world, "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

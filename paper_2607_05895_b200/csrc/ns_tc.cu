@@ -17,6 +17,7 @@
 #include <cuda_bf16.h>
 
 #include <algorithm>
+#include <cstdlib>
 
 #include "mfsdp_internal.h"
 #include "ptx_sm100.cuh"
@@ -29,7 +30,7 @@ struct TcMat {                 // device, one per matrix
   uint64_t x_off[2], a_off, p_off;
   uint32_t rows, cols, d, n_long, pitch_x, pitch_a, tall, pad;
 };
-struct TcTile { uint32_t mat, m0, n0, nkb; };   // output tile origin (rows, cols of the OUTPUT buffer), k blocks
+struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; };   // output tile origin (rows, cols of the OUTPUT buffer), k blocks, UMMA N (multiple of 64)
 
 struct NsTcPlan {
   CUtensorMap* d_tmaps = nullptr;   // 4 per matrix: X0, X1, A, P   (box 64 x 64 bf16, 128-byte swizzle)
@@ -88,8 +89,8 @@ __device__ __forceinline__ TileCfg decode(const TcParams& p, const TcTile& t, co
     c.out_rows = M.rows; c.out_cols = M.cols;
   }
   c.a_boxes = (a_ext - t.m0 > 64u) ? 2u : 1u;
-  const uint32_t rem = b_ext - t.n0;
-  c.n_valid = rem >= kBNMax ? kBNMax : ((rem + 63u) & ~63u);
+  (void)b_ext;
+  c.n_valid = t.nw;
   c.b_boxes = c.n_valid >> 6;
   return c;
 }
@@ -308,19 +309,38 @@ int make_tmap(CUtensorMap* out, void* base, uint32_t rows, uint32_t cols, uint32
   return r == CUDA_SUCCESS ? MFSDP_OK : cuda_fail(cudaErrorInvalidValue);
 }
 
-// Column-panel groups of `group` tiles are swept row-block by row-block so that concurrently running CTAs share
-// operand panels in L2.
+// Tile rasterisation.  The 148 CTAs walk the tile list round-robin, so at any moment ~148 consecutive list entries
+// are in flight and advance along k roughly in lock step; an operand box is fetched from DRAM once and served from
+// L2 to every in-flight tile that shares it.  The list is therefore ordered so that 148 consecutive tiles cover a
+// compact block of the output: `band` row blocks x the column tiles that go with them.
+int tune(const char* name, int dflt) {
+  const char* e = getenv(name);
+  return e && *e ? atoi(e) : dflt;
+}
+// rectangular output (APPLY): column panels of `group` tiles stay L2-resident while all row blocks sweep over them.
 void tiles_rect(std::vector<TcTile>& v, uint32_t mat, uint32_t out_rows, uint32_t out_cols, uint32_t nkb) {
   const uint32_t tm = (out_rows + kBM - 1) / kBM, tn = (out_cols + kBNMax - 1) / kBNMax;
-  const uint32_t group = 16;
+  const uint32_t group = (uint32_t)std::max(1, tune("MFSDP_TUNE_RECT_GROUP", 8));
   for (uint32_t g0 = 0; g0 < tn; g0 += group)
     for (uint32_t i = 0; i < tm; ++i)
-      for (uint32_t j = g0; j < std::min(tn, g0 + group); ++j) v.push_back(TcTile{mat, i * kBM, j * kBNMax, nkb});
+      for (uint32_t j = g0; j < std::min(tn, g0 + group); ++j) v.push_back(TcTile{mat, i * kBM, j * kBNMax, (uint16_t)nkb, (uint16_t)std::min(kBNMax, (out_cols - j * kBNMax + 63u) & ~63u)});
 }
+// symmetric output (GRAM, POLY): upper 128-row blocks only; bands of `band` row blocks, inside a band column-major
+// (all row blocks of the band for one 256-column step, then the next step).
 void tiles_sym(std::vector<TcTile>& v, uint32_t mat, uint32_t d, uint32_t nkb) {
   const uint32_t tm = (d + kBM - 1) / kBM;
-  for (uint32_t i = 0; i < tm; ++i)
-    for (uint32_t n0 = i * kBM; n0 < d; n0 += kBNMax) v.push_back(TcTile{mat, i * kBM, n0, nkb});
+  const uint32_t band = (uint32_t)std::max(1, tune("MFSDP_TUNE_SYM_BAND", 16));
+  for (uint32_t b0 = 0; b0 < tm; b0 += band) {
+    const uint32_t b1 = std::min(tm, b0 + band);
+    for (uint32_t c0 = b0 * kBM; c0 < d; c0 += kBNMax)          // 256-column steps from the band's first diagonal
+      for (uint32_t i = b0; i < b1; ++i) {
+        // row block i owns columns >= i * 128; clip the step to that range (N = 128 when only half of it is owned)
+        const uint32_t lo = std::max(c0, i * kBM);
+        const uint32_t hi = std::min(d, c0 + kBNMax);
+        if (lo >= hi) continue;
+        v.push_back(TcTile{mat, i * kBM, lo, (uint16_t)nkb, (uint16_t)((hi - lo + 63u) & ~63u)});
+      }
+  }
 }
 
 template <typename T>
