@@ -192,6 +192,22 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  * out[4] = X row pitch in elements, out[5] = A/P row pitch in elements. */
 int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t index, size_t out[6]);
 
+/* ---- tuning knobs (HOST) -------------------------------------------------------------------------------------
+ * Scheduling choices of the tensor-core Newton-Schulz path.  They change HOW tiles are formed and ordered, never
+ * what is computed (tests run the parity suite under several settings).  Setting a knob synchronises the device
+ * and drops the cached launch tables, which are rebuilt on the next step.  Initial values come from the
+ * environment variables of the same names, else the defaults below.
+ *   MFSDP_TUNE_PAIR_MIN_D   matrices with min(rows, cols) >= value run on CTA pairs (tcgen05 cta_group::2,
+ *                           256 x 256 tiles); smaller ones on single CTAs (128 x N tiles).  default 768
+ *   MFSDP_TUNE_SYM_BAND     row blocks per band of the symmetric (GRAM, POLY) tile order, single-CTA class.  16
+ *   MFSDP_TUNE_SYM_BAND2    the same for the CTA-pair class.  8
+ *   MFSDP_TUNE_RECT_GROUP   column tiles per panel of the rectangular (APPLY) tile order.  8
+ * Returns MFSDP_EINVAL for an unknown knob or value < 1; mfsdp_get_tune returns the value or a negative code. */
+enum { MFSDP_TUNE_PAIR_MIN_D = 0, MFSDP_TUNE_SYM_BAND = 1, MFSDP_TUNE_SYM_BAND2 = 2, MFSDP_TUNE_RECT_GROUP = 3,
+       MFSDP_TUNE_COUNT_ = 4 };
+int mfsdp_tune(int knob, int value);
+int mfsdp_get_tune(int knob);
+
 /* ---- misc ----------------------------------------------------------------------------------------------------- */
 const char* mfsdp_strerror(int code);      /* static string; for MFSDP_ECUDA the last CUDA error text            */
 int mfsdp_version(void);                   /* ABI version, currently 1                                            */

@@ -65,7 +65,7 @@ class PlanResult:
 _SYMBOLS = ["mfsdp_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
-            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count"]
+            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune"]
 _lib = None
 
 
@@ -108,6 +108,8 @@ def load():
     lib.mfsdp_strerror.restype = C.c_char_p
     lib.mfsdp_version.restype = i32
     lib.mfsdp_launch_count.restype = C.c_uint64
+    lib.mfsdp_tune.argtypes = [i32, i32]
+    lib.mfsdp_get_tune.argtypes = [i32]
     for name in _SYMBOLS:
         getattr(lib, name)          # AttributeError if the library does not export what the header declares
     _lib = lib
@@ -175,6 +177,20 @@ def mfsdp_version():
 
 def mfsdp_launch_count():
     return int(load().mfsdp_launch_count())
+
+
+TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP = 0, 1, 2, 3
+
+
+def mfsdp_tune(knob, value):
+    _check(load().mfsdp_tune(int(knob), int(value)), "mfsdp_tune")
+
+
+def mfsdp_get_tune(knob):
+    v = load().mfsdp_get_tune(int(knob))
+    if v < 0:
+        _check(v, "mfsdp_get_tune")
+    return v
 
 
 def mfsdp_plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0):

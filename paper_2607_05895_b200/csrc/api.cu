@@ -1,5 +1,6 @@
 // C-ABI entry points of the step (include/mfsdp.h): argument checks, workspace layout, the per-table cache of
 // device launch tables, and the launch sequence.  No compute happens here and there is no CPU fallback.
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -16,6 +17,28 @@ std::string g_cuda_err = "no CUDA error recorded";
 std::vector<Plan*> g_plans;
 std::vector<std::vector<uint8_t>> g_plan_keys;
 }  // namespace
+
+namespace {
+int g_tune[MFSDP_TUNE_COUNT_];
+bool g_tune_init = false;
+void tune_init() {
+  if (g_tune_init) return;
+  static const char* names[MFSDP_TUNE_COUNT_] = {"MFSDP_TUNE_PAIR_MIN_D", "MFSDP_TUNE_SYM_BAND",
+                                                 "MFSDP_TUNE_SYM_BAND2", "MFSDP_TUNE_RECT_GROUP"};
+  static const int dflt[MFSDP_TUNE_COUNT_] = {768, 16, 8, 8};
+  for (int k = 0; k < MFSDP_TUNE_COUNT_; ++k) {
+    const char* e = getenv(names[k]);
+    const int v = e && *e ? atoi(e) : 0;
+    g_tune[k] = v >= 1 ? v : dflt[k];
+  }
+  g_tune_init = true;
+}
+}  // namespace
+
+int tune_value(int knob) {
+  tune_init();
+  return knob >= 0 && knob < MFSDP_TUNE_COUNT_ ? g_tune[knob] : -1;
+}
 
 void count_launch(uint64_t n) { g_launches += n; }
 int cuda_fail(cudaError_t e) {
@@ -298,6 +321,27 @@ extern "C" int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, vo
   if (!P || !G || !m || !v || !aligned(P, 128) || !aligned(G, 128) || !aligned(m, 128) || !aligned(v, 128))
     return MFSDP_EINVAL;
   return launch_adamw(*pl, P, G, m, v, *hp, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int mfsdp_tune(int knob, int value) {
+  if (knob < 0 || knob >= MFSDP_TUNE_COUNT_ || value < 1) return MFSDP_EINVAL;
+  std::lock_guard<std::mutex> lock(g_mu);
+  tune_init();
+  if (g_tune[knob] == value) return MFSDP_OK;
+  g_tune[knob] = value;
+  bool any = false;
+  for (Plan* pl : g_plans) any |= pl->tc != nullptr;
+  if (any) {
+    cudaDeviceSynchronize();           // the tables may be in use by launches still in flight
+    for (Plan* pl : g_plans) { destroy_ns_tc(pl->tc); pl->tc = nullptr; }
+  }
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_get_tune(int knob) {
+  if (knob < 0 || knob >= MFSDP_TUNE_COUNT_) return MFSDP_EINVAL;
+  std::lock_guard<std::mutex> lock(g_mu);
+  return tune_value(knob);
 }
 
 extern "C" const char* mfsdp_strerror(int code) {

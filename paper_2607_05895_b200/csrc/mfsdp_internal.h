@@ -82,6 +82,8 @@ void count_launch(uint64_t n = 1);
 int cuda_fail(cudaError_t e);          // records the error text, returns MFSDP_ECUDA
 int check_last_launch();               // cudaGetLastError -> code
 
+int tune_value(int knob);               // current value of an MFSDP_TUNE_* knob
+
 inline uint64_t align_up_u64(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 
 }  // namespace mfsdp

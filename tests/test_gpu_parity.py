@@ -140,6 +140,38 @@ def test_small_ragged_bf16_mode(dtype):
         gh.probe_last_iteration(sess, i, rng, 2e-2)
 
 
+@pytest.fixture
+def pair_min_d():
+    """Sets MFSDP_TUNE_PAIR_MIN_D for one test (which matrices run on CTA pairs) and restores the default."""
+    old = mf.mfsdp_get_tune(mf.TUNE_PAIR_MIN_D)
+
+    def set_(v):
+        mf.mfsdp_tune(mf.TUNE_PAIR_MIN_D, v)
+    yield set_
+    mf.mfsdp_tune(mf.TUNE_PAIR_MIN_D, old)
+
+
+@pytest.mark.parametrize("min_d", [1, 100000])
+@pytest.mark.parametrize("wname", ["small", "medium"])
+def test_both_tile_classes_bf16(pair_min_d, wname, min_d):
+    """The same sets forced entirely onto CTA pairs (cta_group::2, 256 x 256 tiles, incl. the 8 x 24 matrix) and
+    entirely onto single CTAs: both must meet the tolerance, with bit-symmetric A and P (probe)."""
+    pair_min_d(min_d)
+    wl = workloads.get(wname)
+    sess, errs = _full_step_check(wl, precision=mf.NS_BF16)
+    assert max(errs) <= 3e-2
+    rng = np.random.default_rng(6)
+    for i in range(len(sess.mats)):
+        gh.probe_last_iteration(sess, i, rng, 2e-2)
+
+
+def test_medium_ragged_default_split_bf16():
+    """Default threshold: the set is split between the two tile classes inside one step."""
+    wl = workloads.get("medium")
+    _, errs = _full_step_check(wl, precision=mf.NS_BF16)
+    assert max(errs) <= 3e-2
+
+
 @pytest.mark.parametrize("steps", [1, 2, 3])
 def test_ns_step_counts_bf16(steps):
     """K is an argument (the paper's runs use K = 2); odd/even K end in different ping-pong buffers."""

@@ -102,8 +102,18 @@ def small_ragged(seed=7, dtype=BF16, precision=NS_BF16):
     return Workload("small_ragged", params, seed=seed, precision=precision, dtype=dtype)
 
 
+def medium_ragged(seed=11, dtype=BF16, precision=NS_BF16):
+    """Parity-test set for the 256 x 256 CTA-pair tiles: several pair tiles per matrix, ragged edges in both
+    dimensions (not multiples of 64 / 128 / 256), wide / tall / square; still seconds for the oracle."""
+    shapes = [(600, 904), (904, 520), (768, 768), (513, 1288), (1288, 264), (256, 256), (1000, 392)]
+    params = [(i // 3, 2, r, c, dtype, 0) for i, (r, c) in enumerate(shapes)]
+    params += [(0, 1, 513, 1, dtype, 0)]
+    params.sort(key=lambda p: p[0])
+    return Workload("medium_ragged", params, seed=seed, precision=precision, dtype=dtype)
+
+
 CONFIGS = {"c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
-           "small": small_ragged}
+           "small": small_ragged, "medium": medium_ragged}
 
 
 def get(name):
