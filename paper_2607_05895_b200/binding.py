@@ -65,7 +65,7 @@ class PlanResult:
 _SYMBOLS = ["mfsdp_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
-            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune"]
+            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace"]
 _lib = None
 
 
@@ -110,6 +110,7 @@ def load():
     lib.mfsdp_launch_count.restype = C.c_uint64
     lib.mfsdp_tune.argtypes = [i32, i32]
     lib.mfsdp_get_tune.argtypes = [i32]
+    lib.mfsdp_debug_trace.argtypes = [vp, sz]
     for name in _SYMBOLS:
         getattr(lib, name)          # AttributeError if the library does not export what the header declares
     _lib = lib
@@ -184,6 +185,14 @@ TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP = 0, 1, 2, 3
 
 def mfsdp_tune(knob, value):
     _check(load().mfsdp_tune(int(knob), int(value)), "mfsdp_tune")
+
+
+def mfsdp_debug_trace(buf):
+    """buf: zeroed int64 CUDA tensor (kept alive by the caller) or None to switch tracing off."""
+    if buf is None:
+        _check(load().mfsdp_debug_trace(None, 0), "mfsdp_debug_trace")
+    else:
+        _check(load().mfsdp_debug_trace(_ptr(buf), buf.numel() * buf.element_size()), "mfsdp_debug_trace")
 
 
 def mfsdp_get_tune(knob):

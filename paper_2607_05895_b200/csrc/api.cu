@@ -1,5 +1,7 @@
 // C-ABI entry points of the step (include/mfsdp.h): argument checks, workspace layout, the per-table cache of
 // device launch tables, and the launch sequence.  No compute happens here and there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -34,6 +36,12 @@ void tune_init() {
   g_tune_init = true;
 }
 }  // namespace
+
+namespace {
+unsigned long long* g_trace = nullptr;
+uint32_t g_trace_cap = 0;
+}  // namespace
+void get_trace(unsigned long long** buf, uint32_t* cap) { *buf = g_trace; *cap = g_trace_cap; }
 
 int tune_value(int knob) {
   tune_init();
@@ -72,6 +80,9 @@ int build_ws_layout(const mfsdp_desc_t* desc, size_t n_desc, int precision, WsLa
       L.d = L.tall ? q.cols : q.rows; L.n_long = L.tall ? q.rows : q.cols;
       L.pitch_x = (uint32_t)align_up_u64(q.cols, pad);
       L.pitch_a = (uint32_t)align_up_u64(L.d, pad);
+      L.scale[MFSDP_SCALE_MATCH_RMS_ADAMW] = 0.2 * std::sqrt((double)std::max(q.rows, q.cols));
+      L.scale[MFSDP_SCALE_ORIGINAL] = std::sqrt(std::max(1.0, (double)q.rows / (double)q.cols));
+      L.scale[MFSDP_SCALE_NONE] = 1.0;
       L.chunk_begin = out.n_chunks;
       const uint64_t nch = (L.numel + kChunk - 1) / kChunk;
       if (nch + out.n_chunks > 0x7fffffffull) return MFSDP_EINVAL;
@@ -82,7 +93,7 @@ int build_ws_layout(const mfsdp_desc_t* desc, size_t n_desc, int precision, WsLa
       out.tail_dtype = (int)q.dtype;
       TailLayout T;
       T.elem_off = q.elem_off; T.numel = (uint64_t)q.rows * q.cols; T.chunk_begin = out.n_tail_chunks; T.pad = 0;
-      out.n_tail_chunks += (uint32_t)((T.numel + kChunk - 1) / kChunk);
+      out.n_tail_chunks += (uint32_t)((T.numel + kTailChunk - 1) / kTailChunk);
       out.tails.push_back(T);
     }
   }
@@ -153,15 +164,22 @@ int get_plan(const mfsdp_desc_t* desc, size_t n_desc, int precision, void* works
   cb[lay.mats.size()] = lay.n_chunks;
   for (size_t i = 0; i < lay.tails.size(); ++i) tcb[i] = lay.tails[i].chunk_begin;
   tcb[lay.tails.size()] = lay.n_tail_chunks;
+  std::vector<uint32_t> cm(lay.n_chunks), ct(lay.n_tail_chunks);
+  for (size_t i = 0; i < lay.mats.size(); ++i)
+    for (uint32_t c = cb[i]; c < cb[i + 1]; ++c) cm[c] = (uint32_t)i;
+  for (size_t i = 0; i < lay.tails.size(); ++i)
+    for (uint32_t c = tcb[i]; c < tcb[i + 1]; ++c) ct[c] = (uint32_t)i;
   if ((rc = upload(&pl->d_mats, lay.mats.data(), lay.mats.size())) ||
       (rc = upload(&pl->d_tails, lay.tails.data(), lay.tails.size())) ||
       (rc = upload(&pl->d_chunk_begin, cb.data(), cb.size())) ||
-      (rc = upload(&pl->d_tail_chunk_begin, tcb.data(), tcb.size()))) {
+      (rc = upload(&pl->d_tail_chunk_begin, tcb.data(), tcb.size())) ||
+      (rc = upload(&pl->d_chunk_mat, cm.data(), cm.size())) || (rc = upload(&pl->d_chunk_tail, ct.data(), ct.size()))) {
     return rc;   // a failed cudaMalloc on a tiny table: leave the partial plan to process teardown
   }
   if (g_plans.size() >= 64) {          // bound the cache: drop the oldest entry
     Plan* old = g_plans.front();
     cudaFree(old->d_mats); cudaFree(old->d_tails); cudaFree(old->d_chunk_begin); cudaFree(old->d_tail_chunk_begin);
+    cudaFree(old->d_chunk_mat); cudaFree(old->d_chunk_tail);
     destroy_ns_tc(old->tc);
     delete old;
     g_plans.erase(g_plans.begin());
@@ -335,6 +353,14 @@ extern "C" int mfsdp_tune(int knob, int value) {
     cudaDeviceSynchronize();           // the tables may be in use by launches still in flight
     for (Plan* pl : g_plans) { destroy_ns_tc(pl->tc); pl->tc = nullptr; }
   }
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_debug_trace(void* dev_buf, size_t bytes) {
+  if (dev_buf && (bytes < 40 || (reinterpret_cast<uintptr_t>(dev_buf) & 7))) return MFSDP_EINVAL;
+  std::lock_guard<std::mutex> lock(g_mu);
+  g_trace = static_cast<unsigned long long*>(dev_buf);
+  g_trace_cap = dev_buf ? (uint32_t)std::min<size_t>((bytes - 8) / 32, 0x7fffffffu) : 0;
   return MFSDP_OK;
 }
 

@@ -4,7 +4,10 @@
 //   k_update    W <- W (1 - lr wd) - lr s(rows, cols) O
 //   k_adamw     decoupled-decay Adam on the packed tails
 // Work unit = a chunk of kChunk consecutive elements of ONE segment (never straddles segments), so every access
-// is a 128-bit vector on a 128-byte aligned run; chunk -> segment by binary search over a prefix table.
+// is a 128-bit vector on a 128-byte aligned run; chunk -> segment through a host-built table.  A thread owns
+// kVecPerThread 8-element vectors of the chunk and moves them in batches of kBatch: all loads of a batch are issued
+// before the first use, so each thread keeps 4-12 independent 128-bit loads in flight (HBM latency x bandwidth needs
+// ~40 KB in flight per SM).
 #include <cuda_bf16.h>
 
 #include "mfsdp_internal.h"
@@ -12,14 +15,9 @@
 namespace mfsdp {
 namespace {
 
-__device__ __forceinline__ uint32_t find_segment(const uint32_t* __restrict__ begin, uint32_t n_seg, uint32_t chunk) {
-  uint32_t lo = 0, hi = n_seg;                 // begin[lo] <= chunk < begin[hi]
-  while (hi - lo > 1) {
-    const uint32_t mid = (lo + hi) >> 1;
-    if (begin[mid] <= chunk) lo = mid; else hi = mid;
-  }
-  return lo;
-}
+constexpr int kVecPerThread = (int)(kChunk / (kEwThreads * 8));   // 8
+constexpr int kBatch = 4;                                          // vectors per batch
+static_assert(kVecPerThread % kBatch == 0, "chunk = whole batches");
 
 // ---- 8-element vector access ------------------------------------------------------------------------------------
 struct F8 { float v[8]; };
@@ -95,48 +93,72 @@ __device__ __forceinline__ double block_sum(double x, double* smem) {
 // ---- a1: momentum + Nesterov + cast + partial squared norm ---------------------------------------------------------
 template <typename GT, typename XT>
 __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __restrict__ mats,
-                                                         const uint32_t* __restrict__ chunk_begin, uint32_t n_mat,
-                                                         uint32_t n_chunks, const GT* __restrict__ G,
-                                                         float* __restrict__ M, uint8_t* __restrict__ ws,
-                                                         double* __restrict__ partial, float mu, float omm,
-                                                         int nesterov) {
+                                                         const uint32_t* __restrict__ chunk_mat, uint32_t n_chunks,
+                                                         const GT* __restrict__ G, float* __restrict__ M,
+                                                         uint8_t* __restrict__ ws, double* __restrict__ partial,
+                                                         float mu, float omm, int nesterov) {
   __shared__ double red[kEwThreads / 32];
   for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
-    const uint32_t mi = find_segment(chunk_begin, n_mat, c);
-    const MatLayout L = mats[mi];
+    const MatLayout L = mats[chunk_mat[c]];
     const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
     const GT* g = G + L.elem_off;
     float* m = M + L.elem_off;
     XT* x = reinterpret_cast<XT*>(ws + L.x_off[0]);
     const bool vec = (L.cols % 8u) == 0u;      // then pitch_x == cols and a vector never straddles a row
     double acc = 0.0;
+    if (vec && base + kChunk <= L.numel) {     // full chunk: batched 128-bit accesses
 #pragma unroll
-    for (int it = 0; it < (int)(kChunk / (kEwThreads * 8)); ++it) {
-      const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
-      if (e0 >= L.numel) continue;
-      if (vec && e0 + 8 <= L.numel) {
-        const F8 gv = load8_ro(g + e0);
-        F8 mv = load8(m + e0);
-        F8 uv;
+      for (int b = 0; b < kVecPerThread / kBatch; ++b) {
+        F8 gv[kBatch], mv[kBatch];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const float gs = omm * gv.v[i];
-          mv.v[i] = fmaf(mu, mv.v[i], gs);                       // M <- mu M + (1-mu) G
-          uv.v[i] = nesterov ? fmaf(mu, mv.v[i], gs) : mv.v[i];  // U = (1-mu) G + mu M   |   U = M
-          acc = fma((double)uv.v[i], (double)uv.v[i], acc);
+        for (int v = 0; v < kBatch; ++v) {
+          const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
+          gv[v] = load8_ro(g + e0);
+          mv[v] = load8(m + e0);
         }
-        store8(m + e0, mv);
-        store8(x + e0, uv);
-      } else {
-        const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
-        for (uint64_t e = e0; e < e1; ++e) {
-          const float gs = omm * load1(g + e);
-          const float mn = fmaf(mu, m[e], gs);
-          const float u = nesterov ? fmaf(mu, mn, gs) : mn;
-          acc = fma((double)u, (double)u, acc);
-          m[e] = mn;
-          const uint64_t r = e / L.cols, col = e - r * L.cols;
-          store1(x + r * L.pitch_x + col, u);
+#pragma unroll
+        for (int v = 0; v < kBatch; ++v) {
+          const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
+          F8 uv;
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float gs = omm * gv[v].v[i];
+            mv[v].v[i] = fmaf(mu, mv[v].v[i], gs);                       // M <- mu M + (1-mu) G
+            uv.v[i] = nesterov ? fmaf(mu, mv[v].v[i], gs) : mv[v].v[i];  // U = (1-mu) G + mu M   |   U = M
+            acc = fma((double)uv.v[i], (double)uv.v[i], acc);
+          }
+          store8(m + e0, mv[v]);
+          store8(x + e0, uv);
+        }
+      }
+    } else {                                   // ragged chunk or odd pitch: same element -> thread mapping, guarded
+      for (int it = 0; it < kVecPerThread; ++it) {
+        const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
+        if (e0 >= L.numel) break;
+        if (vec && e0 + 8 <= L.numel) {
+          const F8 gv = load8_ro(g + e0);
+          F8 mv = load8(m + e0);
+          F8 uv;
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float gs = omm * gv.v[i];
+            mv.v[i] = fmaf(mu, mv.v[i], gs);
+            uv.v[i] = nesterov ? fmaf(mu, mv.v[i], gs) : mv.v[i];
+            acc = fma((double)uv.v[i], (double)uv.v[i], acc);
+          }
+          store8(m + e0, mv);
+          store8(x + e0, uv);
+        } else {
+          const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
+          for (uint64_t e = e0; e < e1; ++e) {
+            const float gs = omm * load1(g + e);
+            const float mn = fmaf(mu, m[e], gs);
+            const float u = nesterov ? fmaf(mu, mn, gs) : mn;
+            acc = fma((double)u, (double)u, acc);
+            m[e] = mn;
+            const uint64_t r = e / L.cols, col = e - r * L.cols;
+            store1(x + r * L.pitch_x + col, u);
+          }
         }
       }
     }
@@ -163,42 +185,55 @@ __global__ void __launch_bounds__(kEwThreads) k_ssq(const uint32_t* __restrict__
 }
 
 // ---- a4: scaled, weight-decayed update ------------------------------------------------------------------------------
-__device__ __forceinline__ double update_scale(uint32_t rows, uint32_t cols, int mode) {
-  if (mode == MFSDP_SCALE_MATCH_RMS_ADAMW) return 0.2 * sqrt((double)(rows > cols ? rows : cols));
-  if (mode == MFSDP_SCALE_ORIGINAL) { const double r = (double)rows / (double)cols; return sqrt(r > 1.0 ? r : 1.0); }
-  return 1.0;
-}
-
+// s(rows, cols) is tabulated per matrix on the host (MatLayout::scale, one entry per MFSDP_SCALE_* mode).
 template <typename WT, typename OT>
 __global__ void __launch_bounds__(kEwThreads) k_update(const MatLayout* __restrict__ mats,
-                                                       const uint32_t* __restrict__ chunk_begin, uint32_t n_mat,
-                                                       uint32_t n_chunks, WT* __restrict__ W,
-                                                       const uint8_t* __restrict__ ws, int o_buf, double lr,
-                                                       float decay, int scale_mode) {
+                                                       const uint32_t* __restrict__ chunk_mat, uint32_t n_chunks,
+                                                       WT* __restrict__ W, const uint8_t* __restrict__ ws, int o_buf,
+                                                       double lr, float decay, int scale_mode) {
   for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
-    const uint32_t mi = find_segment(chunk_begin, n_mat, c);
+    const uint32_t mi = chunk_mat[c];
     const MatLayout L = mats[mi];
     const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
     WT* w = W + L.elem_off;
-    const OT* o = reinterpret_cast<const OT*>(ws + L.x_off[o_buf]);
-    const float coef = (float)(lr * update_scale(L.rows, L.cols, scale_mode));   // lr s, rounded once
+    const OT* o = reinterpret_cast<const OT*>(ws + (o_buf ? L.x_off[1] : L.x_off[0]));
+    const float coef = (float)(lr * mats[mi].scale[scale_mode]);   // lr s, rounded once
     const bool vec = (L.cols % 8u) == 0u;
+    if (vec && base + kChunk <= L.numel) {
 #pragma unroll
-    for (int it = 0; it < (int)(kChunk / (kEwThreads * 8)); ++it) {
-      const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
-      if (e0 >= L.numel) continue;
-      if (vec && e0 + 8 <= L.numel) {
-        F8 wv = load8(w + e0);
-        const F8 ov = load8(o + e0);
+      for (int b = 0; b < kVecPerThread / kBatch; ++b) {
+        F8 wv[kBatch], ov[kBatch];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) wv.v[i] = fmaf(-coef, ov.v[i], decay * wv.v[i]);
-        store8(w + e0, wv);
-      } else {
-        const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
-        for (uint64_t e = e0; e < e1; ++e) {
-          const uint64_t r = e / L.cols, col = e - r * L.cols;
-          const float ov = load1(o + r * L.pitch_x + col);
-          store1(w + e, fmaf(-coef, ov, decay * load1(w + e)));
+        for (int v = 0; v < kBatch; ++v) {
+          const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
+          wv[v] = load8(w + e0);
+          ov[v] = load8_ro(o + e0);
+        }
+#pragma unroll
+        for (int v = 0; v < kBatch; ++v) {
+          const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
+#pragma unroll
+          for (int i = 0; i < 8; ++i) wv[v].v[i] = fmaf(-coef, ov[v].v[i], decay * wv[v].v[i]);
+          store8(w + e0, wv[v]);
+        }
+      }
+    } else {
+      for (int it = 0; it < kVecPerThread; ++it) {
+        const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
+        if (e0 >= L.numel) break;
+        if (vec && e0 + 8 <= L.numel) {
+          F8 wv = load8(w + e0);
+          const F8 ov = load8(o + e0);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) wv.v[i] = fmaf(-coef, ov.v[i], decay * wv.v[i]);
+          store8(w + e0, wv);
+        } else {
+          const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
+          for (uint64_t e = e0; e < e1; ++e) {
+            const uint64_t r = e / L.cols, col = e - r * L.cols;
+            const float ov = load1(o + r * L.pitch_x + col);
+            store1(w + e, fmaf(-coef, ov, decay * load1(w + e)));
+          }
         }
       }
     }
@@ -218,22 +253,19 @@ __device__ __forceinline__ void adam1(float& p, float g, float& m, float& v, con
 
 template <typename PT>
 __global__ void __launch_bounds__(kEwThreads) k_adamw(const TailLayout* __restrict__ tails,
-                                                      const uint32_t* __restrict__ chunk_begin, uint32_t n_tail,
-                                                      uint32_t n_chunks, PT* __restrict__ P,
-                                                      const PT* __restrict__ G, float* __restrict__ Mo,
-                                                      float* __restrict__ Vo, AdamConst k) {
+                                                      const uint32_t* __restrict__ chunk_tail, uint32_t n_chunks,
+                                                      PT* __restrict__ P, const PT* __restrict__ G,
+                                                      float* __restrict__ Mo, float* __restrict__ Vo, AdamConst k) {
   for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
-    const uint32_t ti = find_segment(chunk_begin, n_tail, c);
-    const TailLayout L = tails[ti];
-    const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
+    const TailLayout L = tails[chunk_tail[c]];
+    const uint64_t base = (uint64_t)(c - L.chunk_begin) * kTailChunk;
     PT* p = P + L.elem_off;
     const PT* g = G + L.elem_off;
     float* m = Mo + L.elem_off;
     float* v = Vo + L.elem_off;
-#pragma unroll
-    for (int it = 0; it < (int)(kChunk / (kEwThreads * 8)); ++it) {
+    for (int it = 0; it < (int)(kTailChunk / (kEwThreads * 8)); ++it) {
       const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
-      if (e0 >= L.numel) continue;
+      if (e0 >= L.numel) break;
       if (e0 + 8 <= L.numel) {
         F8 pv = load8(p + e0);
         const F8 gv = load8_ro(g + e0);
@@ -272,7 +304,7 @@ int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hpa
   const int grid = ew_grid(lay.n_chunks);
   const bool gbf = lay.mat_dtype == MFSDP_BF16, xbf = pl.precision == MFSDP_NS_BF16;
 #define MOM(GT, XT)                                                                                             \
-  k_momentum<GT, XT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_begin, n_mat, lay.n_chunks,             \
+  k_momentum<GT, XT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                      \
                                                   static_cast<const GT*>(G), static_cast<float*>(M), ws, partial, \
                                                   mu, omm, hp.nesterov)
   if (gbf && xbf) MOM(__nv_bfloat16, __nv_bfloat16);
@@ -299,7 +331,7 @@ int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaS
   const int grid = ew_grid(lay.n_chunks);
   const bool wbf = lay.mat_dtype == MFSDP_BF16, obf = pl.precision == MFSDP_NS_BF16;
 #define UPD(WT, OT)                                                                                      \
-  k_update<WT, OT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_begin, n_mat, lay.n_chunks,        \
+  k_update<WT, OT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                 \
                                                 static_cast<WT*>(W), ws, o_buf, hp.lr, decay, hp.scale_mode)
   if (wbf && obf) UPD(__nv_bfloat16, __nv_bfloat16);
   else if (wbf) UPD(__nv_bfloat16, float);
@@ -326,12 +358,12 @@ int launch_adamw(const Plan& pl, void* P, const void* G, void* m, void* v, const
   k.lr = (float)hp.lr; k.eps = (float)hp.eps;
   const int grid = ew_grid(lay.n_tail_chunks);
   if (lay.tail_dtype == MFSDP_BF16)
-    k_adamw<__nv_bfloat16><<<grid, kEwThreads, 0, st>>>(pl.d_tails, pl.d_tail_chunk_begin, n_tail, lay.n_tail_chunks,
+    k_adamw<__nv_bfloat16><<<grid, kEwThreads, 0, st>>>(pl.d_tails, pl.d_chunk_tail, lay.n_tail_chunks,
                                                         static_cast<__nv_bfloat16*>(P),
                                                         static_cast<const __nv_bfloat16*>(G), static_cast<float*>(m),
                                                         static_cast<float*>(v), k);
   else
-    k_adamw<float><<<grid, kEwThreads, 0, st>>>(pl.d_tails, pl.d_tail_chunk_begin, n_tail, lay.n_tail_chunks,
+    k_adamw<float><<<grid, kEwThreads, 0, st>>>(pl.d_tails, pl.d_chunk_tail, lay.n_tail_chunks,
                                                 static_cast<float*>(P), static_cast<const float*>(G),
                                                 static_cast<float*>(m), static_cast<float*>(v), k);
   count_launch();

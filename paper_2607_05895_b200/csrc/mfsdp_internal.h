@@ -14,7 +14,8 @@ namespace mfsdp {
 // ---- workspace layout ---------------------------------------------------------------------------------------
 // [ssq: double x n_mat][inv_norm: float x n_mat][partials: double x n_chunks] then per matrix X0, X1 (rows x
 // pitch_x), A, P (d x pitch_a), every buffer 1024-byte aligned (TMA / 128B-swizzle friendly).
-constexpr uint32_t kChunk = 4096;        // elements per elementwise work unit (256 threads x 16)
+constexpr uint32_t kChunk = 16384;       // elements per elementwise work unit (256 threads x 8 vectors of 8)
+constexpr uint32_t kTailChunk = 2048;    // tails are short (<= ~1e5 elements per rank): one vector per thread spreads them over the SMs
 constexpr uint32_t kEwThreads = 256;
 constexpr size_t kBufAlign = 1024;
 
@@ -28,6 +29,7 @@ struct MatLayout {          // host + device; one per MATRIX descriptor, in tabl
   uint32_t pitch_x, pitch_a;  // row pitches in elements
   uint32_t chunk_begin;     // index of this matrix' first chunk (partials / grid mapping)
   uint32_t tall;            // rows > cols
+  double scale[3];          // update scale s(rows, cols) per MFSDP_SCALE_* mode (reading M7)
 };
 
 struct TailLayout {         // one per TAIL descriptor
@@ -62,6 +64,8 @@ struct Plan {
   TailLayout* d_tails = nullptr;
   uint32_t* d_chunk_begin = nullptr;       // [n_mat + 1]
   uint32_t* d_tail_chunk_begin = nullptr;  // [n_tail + 1]
+  uint32_t* d_chunk_mat = nullptr;         // [n_chunks] chunk -> matrix index
+  uint32_t* d_chunk_tail = nullptr;        // [n_tail_chunks] chunk -> tail index
   NsTcPlan* tc = nullptr;
 };
 
@@ -82,7 +86,8 @@ void count_launch(uint64_t n = 1);
 int cuda_fail(cudaError_t e);          // records the error text, returns MFSDP_ECUDA
 int check_last_launch();               // cudaGetLastError -> code
 
-int tune_value(int knob);               // current value of an MFSDP_TUNE_* knob
+int tune_value(int knob);
+void get_trace(unsigned long long** buf, uint32_t* cap);   // mfsdp_debug_trace target (null when off)               // current value of an MFSDP_TUNE_* knob
 
 inline uint64_t align_up_u64(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 

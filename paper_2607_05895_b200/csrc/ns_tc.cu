@@ -76,6 +76,8 @@ struct TcParams {
   const float* inv_norm;
   int phase, src, first;
   float a, b, c;
+  unsigned long long* trace;    // optional (mfsdp_debug_trace): [0] = record counter, then 4 words per tile
+  uint32_t trace_cap, launch_idx;
 };
 
 struct TileCfg {
@@ -230,6 +232,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
 
       ptx::mbar_wait(tfull0 + 8 * acc, acc_phase);
       ptx::tc_fence_after();
+      const unsigned long long t_ready = p.trace ? ptx::globaltimer() : 0ull;
       const uint32_t taddr0 = tmem_base + ((q * 32u) << 16) + acc * kBNMax;
       for (uint32_t c0 = 0; c0 < t.nw; c0 += 32) {
         const uint32_t col0 = t.n0 + c0;
@@ -296,6 +299,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       }
       ptx::tc_fence_before();
       __syncwarp();
+      if (p.trace && q == 0 && lane == 0 && rank == 0) {         // one record per tile: when its accumulator was ready
+        const unsigned long long slot = atomicAdd(p.trace, 1ull);   // and when this warp had stored its share
+        if (slot < p.trace_cap) {
+          unsigned long long* rec = p.trace + 1 + 4 * slot;
+          rec[0] = ((unsigned long long)p.launch_idx << 32) | ti;
+          rec[1] = ((unsigned long long)unit << 32) | ptx::smid();
+          rec[2] = t_ready;
+          rec[3] = ptx::globaltimer();
+        }
+      }
       if (lane == 0) {
         if constexpr (kCG == 2) ptx::mbar_arrive_cluster(tempty_lead0 + 8 * acc); else ptx::mbar_arrive(tempty0 + 8 * acc);
       }
@@ -497,6 +510,8 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
   p.ws = static_cast<uint8_t*>(pl.workspace);
   p.inv_norm = reinterpret_cast<const float*>(p.ws + pl.lay.invn_off);
   p.a = (float)hp.a; p.b = (float)hp.b; p.c = (float)hp.c;
+  get_trace(&p.trace, &p.trace_cap);
+  p.launch_idx = 0;
   for (int it = 0; it < hp.ns_steps; ++it) {
     p.src = it & 1;
     p.first = (it == 0);
@@ -511,6 +526,7 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
         if (g == 1) e = launch_phase<2>(p, std::min<uint32_t>(p.n_tiles, (uint32_t)tc.max_pairs), st);
         else e = launch_phase<1>(p, std::min<uint32_t>(p.n_tiles, (uint32_t)tc.sms), st);
         if (e != cudaSuccess) return cuda_fail(e);
+        ++p.launch_idx;
         count_launch();
         const int rc = check_last_launch();
         if (rc) return rc;
