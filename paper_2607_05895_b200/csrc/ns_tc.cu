@@ -43,6 +43,7 @@ struct NsTcPlan {
   TcMat* d_mats = nullptr;
   TcTile* d_tiles[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // [kCG - 1][phase]
   uint32_t n_tiles[2][3] = {{0, 0, 0}, {0, 0, 0}};
+  uint32_t* d_counters = nullptr;   // one tile counter per launch of a pass (zeroed at the start of every pass)
   int sms = 148;
   int max_pairs = 74;               // co-resident CTA pairs
 };
@@ -55,6 +56,7 @@ constexpr uint32_t kBK = 64;                   // k elements per stage (one 128-
 constexpr uint32_t kBoxBytes = 64 * 64 * 2;    // one TMA box: 64 rows x 128 B
 constexpr uint32_t kABytes = 2 * kBoxBytes;    // 128 x 64
 constexpr uint32_t kThreads = 192;
+constexpr uint32_t kMaxLaunches = 64 * 3 * 2;   // ns_steps <= 64, three phases, two tile classes
 constexpr uint32_t kTmemCols = 512;
 
 template <int kCG>
@@ -76,6 +78,7 @@ struct TcParams {
   const float* inv_norm;
   int phase, src, first;
   float a, b, c;
+  uint32_t* counter;            // dynamic tile scheduler: next unclaimed tile of THIS launch (zero at launch)
   unsigned long long* trace;    // optional (mfsdp_debug_trace): [0] = record counter, then 4 words per tile
   uint32_t trace_cap, launch_idx;
 };
@@ -109,6 +112,55 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return *reinterpret_cast<const uint32_t*>(&h);
 }
 
+// ---- dynamic tile scheduler ------------------------------------------------------------------------------------
+// The producer thread of a walking unit (CTA, or leader CTA of a pair) claims the next tile of the launch with one
+// atomicAdd when it is ready to start loading it, and publishes the index through a small shared-memory ring
+// (kFeed slots, full/empty mbarriers) to the other roles: UMMA issuer and epilogue warps of its own CTA and, when
+// paired, the producer and epilogue warps of the peer CTA (remote store + remote arrive).  Tiles are therefore
+// handed out in list order at the pace of the fastest units: the tiles in flight are always a contiguous window of
+// the (rasterised) list, started at staggered times, and no unit idles while tiles remain.
+constexpr uint32_t kFeed = 4;
+constexpr uint32_t kNoTile = 0xffffffffu;
+
+template <int kCG>
+struct Feed {
+  uint32_t full0, empty0, slots0;        // shared::cta addresses: full barriers, empty barriers (used by the leader), slots
+  uint32_t empty_lead0;                  // the leader's empty barriers as a shared::cluster address (paired) / = empty0
+  uint32_t s = 0, ph = 0;
+  __device__ __forceinline__ void advance() { if (++s == kFeed) { s = 0; ph ^= 1; } }
+  // leader producer: claim and publish.  Returns the tile index or kNoTile.
+  __device__ __forceinline__ uint32_t claim(uint32_t* counter, uint32_t n_tiles) {
+    ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);                // every consumer has read the slot's previous content
+    uint32_t ti = atomicAdd(counter, 1u);
+    if (ti >= n_tiles) ti = kNoTile;
+    ptx::st_shared_u32(slots0 + 4 * s, ti);
+    if constexpr (kCG == 2) {
+      ptx::st_shared_cluster_u32(ptx::mapa(slots0 + 4 * s, 1), ti);
+      ptx::mbar_arrive_cluster(ptx::mapa(full0 + 8 * s, 1));
+    }
+    ptx::mbar_arrive(full0 + 8 * s);
+    advance();
+    return ti;
+  }
+  // any other role: wait for the next index ...
+  __device__ __forceinline__ uint32_t peek() const {
+    if constexpr (kCG == 2) ptx::mbar_wait_cluster(full0 + 8 * s, ph); else ptx::mbar_wait(full0 + 8 * s, ph);
+    return ptx::ld_shared_u32(slots0 + 4 * s);
+  }
+  // ... and report the slot as consumed (`arrive`: one thread per role, after every thread of the role has read it).
+  __device__ __forceinline__ void release(bool arrive) {
+    if (arrive) {
+      if constexpr (kCG == 2) ptx::mbar_arrive_cluster(empty_lead0 + 8 * s); else ptx::mbar_arrive(empty_lead0 + 8 * s);
+    }
+    advance();
+  }
+  __device__ __forceinline__ uint32_t next_single() {      // single-thread roles
+    const uint32_t ti = peek();
+    release(true);
+    return ti;
+  }
+};
+
 template <int kCG>
 __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   using G = Geo<kCG>;
@@ -118,15 +170,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   const uint32_t full0 = ptx::smem_u32(bars), empty0 = ptx::smem_u32(bars + G::kStages);
   const uint32_t tfull0 = ptx::smem_u32(bars + 2 * G::kStages), tempty0 = ptx::smem_u32(bars + 2 * G::kStages + 2);
   uint32_t* tmem_holder = reinterpret_cast<uint32_t*>(bars + 2 * G::kStages + 4);
+  Feed<kCG> feed;
+  feed.full0 = ptx::smem_u32(bars + 2 * G::kStages + 5);
+  feed.empty0 = ptx::smem_u32(bars + 2 * G::kStages + 5 + kFeed);
+  feed.slots0 = ptx::smem_u32(bars + 2 * G::kStages + 5 + 2 * kFeed);
   const uint32_t stage0 = ptx::smem_u32(smem);
   const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = kCG == 2 ? ptx::cluster_ctarank() : 0u;          // 0 = leader of the pair
   const uint32_t unit = kCG == 2 ? blockIdx.x >> 1 : blockIdx.x;          // tile-walking unit: CTA or CTA pair
-  const uint32_t n_units = kCG == 2 ? gridDim.x >> 1 : gridDim.x;
+  feed.empty_lead0 = kCG == 2 ? ptx::mapa(feed.empty0, 0) : feed.empty0;
 
   if (threadIdx.x == 0) {
     for (uint32_t s = 0; s < G::kStages; ++s) { ptx::mbar_init(full0 + 8 * s, 1); ptx::mbar_init(empty0 + 8 * s, 1); }
     for (uint32_t s = 0; s < 2; ++s) { ptx::mbar_init(tfull0 + 8 * s, 1); ptx::mbar_init(tempty0 + 8 * s, 4 * kCG); }
+    // feed consumers per slot: UMMA issuer + 4 epilogue warps of the leader, producer + 4 epilogue warps of the peer
+    for (uint32_t s = 0; s < kFeed; ++s) { ptx::mbar_init(feed.full0 + 8 * s, 1); ptx::mbar_init(feed.empty0 + 8 * s, 5 * kCG); }
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc<kTmemCols, kCG>(ptx::smem_u32(tmem_holder));
@@ -140,7 +198,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     if (lane == 0) {
       uint32_t stage = 0, phase = 0;
       const uint32_t full_lead0 = kCG == 2 ? ptx::mapa(full0, 0) : full0;
-      for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
+      for (;;) {
+        const uint32_t ti = rank == 0 ? feed.claim(p.counter, p.n_tiles) : feed.next_single();
+        if (ti == kNoTile) break;
         const TcTile t = p.tiles[ti];
         const TcMat M = p.mats[t.mat];
         const TileCfg c = decode(p, t, M);
@@ -176,7 +236,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     // ===== UMMA issuer (leader CTA only when paired) =====
     if (lane == 0 && rank == 0) {
       uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
-      for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
+      for (;;) {
+        const uint32_t ti = feed.next_single();
+        if (ti == kNoTile) break;
         const TcTile t = p.tiles[ti];
         const TcMat M = p.mats[t.mat];
         const TileCfg c = decode(p, t, M);
@@ -213,7 +275,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     const uint32_t q = warp & 3;
     uint32_t acc = 0, acc_phase = 0;
     const uint32_t tempty_lead0 = kCG == 2 ? ptx::mapa(tempty0, 0) : tempty0;
-    for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
+    for (;;) {
+      const uint32_t ti = feed.peek();
+      __syncwarp();
+      feed.release(lane == 0);
+      if (ti == kNoTile) break;
       const TcTile t = p.tiles[ti];
       const TcMat M = p.mats[t.mat];
       const TileCfg c = decode(p, t, M);
@@ -357,11 +423,12 @@ int make_tmap(CUtensorMap* out, void* base, uint32_t rows, uint32_t cols, uint32
   return r == CUDA_SUCCESS ? MFSDP_OK : cuda_fail(cudaErrorInvalidValue);
 }
 
-// Tile rasterisation.  The units (CTAs or CTA pairs) walk the tile list round-robin, so at any moment about
-// n_units consecutive list entries are in flight and advance along k roughly in lock step; an operand box is
-// fetched from DRAM once and served from L2 to every in-flight tile that shares it.  The list is therefore ordered
-// so that n_units consecutive tiles cover a compact block of the output: `band` row blocks x the column tiles that
-// go with them.
+// Tile rasterisation.  The units (CTAs or CTA pairs) claim tiles in list order, so at any moment the tiles in
+// flight are a contiguous window of about n_units list entries, started at staggered times: entry j + s starts about
+// s / n_units of a tile duration after entry j.  An operand box fetched from DRAM by one tile is re-read from L2 by
+// the tiles that share it as long as the next sharer follows soon enough.  The list is therefore ordered so that a
+// window covers a compact block of the output (`band` row blocks x the column tiles that go with them) and sharers
+// are few entries apart: column-panel sharers adjacent, row-panel sharers `band` entries apart.
 uint16_t tile_n(uint32_t remaining, uint32_t gran) {     // UMMA N of a tile that has `remaining` columns to cover
   return (uint16_t)std::min(kBNMax, (remaining + gran - 1) / gran * gran);
 }
@@ -466,7 +533,9 @@ int build_tc_plan(Plan& pl) {
       if ((rc = dev_upload(&tc->d_tiles[g][ph], tiles[g][ph]))) return rc;
     }
   cudaDeviceGetAttribute(&tc->sms, cudaDevAttrMultiProcessorCount, pl.device);
-  cudaError_t e = cudaFuncSetAttribute(k_ns_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geo<1>::kSmemBytes);
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), kMaxLaunches * sizeof(uint32_t));
+  if (e != cudaSuccess) return cuda_fail(e);
+  e = cudaFuncSetAttribute(k_ns_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geo<1>::kSmemBytes);
   if (e != cudaSuccess) return cuda_fail(e);
   e = cudaFuncSetAttribute(k_ns_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geo<2>::kSmemBytes);
   if (e != cudaSuccess) return cuda_fail(e);
@@ -492,7 +561,7 @@ int build_tc_plan(Plan& pl) {
 
 void destroy_ns_tc(NsTcPlan* p) {
   if (!p) return;
-  cudaFree(p->d_tmaps); cudaFree(p->d_mats);
+  cudaFree(p->d_tmaps); cudaFree(p->d_mats); cudaFree(p->d_counters);
   for (int g = 0; g < 2; ++g)
     for (int ph = 0; ph < 3; ++ph) cudaFree(p->d_tiles[g][ph]);
   delete p;
@@ -512,6 +581,10 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
   p.a = (float)hp.a; p.b = (float)hp.b; p.c = (float)hp.c;
   get_trace(&p.trace, &p.trace_cap);
   p.launch_idx = 0;
+  {
+    const cudaError_t e = cudaMemsetAsync(tc.d_counters, 0, kMaxLaunches * sizeof(uint32_t), st);
+    if (e != cudaSuccess) return cuda_fail(e);
+  }
   for (int it = 0; it < hp.ns_steps; ++it) {
     p.src = it & 1;
     p.first = (it == 0);
@@ -522,6 +595,7 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
         p.tiles = tc.d_tiles[g][ph];
         p.n_tiles = tc.n_tiles[g][ph];
         if (p.n_tiles == 0) continue;
+        p.counter = tc.d_counters + p.launch_idx;
         cudaError_t e;
         if (g == 1) e = launch_phase<2>(p, std::min<uint32_t>(p.n_tiles, (uint32_t)tc.max_pairs), st);
         else e = launch_phase<1>(p, std::min<uint32_t>(p.n_tiles, (uint32_t)tc.sms), st);
