@@ -210,9 +210,10 @@ int mfsdp_get_tune(int knob);
 
 /* Debug aid: tile trace of the tensor-core Newton-Schulz kernels.  dev_buf: DEVICE buffer of `bytes` bytes, 8-byte
  * aligned, zeroed by the caller and owned by the caller; NULL switches tracing off (the default).  While set, every
- * NS tile appends one record of four 64-bit words after the counter word dev_buf[0]:
+ * NS tile appends one record of six 64-bit words after the counter word dev_buf[0]:
  *   (launch index within the pass << 32 | tile index), (walking unit << 32 | SM id),
- *   %globaltimer ns when the tile's accumulator was complete, %globaltimer ns when its first epilogue warp was done.
+ *   %globaltimer ns when the tile's accumulator was complete, %globaltimer ns when its first epilogue warp was done,
+ *   the SM's clock64 at the first instant, (k blocks of the tile << 32 | UMMA N).
  * Records beyond the capacity are dropped (the counter keeps counting).  Returns MFSDP_EINVAL on a misaligned or
  * too-small buffer. */
 int mfsdp_debug_trace(void* dev_buf, size_t bytes);

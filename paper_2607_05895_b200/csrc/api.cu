@@ -357,10 +357,10 @@ extern "C" int mfsdp_tune(int knob, int value) {
 }
 
 extern "C" int mfsdp_debug_trace(void* dev_buf, size_t bytes) {
-  if (dev_buf && (bytes < 40 || (reinterpret_cast<uintptr_t>(dev_buf) & 7))) return MFSDP_EINVAL;
+  if (dev_buf && (bytes < 56 || (reinterpret_cast<uintptr_t>(dev_buf) & 7))) return MFSDP_EINVAL;
   std::lock_guard<std::mutex> lock(g_mu);
   g_trace = static_cast<unsigned long long*>(dev_buf);
-  g_trace_cap = dev_buf ? (uint32_t)std::min<size_t>((bytes - 8) / 32, 0x7fffffffu) : 0;
+  g_trace_cap = dev_buf ? (uint32_t)std::min<size_t>((bytes - 8) / 48, 0x7fffffffu) : 0;
   return MFSDP_OK;
 }
 

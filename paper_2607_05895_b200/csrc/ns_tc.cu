@@ -10,14 +10,20 @@
 // alpha = 1/||U||^2 and beta = 1/||U|| at iteration 0 (Frobenius normalisation folded in), 1 afterwards.
 //
 // Two tile classes share one kernel template (kCG = tcgen05 cta_group):
-//   kCG = 2  matrices with d >= MFSDP_TUNE_PAIR_MIN_D: a CTA PAIR (cluster of two SMs of one TPC) owns a 256 x 256
-//            output tile; each CTA stages its 128 rows of the A operand and its 128-column half of the B operand
-//            (32 KB per 64-k stage instead of 48 KB per 128 x 256 tile -> 2/3 of the L2->smem traffic per flop),
-//            the leader CTA issues tcgen05.mma.cta_group::2 (M = 256), 6-stage ring;
-//   kCG = 1  small / ragged matrices: one CTA owns a 128 x (64..256) tile, 4-stage ring.
+//   kCG = 2  matrices with d >= MFSDP_TUNE_PAIR_MIN_D: a CTA PAIR (cluster of two SMs of one TPC) owns a 256 x 512
+//            output tile held as two 256-column TMEM accumulators.  Per 64-k stage a CTA stages its 128 rows of the
+//            A operand and its half of both 256-column B panels (48 KB): 171 flop per byte fetched from L2, which
+//            is what the measured L2->SM ceiling (~7 KB/clk chip-wide) needs to keep the tensor pipes busy (a
+//            256 x 256 tile has 128 flop/B and measured 75 % pipe utilisation, L2-bound).  The leader CTA issues
+//            tcgen05.mma.cta_group::2 (M = 256, N = 256) for the two halves in turn; the halves finish 4 MMAs
+//            apart, so the epilogue of half 0 starts while half 1 still runs, and the next tile's MMAs into a half
+//            start as soon as that half has been drained.
+//   kCG = 1  small / ragged matrices: one CTA owns a 128 x (64..256) tile, two accumulator stages alternate
+//            between tiles (the epilogue of tile t overlaps the main loop of tile t + 1).
 // Kernel anatomy (192 threads per CTA): warp 0 = TMA producer (one lane), warp 1 = TMEM owner + UMMA issuer (one
-// lane, leader CTA only when paired), warps 2-5 = epilogue (TMEM -> registers -> global).  Two TMEM accumulator
-// stages (2 x 256 columns) let the epilogue of tile t overlap the main loop of tile t + 1.
+// lane, leader CTA only when paired), warps 2-5 = epilogue: TMEM -> registers -> fused scale / polynomial -> bf16
+// -> swizzled shared-memory staging -> TMA tensor stores (direct tile and, for the symmetric phases, the transposed
+// mirror tile); the b A term of POLY is TMA-loaded into the same staging buffer.  4-stage operand ring.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -30,16 +36,22 @@
 namespace mfsdp {
 
 enum { PH_GRAM = 0, PH_POLY = 1, PH_APPLY = 2 };
+// tensor maps per matrix
+enum { TM_X0 = 0, TM_X1 = 1, TM_A = 2, TM_P = 3,            // operand loads: box 64 x 64, 128-byte swizzle
+       TM_X0_ST = 4, TM_X1_ST = 5, TM_A_ST = 6, TM_P_ST = 7,  // epilogue tiles: box 64 cols x 32 rows, 128-byte swizzle
+       TM_A_MIR = 8, TM_P_MIR = 9,                            // mirror tiles: box 32 cols x 64 rows, no swizzle
+       TM_COUNT = 10 };
 
 struct TcMat {                 // device, one per matrix
   uint64_t x_off[2], a_off, p_off;
   uint32_t rows, cols, d, n_long, pitch_x, pitch_a, tall, pad;
 };
-// Output tile: origin (rows, cols of the OUTPUT buffer), k blocks, UMMA N (multiple of 64; of 128 when paired).
+// Output tile: origin (rows, cols of the OUTPUT buffer), k blocks, width in columns (multiple of 64; of 128 when
+// paired; <= 256 single CTA, <= 512 paired).
 struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; };
 
 struct NsTcPlan {
-  CUtensorMap* d_tmaps = nullptr;   // 4 per matrix: X0, X1, A, P   (box 64 x 64 bf16, 128-byte swizzle)
+  CUtensorMap* d_tmaps = nullptr;   // TM_COUNT per matrix
   TcMat* d_mats = nullptr;
   TcTile* d_tiles[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // [kCG - 1][phase]
   uint32_t n_tiles[2][3] = {{0, 0, 0}, {0, 0, 0}};
@@ -51,23 +63,23 @@ struct NsTcPlan {
 namespace {
 
 constexpr uint32_t kBM = 128;                  // UMMA M per CTA
-constexpr uint32_t kBNMax = 256;               // max UMMA N per tile
+constexpr uint32_t kBN = 256;                  // UMMA N = columns of one TMEM accumulator
 constexpr uint32_t kBK = 64;                   // k elements per stage (one 128-byte swizzle row)
 constexpr uint32_t kBoxBytes = 64 * 64 * 2;    // one TMA box: 64 rows x 128 B
 constexpr uint32_t kABytes = 2 * kBoxBytes;    // 128 x 64
+constexpr uint32_t kBBytes = 4 * kBoxBytes;    // single CTA: 256 x 64; paired: 2 halves x (128 x 64)
+constexpr uint32_t kStageBytes = kABytes + kBBytes;   // 48 KB
+constexpr uint32_t kStages = 4;
+#ifndef MFSDP_NS_GROUP
+#define MFSDP_NS_GROUP 2
+#endif
 constexpr uint32_t kThreads = 192;
-constexpr uint32_t kMaxLaunches = 64 * 3 * 2;   // ns_steps <= 64, three phases, two tile classes
 constexpr uint32_t kTmemCols = 512;
-
-template <int kCG>
-struct Geo {
-  static constexpr uint32_t kBBoxes = kCG == 1 ? 4 : 2;           // B-operand boxes per CTA and stage
-  static constexpr uint32_t kBBytes = kBBoxes * kBoxBytes;
-  static constexpr uint32_t kStageBytes = kABytes + kBBytes;      // 48 KB | 32 KB
-  static constexpr uint32_t kStages = kCG == 1 ? 4 : 6;
-  static constexpr uint32_t kTileM = kBM * kCG;                   // rows of the output tile
-  static constexpr uint32_t kSmemBytes = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
-};
+constexpr uint32_t kEpiBufBytes = 4096;        // one staging tile: 32 rows x 64 cols (or 64 x 32 transposed) bf16
+constexpr uint32_t kEpiBytes = 4 * 2 * kEpiBufBytes;   // 4 epilogue warps x 2 buffers
+constexpr uint32_t kBarBytes = 256;
+constexpr uint32_t kSmemBytes = kStages * kStageBytes + kEpiBytes + kBarBytes + 1024 /*align slack*/;
+constexpr uint32_t kMaxLaunches = 64 * 3 * 2;   // ns_steps <= 64, three phases, two tile classes
 
 struct TcParams {
   const TcTile* tiles;
@@ -79,12 +91,13 @@ struct TcParams {
   int phase, src, first;
   float a, b, c;
   uint32_t* counter;            // dynamic tile scheduler: next unclaimed tile of THIS launch (zero at launch)
-  unsigned long long* trace;    // optional (mfsdp_debug_trace): [0] = record counter, then 4 words per tile
+  unsigned long long* trace;    // optional (mfsdp_debug_trace): [0] = record counter, then 6 words per tile
   uint32_t trace_cap, launch_idx;
 };
 
 struct TileCfg {
-  const CUtensorMap *ta, *tb;
+  const CUtensorMap *ta, *tb;   // operand loads
+  const CUtensorMap *tout, *tmir, *tain;   // epilogue: output tile, mirror tile (symmetric phases), A tile (POLY)
   uint32_t a_mn, b_mn;          // operand majorness (1 = MN-major)
   uint32_t a_ext;               // extent of the A operand's M dimension
   uint32_t out_rows, out_cols;  // bounds of the output buffer
@@ -92,17 +105,20 @@ struct TileCfg {
 
 __device__ __forceinline__ TileCfg decode(const TcParams& p, const TcTile& t, const TcMat& M) {
   TileCfg c;
-  const CUtensorMap* tm = p.tmaps + 4 * (size_t)t.mat;
+  const CUtensorMap* tm = p.tmaps + TM_COUNT * (size_t)t.mat;
+  c.tmir = nullptr; c.tain = tm + TM_A_ST;
   if (p.phase == PH_GRAM) {
     c.ta = c.tb = tm + p.src; c.a_mn = c.b_mn = M.tall; c.a_ext = M.d; c.out_rows = c.out_cols = M.d;
+    c.tout = tm + TM_A_ST; c.tmir = tm + TM_A_MIR;
   } else if (p.phase == PH_POLY) {
-    c.ta = c.tb = tm + 2; c.a_mn = c.b_mn = 0; c.a_ext = M.d; c.out_rows = c.out_cols = M.d;
+    c.ta = c.tb = tm + TM_A; c.a_mn = c.b_mn = 0; c.a_ext = M.d; c.out_rows = c.out_cols = M.d;
+    c.tout = tm + TM_P_ST; c.tmir = tm + TM_P_MIR;
   } else if (!M.tall) {          // X_new (d x n) = P (K-major) * X (k x n, MN-major)
-    c.ta = tm + 3; c.a_mn = 0; c.a_ext = M.d; c.tb = tm + p.src; c.b_mn = 1;
-    c.out_rows = M.rows; c.out_cols = M.cols;
+    c.ta = tm + TM_P; c.a_mn = 0; c.a_ext = M.d; c.tb = tm + p.src; c.b_mn = 1;
+    c.out_rows = M.rows; c.out_cols = M.cols; c.tout = tm + TM_X0_ST + (p.src ^ 1);
   } else {                       // X_new (n x d) = X (K-major) * P^T, P symmetric (K-major)
-    c.ta = tm + p.src; c.a_mn = 0; c.a_ext = M.rows; c.tb = tm + 3; c.b_mn = 0;
-    c.out_rows = M.rows; c.out_cols = M.cols;
+    c.ta = tm + p.src; c.a_mn = 0; c.a_ext = M.rows; c.tb = tm + TM_P; c.b_mn = 0;
+    c.out_rows = M.rows; c.out_cols = M.cols; c.tout = tm + TM_X0_ST + (p.src ^ 1);
   }
   return c;
 }
@@ -163,28 +179,32 @@ struct Feed {
 
 template <int kCG>
 __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
-  using G = Geo<kCG>;
+  constexpr uint32_t kGroup = kCG == 2 ? MFSDP_NS_GROUP : 1;   // ring stages per accumulator visit
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + G::kStages * G::kStageBytes);
-  const uint32_t full0 = ptx::smem_u32(bars), empty0 = ptx::smem_u32(bars + G::kStages);
-  const uint32_t tfull0 = ptx::smem_u32(bars + 2 * G::kStages), tempty0 = ptx::smem_u32(bars + 2 * G::kStages + 2);
-  uint32_t* tmem_holder = reinterpret_cast<uint32_t*>(bars + 2 * G::kStages + 4);
+  // [operand ring: kStages x 48 KB][epilogue staging: 4 warps x 2 x 4 KB][barriers]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + kStages * kStageBytes + kEpiBytes);
+  const uint32_t full0 = ptx::smem_u32(bars), empty0 = ptx::smem_u32(bars + kStages);
+  const uint32_t tfull0 = ptx::smem_u32(bars + 2 * kStages), tempty0 = ptx::smem_u32(bars + 2 * kStages + 2);
+  uint32_t* tmem_holder = reinterpret_cast<uint32_t*>(bars + 2 * kStages + 4);
   Feed<kCG> feed;
-  feed.full0 = ptx::smem_u32(bars + 2 * G::kStages + 5);
-  feed.empty0 = ptx::smem_u32(bars + 2 * G::kStages + 5 + kFeed);
-  feed.slots0 = ptx::smem_u32(bars + 2 * G::kStages + 5 + 2 * kFeed);
+  feed.full0 = ptx::smem_u32(bars + 2 * kStages + 5);
+  feed.empty0 = ptx::smem_u32(bars + 2 * kStages + 5 + kFeed);
+  feed.slots0 = ptx::smem_u32(bars + 2 * kStages + 5 + 2 * kFeed);
+  const uint32_t epibar0 = ptx::smem_u32(bars + 2 * kStages + 7 + 2 * kFeed);   // one per epilogue warp (POLY A-tile loads)
   const uint32_t stage0 = ptx::smem_u32(smem);
+  const uint32_t epi0 = stage0 + kStages * kStageBytes;
   const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = kCG == 2 ? ptx::cluster_ctarank() : 0u;          // 0 = leader of the pair
   const uint32_t unit = kCG == 2 ? blockIdx.x >> 1 : blockIdx.x;          // tile-walking unit: CTA or CTA pair
   feed.empty_lead0 = kCG == 2 ? ptx::mapa(feed.empty0, 0) : feed.empty0;
 
   if (threadIdx.x == 0) {
-    for (uint32_t s = 0; s < G::kStages; ++s) { ptx::mbar_init(full0 + 8 * s, 1); ptx::mbar_init(empty0 + 8 * s, 1); }
+    for (uint32_t s = 0; s < kStages; ++s) { ptx::mbar_init(full0 + 8 * s, 1); ptx::mbar_init(empty0 + 8 * s, 1); }
     for (uint32_t s = 0; s < 2; ++s) { ptx::mbar_init(tfull0 + 8 * s, 1); ptx::mbar_init(tempty0 + 8 * s, 4 * kCG); }
     // feed consumers per slot: UMMA issuer + 4 epilogue warps of the leader, producer + 4 epilogue warps of the peer
     for (uint32_t s = 0; s < kFeed; ++s) { ptx::mbar_init(feed.full0 + 8 * s, 1); ptx::mbar_init(feed.empty0 + 8 * s, 5 * kCG); }
+    for (uint32_t s = 0; s < 4; ++s) ptx::mbar_init(epibar0 + 8 * s, 1);
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc<kTmemCols, kCG>(ptx::smem_u32(tmem_holder));
@@ -205,77 +225,133 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
         const TcMat M = p.mats[t.mat];
         const TileCfg c = decode(p, t, M);
         const uint32_t am0 = t.m0 + rank * kBM;
-        uint32_t a_boxes, b_boxes, bn0;
+        // B boxes of this CTA: single CTA: nw / 64 consecutive boxes.  Paired: per 256-column half h its own half of
+        // the panel, nh / 128 boxes (nh = width of the half), stored at box slot 2 h + j.
+        uint32_t a_boxes, n_b = 0, b_mask = 0;
+        uint32_t b_col[4];
         if constexpr (kCG == 2) {      // fixed box counts (out-of-range boxes are zero-filled) keep the byte count static
-          a_boxes = 2; b_boxes = t.nw >> 7; bn0 = t.n0 + rank * (t.nw >> 1);
+          a_boxes = 2;
+#pragma unroll
+          for (uint32_t h = 0; h < 2; ++h) {
+            const uint32_t nh = h * kBN < t.nw ? min((uint32_t)t.nw - h * kBN, kBN) : 0u;
+#pragma unroll
+            for (uint32_t j = 0; j < 2; ++j) {
+              b_col[2 * h + j] = t.n0 + h * kBN + rank * (nh >> 1) + 64 * j;
+              if (j < (nh >> 7)) { b_mask |= 1u << (2 * h + j); ++n_b; }
+            }
+          }
         } else {
-          a_boxes = (c.a_ext - t.m0 > 64u) ? 2u : 1u; b_boxes = t.nw >> 6; bn0 = t.n0;
+          a_boxes = (c.a_ext - t.m0 > 64u) ? 2u : 1u; n_b = t.nw >> 6;
+#pragma unroll
+          for (uint32_t j = 0; j < 4; ++j) { b_col[j] = t.n0 + 64 * j; if (j < n_b) b_mask |= 1u << j; }
         }
-        const uint32_t tx = (a_boxes + b_boxes) * kBoxBytes * kCG;
+        const uint32_t tx = (a_boxes + n_b) * kBoxBytes * kCG;
         for (uint32_t kb = 0; kb < t.nkb; ++kb) {
           ptx::mbar_wait(empty0 + 8 * stage, phase ^ 1);
           if (rank == 0) ptx::mbar_arrive_expect_tx(full0 + 8 * stage, tx);
           const uint32_t fb = full_lead0 + 8 * stage;
-          const uint32_t sa = stage0 + stage * G::kStageBytes, sb = sa + kABytes;
+          const uint32_t sa = stage0 + stage * kStageBytes, sb = sa + kABytes;
           const int k0 = (int)(kb * kBK);
           for (uint32_t h = 0; h < a_boxes; ++h) {
             const int mn = (int)(am0 + 64 * h);
             if constexpr (kCG == 2) ptx::tma_load_2d_cg2(sa + h * kBoxBytes, c.ta, c.a_mn ? mn : k0, c.a_mn ? k0 : mn, fb);
             else ptx::tma_load_2d(sa + h * kBoxBytes, c.ta, c.a_mn ? mn : k0, c.a_mn ? k0 : mn, fb);
           }
-          for (uint32_t j = 0; j < b_boxes; ++j) {
-            const int mn = (int)(bn0 + 64 * j);
-            if constexpr (kCG == 2) ptx::tma_load_2d_cg2(sb + j * kBoxBytes, c.tb, c.b_mn ? mn : k0, c.b_mn ? k0 : mn, fb);
-            else ptx::tma_load_2d(sb + j * kBoxBytes, c.tb, c.b_mn ? mn : k0, c.b_mn ? k0 : mn, fb);
+#pragma unroll
+          for (uint32_t j = 0; j < 4; ++j) {
+            if (b_mask & (1u << j)) {
+              const int mn = (int)b_col[j];
+              const uint32_t dst = sb + j * kBoxBytes;
+              if constexpr (kCG == 2) ptx::tma_load_2d_cg2(dst, c.tb, c.b_mn ? mn : k0, c.b_mn ? k0 : mn, fb);
+              else ptx::tma_load_2d(dst, c.tb, c.b_mn ? mn : k0, c.b_mn ? k0 : mn, fb);
+            }
           }
-          if (++stage == G::kStages) { stage = 0; phase ^= 1; }
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===== UMMA issuer (leader CTA only when paired) =====
-    if (lane == 0 && rank == 0) {
-      uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
-      for (;;) {
-        const uint32_t ti = feed.next_single();
+    // ===== UMMA issuer (leader CTA only when paired).  The whole warp runs the loop converged, so that descriptors,
+    // barrier addresses and the TMEM address are warp-uniform values (uniform registers, no per-instruction
+    // vector->uniform election loops); one elected lane issues the UMMAs and their commits. =====
+    if (rank == 0) {
+      const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem_base, 0);
+      uint32_t stage = 0, phase = 0, tile_no = 0;
+      uint32_t acc_phase = 0;                                      // bit per accumulator
+      for (;; ++tile_no) {
+        const uint32_t ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
+        __syncwarp();
+        feed.release(lane == 0);
         if (ti == kNoTile) break;
         const TcTile t = p.tiles[ti];
         const TcMat M = p.mats[t.mat];
         const TileCfg c = decode(p, t, M);
-        const uint32_t idesc = ptx::idesc_bf16_f32(G::kTileM, t.nw, c.a_mn, c.b_mn);
         // K-major: +32 B per 16-k step; MN-major: +16 rows of 128 B.  (descriptor address field is in 16-byte units)
         const uint32_t a_step = c.a_mn ? (2048u >> 4) : (32u >> 4), b_step = c.b_mn ? (2048u >> 4) : (32u >> 4);
         const uint32_t a_lbo = c.a_mn ? kBoxBytes : 16u, b_lbo = c.b_mn ? kBoxBytes : 16u;
-        ptx::mbar_wait(tempty0 + 8 * acc, acc_phase ^ 1);       // every epilogue warp has drained this accumulator
-        ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + acc * kBNMax;
-        for (uint32_t kb = 0; kb < t.nkb; ++kb) {
-          ptx::mbar_wait(full0 + 8 * stage, phase);
-          ptx::tc_fence_after();
-          const uint32_t sa = stage0 + stage * G::kStageBytes, sb = sa + kABytes;
-          const uint64_t ad = ptx::smem_desc_sw128(sa, a_lbo, 1024), bd = ptx::smem_desc_sw128(sb, b_lbo, 1024);
-#pragma unroll
-          for (uint32_t ks = 0; ks < kBK / 16; ++ks) {
-            if constexpr (kCG == 2)
-              ptx::umma_bf16_cg2(d_tmem, ad + (uint64_t)(ks * a_step), bd + (uint64_t)(ks * b_step), idesc, (kb | ks) != 0);
-            else
-              ptx::umma_bf16(d_tmem, ad + (uint64_t)(ks * a_step), bd + (uint64_t)(ks * b_step), idesc, (kb | ks) != 0);
+        // accumulators of this tile: paired -> halves h = 0 (, 1) in TMEM columns 256 h; single -> one accumulator,
+        // alternating between the two column ranges from tile to tile
+        const uint32_t n_acc = kCG == 2 ? (t.nw > kBN ? 2u : 1u) : 1u;
+        const uint32_t acc0 = kCG == 2 ? 0u : (tile_no & 1u);
+        // The two accumulators of a paired tile are visited in turn; a visit covers kGroup ring stages (switching the
+        // accumulator after every stage measured ~20 % slower UMMA issue than staying on one).
+        for (uint32_t kb = 0; kb < t.nkb; kb += kGroup) {
+          const uint32_t gcnt = min(kGroup, (uint32_t)t.nkb - kb);
+          for (uint32_t s = 0; s < gcnt; ++s) {
+            const uint32_t st = stage + s;
+            ptx::mbar_wait(full0 + 8 * (st % kStages), phase ^ (st >= kStages ? 1u : 0u));
           }
-          // frees the smem slot (in both CTAs when paired) once these MMAs have finished
-          if constexpr (kCG == 2) ptx::umma_commit_cg2(empty0 + 8 * stage); else ptx::umma_commit(empty0 + 8 * stage);
-          if (++stage == G::kStages) { stage = 0; phase ^= 1; }
+          ptx::tc_fence_after();
+          for (uint32_t h = 0; h < n_acc; ++h) {
+            const uint32_t acc = acc0 + h;
+            const uint32_t nh = kCG == 2 ? min((uint32_t)t.nw - h * kBN, kBN) : (uint32_t)t.nw;
+            const uint32_t idesc = ptx::idesc_bf16_f32(kBM * kCG, nh, c.a_mn, c.b_mn);
+            const uint32_t d_tmem = tmem_u + acc * kBN;
+            if (kb == 0) {                                         // every epilogue warp has drained this accumulator
+              ptx::mbar_wait(tempty0 + 8 * acc, ((acc_phase >> acc) & 1u) ^ 1u);
+              ptx::tc_fence_after();
+            }
+            if (ptx::elect_one()) {
+            for (uint32_t s = 0; s < gcnt; ++s) {
+              const uint32_t sa = stage0 + ((stage + s) % kStages) * kStageBytes, sb = sa + kABytes;
+              const uint64_t ad = ptx::smem_desc_sw128(sa, a_lbo, 1024);
+              const uint64_t bd = ptx::smem_desc_sw128(sb + h * 2 * kBoxBytes, b_lbo, 1024);
+#pragma unroll
+              for (uint32_t ks = 0; ks < kBK / 16; ++ks) {
+                if constexpr (kCG == 2)
+                  ptx::umma_bf16_cg2(d_tmem, ad + (uint64_t)(ks * a_step), bd + (uint64_t)(ks * b_step), idesc, (kb | s | ks) != 0);
+                else
+                  ptx::umma_bf16(d_tmem, ad + (uint64_t)(ks * a_step), bd + (uint64_t)(ks * b_step), idesc, (kb | s | ks) != 0);
+              }
+            }
+            if (kb + gcnt == t.nkb) {                              // accumulator complete: hand it to the epilogue warps
+              if constexpr (kCG == 2) ptx::umma_commit_cg2(tfull0 + 8 * acc); else ptx::umma_commit(tfull0 + 8 * acc);
+            }
+            }
+            __syncwarp();
+            if (kb + gcnt == t.nkb) acc_phase ^= 1u << acc;
+          }
+          // free the smem slots (in both CTAs when paired) once these MMAs have finished
+          for (uint32_t s = 0; s < gcnt; ++s) {
+            if (ptx::elect_one()) {
+              if constexpr (kCG == 2) ptx::umma_commit_cg2(empty0 + 8 * stage); else ptx::umma_commit(empty0 + 8 * stage);
+            }
+            __syncwarp();
+            if (++stage == kStages) { stage = 0; phase ^= 1; }
+          }
         }
-        // accumulator ready for the epilogue warps (of both CTAs)
-        if constexpr (kCG == 2) ptx::umma_commit_cg2(tfull0 + 8 * acc); else ptx::umma_commit(tfull0 + 8 * acc);
-        if (++acc == 2) { acc = 0; acc_phase ^= 1; }
       }
     }
   } else {
-    // ===== epilogue: warps 2..5, warp w owns TMEM lanes 32 (w % 4) .. + 31 =====
-    const uint32_t q = warp & 3;
-    uint32_t acc = 0, acc_phase = 0;
+    // ===== epilogue: warps 2..5, warp w owns TMEM lanes 32 (w % 4) .. + 31 = 32 rows of the CTA's 128 =====
+    const uint32_t q = warp & 3, ew = warp - 2;
+    const uint32_t buf0 = epi0 + ew * 2 * kEpiBufBytes;          // two 4 KB staging tiles, used alternately
+    const uint32_t ldbar = epibar0 + 8 * ew;
+    uint32_t ld_phase = 0, n_store = 0, epi_phase = 0, tile_no = 0;
     const uint32_t tempty_lead0 = kCG == 2 ? ptx::mapa(tempty0, 0) : tempty0;
-    for (;;) {
+    const uint32_t sw = (lane & 7) << 4;                         // 128-byte swizzle: 16-byte chunk j of row i sits at j ^ (i & 7)
+    const uint32_t row_smem = lane * 128;
+    for (;; ++tile_no) {
       const uint32_t ti = feed.peek();
       __syncwarp();
       feed.release(lane == 0);
@@ -286,100 +362,117 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       const float inv = p.first ? p.inv_norm[t.mat] : 1.f;
       const float alpha = p.phase == PH_GRAM ? inv * inv : inv;
       const uint32_t rb0 = t.m0 + rank * kBM;                    // first output row of this CTA
-      const uint32_t r = rb0 + q * 32 + lane;                    // output row of this thread
-      const bool row_ok = r < c.out_rows;
-      __nv_bfloat16* out;
-      uint32_t pitch;
-      if (p.phase == PH_GRAM) { out = reinterpret_cast<__nv_bfloat16*>(p.ws + M.a_off); pitch = M.pitch_a; }
-      else if (p.phase == PH_POLY) { out = reinterpret_cast<__nv_bfloat16*>(p.ws + M.p_off); pitch = M.pitch_a; }
-      else { out = reinterpret_cast<__nv_bfloat16*>(p.ws + M.x_off[p.src ^ 1]); pitch = M.pitch_x; }
-      const __nv_bfloat16* Ain = reinterpret_cast<const __nv_bfloat16*>(p.ws + M.a_off);
+      const uint32_t rw0 = rb0 + q * 32;                         // ... of this warp
+      const uint32_t r = rw0 + lane;                             // ... of this thread
+      const bool rows_ok = rw0 < c.out_rows;                     // warp-uniform
       const bool sym = p.phase != PH_APPLY;
+      const uint32_t n_acc = kCG == 2 ? (t.nw > kBN ? 2u : 1u) : 1u;
+      const uint32_t acc0 = kCG == 2 ? 0u : (tile_no & 1u);
+      unsigned long long t_ready = 0ull;
+      long long c_ready = 0ll;
 
-      ptx::mbar_wait(tfull0 + 8 * acc, acc_phase);
-      ptx::tc_fence_after();
-      const unsigned long long t_ready = p.trace ? ptx::globaltimer() : 0ull;
-      const uint32_t taddr0 = tmem_base + ((q * 32u) << 16) + acc * kBNMax;
-      for (uint32_t c0 = 0; c0 < t.nw; c0 += 32) {
-        const uint32_t col0 = t.n0 + c0;
-        if (col0 >= c.out_cols) break;                           // warp-uniform
-        // symmetric outputs: a 128-block below the diagonal is the mirror image of one that is written from above
-        if (sym && (col0 >> 7) < (rb0 >> 7)) continue;           // warp-uniform
-        uint32_t v[32];
-        ptx::tmem_ld32(taddr0 + c0, v);
-        ptx::tmem_ld_wait();
-        float f[32];
-#pragma unroll
-        for (int j = 0; j < 32; ++j) f[j] = __uint_as_float(v[j]);
-        const bool full_cols = col0 + 32 <= c.out_cols;
-        if (p.phase == PH_POLY) {
-          if (row_ok) {
-            const __nv_bfloat16* arow = Ain + (size_t)r * pitch + col0;
-            if (full_cols) {
-#pragma unroll
-              for (int g4 = 0; g4 < 4; ++g4) {
-                const uint4 u = *reinterpret_cast<const uint4*>(arow + 8 * g4);
-                const uint32_t w[4] = {u.x, u.y, u.z, u.w};
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                  const int j = 8 * g4 + 2 * i;
-                  f[j] = fmaf(p.c, f[j], p.b * __uint_as_float(w[i] << 16));
-                  f[j + 1] = fmaf(p.c, f[j + 1], p.b * __uint_as_float(w[i] & 0xffff0000u));
-                }
-              }
-            } else {
-              for (int j = 0; j < 32; ++j)
-                if (col0 + j < c.out_cols) f[j] = fmaf(p.c, f[j], p.b * __bfloat162float(arow[j]));
-            }
-            if (r >= col0 && r < col0 + 32) {                    // the diagonal element: + a
-#pragma unroll
-              for (int j = 0; j < 32; ++j) if (col0 + j == r) f[j] += p.a;
+      for (uint32_t h = 0; h < n_acc; ++h) {
+        const uint32_t acc = acc0 + h;
+        const uint32_t nh = kCG == 2 ? min((uint32_t)t.nw - h * kBN, kBN) : (uint32_t)t.nw;
+        ptx::mbar_wait(tfull0 + 8 * acc, (epi_phase >> acc) & 1u);
+        epi_phase ^= 1u << acc;
+        ptx::tc_fence_after();
+        if (p.trace && h == 0) { t_ready = ptx::globaltimer(); c_ready = clock64(); }
+        const uint32_t taddr0 = tmem_base + ((q * 32u) << 16) + acc * kBN;
+        const uint32_t colh = t.n0 + (kCG == 2 ? h * kBN : 0u);
+        for (uint32_t c0 = 0; c0 < nh; c0 += 64) {
+          const uint32_t col0 = colh + c0;
+          if (col0 >= c.out_cols) break;                         // warp-uniform
+          if (!rows_ok) continue;
+          // symmetric outputs: a 128-block below the diagonal is the mirror image of one that is written from above
+          if (sym && (col0 >> 7) < (rb0 >> 7)) continue;         // warp-uniform
+          const uint32_t buf = buf0 + (n_store & 1u) * kEpiBufBytes;
+          if (lane == 0) {
+            ptx::bulk_wait_read<1>();                            // the store issued two stores ago has released `buf`
+            if (p.phase == PH_POLY) {                            // A tile (32 rows x 64 cols) -> staging, for the b A term
+              ptx::mbar_arrive_expect_tx(ldbar, kEpiBufBytes);
+              ptx::tma_load_2d(buf, c.tain, (int)col0, (int)rw0, ldbar);
             }
           }
-        } else {
+          __syncwarp();
+          uint32_t v[64];
+          {
+            uint32_t lo[32], hi[32];
+            ptx::tmem_ld32(taddr0 + c0, lo);
+            ptx::tmem_ld32(taddr0 + c0 + 32, hi);
+            ptx::tmem_ld_wait();
 #pragma unroll
-          for (int j = 0; j < 32; ++j) f[j] *= alpha;
-        }
-        // direct write: row r, columns col0 .. col0 + 31
-        if (row_ok) {
-          __nv_bfloat16* orow = out + (size_t)r * pitch + col0;
-          if (full_cols) {
+            for (int j = 0; j < 32; ++j) { v[j] = lo[j]; v[32 + j] = hi[j]; }
+          }
+          uint32_t pk[32];                                       // the thread's 64 outputs as bf16 pairs
+          if (p.phase == PH_POLY) {
+            ptx::mbar_wait(ldbar, ld_phase);
+            ld_phase ^= 1u;
+            const bool on_diag = col0 < rw0 + 32u && rw0 < col0 + 64u;   // warp-uniform: the tile crosses the diagonal
 #pragma unroll
-            for (int g4 = 0; g4 < 4; ++g4) {
-              uint4 u;
-              u.x = pack_bf16(f[8 * g4 + 0], f[8 * g4 + 1]); u.y = pack_bf16(f[8 * g4 + 2], f[8 * g4 + 3]);
-              u.z = pack_bf16(f[8 * g4 + 4], f[8 * g4 + 5]); u.w = pack_bf16(f[8 * g4 + 6], f[8 * g4 + 7]);
-              *reinterpret_cast<uint4*>(orow + 8 * g4) = u;
+            for (int j = 0; j < 8; ++j) {
+              uint32_t a4[4];
+              ptx::ld_shared_v4(buf + row_smem + (((uint32_t)j << 4) ^ sw), a4[0], a4[1], a4[2], a4[3]);
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                float f0 = fmaf(p.c, __uint_as_float(v[8 * j + 2 * i]), p.b * __uint_as_float(a4[i] << 16));
+                float f1 = fmaf(p.c, __uint_as_float(v[8 * j + 2 * i + 1]), p.b * __uint_as_float(a4[i] & 0xffff0000u));
+                if (on_diag) {                                   // the diagonal element: + a
+                  if (col0 + 8 * j + 2 * i == r) f0 += p.a;
+                  if (col0 + 8 * j + 2 * i + 1 == r) f1 += p.a;
+                }
+                pk[4 * j + i] = pack_bf16(f0, f1);
+              }
             }
           } else {
+#pragma unroll
             for (int j = 0; j < 32; ++j)
-              if (col0 + j < c.out_cols) orow[j] = __float2bfloat16_rn(f[j]);
+              pk[j] = pack_bf16(alpha * __uint_as_float(v[2 * j]), alpha * __uint_as_float(v[2 * j + 1]));
+          }
+          // direct tile: row `lane` of the staging tile, swizzled; then one TMA store (clipped at the matrix edges)
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            ptx::st_shared_v4(buf + row_smem + (((uint32_t)j << 4) ^ sw), pk[4 * j], pk[4 * j + 1], pk[4 * j + 2], pk[4 * j + 3]);
+          ptx::fence_async_smem();
+          __syncwarp();
+          if (lane == 0) { ptx::tma_store_2d(c.tout, (int)col0, (int)rw0, buf); ptx::bulk_commit(); }
+          ++n_store;
+          // mirror tile of strictly-upper 128-blocks: staged transposed (64 x 32), stored at (row col0, column rw0)
+          if (sym && (col0 >> 7) > (rb0 >> 7)) {
+            const uint32_t mbuf = buf0 + (n_store & 1u) * kEpiBufBytes;
+            if (lane == 0) ptx::bulk_wait_read<1>();
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              ptx::st_shared_b16(mbuf + (2 * j) * 64 + lane * 2, (uint16_t)(pk[j] & 0xffffu));
+              ptx::st_shared_b16(mbuf + (2 * j + 1) * 64 + lane * 2, (uint16_t)(pk[j] >> 16));
+            }
+            ptx::fence_async_smem();
+            __syncwarp();
+            if (lane == 0) { ptx::tma_store_2d(c.tmir, (int)rw0, (int)col0, mbuf); ptx::bulk_commit(); }
+            ++n_store;
           }
         }
-        // mirrored write of strictly-upper 128-blocks (lanes = consecutive r -> 64-byte runs)
-        if (sym && (col0 >> 7) > (rb0 >> 7) && row_ok) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (col0 + j < c.out_cols) out[(size_t)(col0 + j) * pitch + r] = __float2bfloat16_rn(f[j]);
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          if constexpr (kCG == 2) ptx::mbar_arrive_cluster(tempty_lead0 + 8 * acc); else ptx::mbar_arrive(tempty0 + 8 * acc);
         }
       }
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (p.trace && q == 0 && lane == 0 && rank == 0) {         // one record per tile: when its accumulator was ready
-        const unsigned long long slot = atomicAdd(p.trace, 1ull);   // and when this warp had stored its share
+      if (p.trace && q == 0 && lane == 0 && rank == 0) {         // one record per tile: when its (first) accumulator was
+        const unsigned long long slot = atomicAdd(p.trace, 1ull);   // ready and when this warp had issued its stores
         if (slot < p.trace_cap) {
-          unsigned long long* rec = p.trace + 1 + 4 * slot;
+          unsigned long long* rec = p.trace + 1 + 6 * slot;
           rec[0] = ((unsigned long long)p.launch_idx << 32) | ti;
           rec[1] = ((unsigned long long)unit << 32) | ptx::smid();
           rec[2] = t_ready;
           rec[3] = ptx::globaltimer();
+          rec[4] = (unsigned long long)c_ready;
+          rec[5] = ((unsigned long long)t.nkb << 32) | t.nw;
         }
       }
-      if (lane == 0) {
-        if constexpr (kCG == 2) ptx::mbar_arrive_cluster(tempty_lead0 + 8 * acc); else ptx::mbar_arrive(tempty0 + 8 * acc);
-      }
-      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
+    if (lane == 0) ptx::bulk_wait_all();                         // every store of this warp has reached global memory
   }
 
   __syncwarp();
@@ -408,17 +501,19 @@ EncodeTiledFn get_encode() {
   return fn;
 }
 
-// Row-major bf16 matrix rows x cols with row pitch `pitch` elements; box = 64 (inner) x 64 (outer), 128-byte swizzle,
-// out-of-bounds elements read as zero (ragged edges, partial k blocks and whole out-of-range boxes rely on it).
-int make_tmap(CUtensorMap* out, void* base, uint32_t rows, uint32_t cols, uint32_t pitch) {
+// Row-major bf16 matrix rows x cols with row pitch `pitch` elements; box = box_cols (inner) x box_rows (outer);
+// out-of-bounds elements read as zero (ragged edges, partial k blocks and whole out-of-range boxes rely on it) and
+// are dropped by stores.
+int make_tmap(CUtensorMap* out, void* base, uint32_t rows, uint32_t cols, uint32_t pitch, uint32_t box_cols,
+              uint32_t box_rows, CUtensorMapSwizzle swz) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return cuda_fail(cudaErrorSymbolNotFound);
   const cuuint64_t dims[2] = {cols, rows};
   const cuuint64_t strides[1] = {(cuuint64_t)pitch * 2};
-  const cuuint32_t box[2] = {64, 64};
+  const cuuint32_t box[2] = {box_cols, box_rows};
   const cuuint32_t estr[2] = {1, 1};
   const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? MFSDP_OK : cuda_fail(cudaErrorInvalidValue);
 }
@@ -429,35 +524,36 @@ int make_tmap(CUtensorMap* out, void* base, uint32_t rows, uint32_t cols, uint32
 // the tiles that share it as long as the next sharer follows soon enough.  The list is therefore ordered so that a
 // window covers a compact block of the output (`band` row blocks x the column tiles that go with them) and sharers
 // are few entries apart: column-panel sharers adjacent, row-panel sharers `band` entries apart.
-uint16_t tile_n(uint32_t remaining, uint32_t gran) {     // UMMA N of a tile that has `remaining` columns to cover
-  return (uint16_t)std::min(kBNMax, (remaining + gran - 1) / gran * gran);
+uint16_t tile_w(uint32_t remaining, uint32_t cg) {        // width of a tile that has `remaining` columns to cover
+  const uint32_t gran = 64 * cg;
+  return (uint16_t)std::min(kBN * cg, (remaining + gran - 1) / gran * gran);
 }
 // rectangular output (APPLY): column panels of `group` tiles stay L2-resident while all row blocks sweep over them.
 void tiles_rect(std::vector<TcTile>& v, uint32_t mat, uint32_t out_rows, uint32_t out_cols, uint32_t nkb, uint32_t cg) {
-  const uint32_t bm = kBM * cg;
-  const uint32_t tm = (out_rows + bm - 1) / bm, tn = (out_cols + kBNMax - 1) / kBNMax;
+  const uint32_t bm = kBM * cg, bn = kBN * cg;
+  const uint32_t tm = (out_rows + bm - 1) / bm, tn = (out_cols + bn - 1) / bn;
   const uint32_t group = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_RECT_GROUP));
   for (uint32_t g0 = 0; g0 < tn; g0 += group)
     for (uint32_t i = 0; i < tm; ++i)
       for (uint32_t j = g0; j < std::min(tn, g0 + group); ++j)
-        v.push_back(TcTile{mat, i * bm, j * kBNMax, (uint16_t)nkb, tile_n(out_cols - j * kBNMax, 64 * cg)});
+        v.push_back(TcTile{mat, i * bm, j * bn, (uint16_t)nkb, tile_w(out_cols - j * bn, cg)});
 }
 // symmetric output (GRAM, POLY): upper row blocks only; bands of `band` row blocks, inside a band column-major
-// (all row blocks of the band for one 256-column step, then the next step).
+// (all row blocks of the band for one column step of a tile width, then the next step).
 void tiles_sym(std::vector<TcTile>& v, uint32_t mat, uint32_t d, uint32_t nkb, uint32_t cg) {
-  const uint32_t bm = kBM * cg;
+  const uint32_t bm = kBM * cg, bn = kBN * cg;
   const uint32_t tm = (d + bm - 1) / bm;
   const uint32_t band = (uint32_t)std::max(1, tune_value(cg == 2 ? MFSDP_TUNE_SYM_BAND2 : MFSDP_TUNE_SYM_BAND));
   for (uint32_t b0 = 0; b0 < tm; b0 += band) {
     const uint32_t b1 = std::min(tm, b0 + band);
-    for (uint32_t c0 = b0 * bm; c0 < d; c0 += kBNMax)            // 256-column steps from the band's first diagonal
+    for (uint32_t c0 = b0 * bm; c0 < d; c0 += bn)                // column steps from the band's first diagonal
       for (uint32_t i = b0; i < b1; ++i) {
-        // row block i owns columns >= i * bm; clip the step to that range (128 x 256 tiles: N = 128 when only half
-        // of the step is owned; 256 x 256 tiles are aligned with the steps)
+        // row block i owns columns >= i * bm; clip the step to that range (the tile is half as wide when only half
+        // of the step is owned)
         const uint32_t lo = std::max(c0, i * bm);
-        const uint32_t hi = std::min(d, c0 + kBNMax);
+        const uint32_t hi = std::min(d, c0 + bn);
         if (lo >= hi) continue;
-        v.push_back(TcTile{mat, i * bm, lo, (uint16_t)nkb, tile_n(hi - lo, 64 * cg)});
+        v.push_back(TcTile{mat, i * bm, lo, (uint16_t)nkb, tile_w(hi - lo, cg)});
       }
   }
 }
@@ -479,7 +575,7 @@ cudaError_t launch_phase(const TcParams& p, uint32_t units, cudaStream_t st) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(units * kCG);
   cfg.blockDim = dim3(kThreads);
-  cfg.dynamicSmemBytes = Geo<kCG>::kSmemBytes;
+  cfg.dynamicSmemBytes = kSmemBytes;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -494,7 +590,7 @@ int build_tc_plan(Plan& pl) {
   pl.tc = tc;
   const WsLayout& lay = pl.lay;
   uint8_t* ws = static_cast<uint8_t*>(pl.workspace);
-  std::vector<CUtensorMap> maps(4 * lay.mats.size());
+  std::vector<CUtensorMap> maps(TM_COUNT * lay.mats.size());
   std::vector<TcMat> mats(lay.mats.size());
   std::vector<TcTile> tiles[2][3];
   // big matrices first so that the static round-robin over units ends with the cheap tiles
@@ -510,11 +606,20 @@ int build_tc_plan(Plan& pl) {
     m.x_off[0] = L.x_off[0]; m.x_off[1] = L.x_off[1]; m.a_off = L.a_off; m.p_off = L.p_off;
     m.rows = L.rows; m.cols = L.cols; m.d = L.d; m.n_long = L.n_long; m.pitch_x = L.pitch_x; m.pitch_a = L.pitch_a;
     m.tall = L.tall; m.pad = 0;
+    CUtensorMap* tm = &maps[TM_COUNT * i];
+    void *x0 = ws + L.x_off[0], *x1 = ws + L.x_off[1], *pa = ws + L.a_off, *pp = ws + L.p_off;
+    const CUtensorMapSwizzle s128 = CU_TENSOR_MAP_SWIZZLE_128B, s0 = CU_TENSOR_MAP_SWIZZLE_NONE;
     int rc;
-    if ((rc = make_tmap(&maps[4 * i + 0], ws + L.x_off[0], L.rows, L.cols, L.pitch_x)) ||
-        (rc = make_tmap(&maps[4 * i + 1], ws + L.x_off[1], L.rows, L.cols, L.pitch_x)) ||
-        (rc = make_tmap(&maps[4 * i + 2], ws + L.a_off, L.d, L.d, L.pitch_a)) ||
-        (rc = make_tmap(&maps[4 * i + 3], ws + L.p_off, L.d, L.d, L.pitch_a)))
+    if ((rc = make_tmap(tm + TM_X0, x0, L.rows, L.cols, L.pitch_x, 64, 64, s128)) ||
+        (rc = make_tmap(tm + TM_X1, x1, L.rows, L.cols, L.pitch_x, 64, 64, s128)) ||
+        (rc = make_tmap(tm + TM_A, pa, L.d, L.d, L.pitch_a, 64, 64, s128)) ||
+        (rc = make_tmap(tm + TM_P, pp, L.d, L.d, L.pitch_a, 64, 64, s128)) ||
+        (rc = make_tmap(tm + TM_X0_ST, x0, L.rows, L.cols, L.pitch_x, 64, 32, s128)) ||
+        (rc = make_tmap(tm + TM_X1_ST, x1, L.rows, L.cols, L.pitch_x, 64, 32, s128)) ||
+        (rc = make_tmap(tm + TM_A_ST, pa, L.d, L.d, L.pitch_a, 64, 32, s128)) ||
+        (rc = make_tmap(tm + TM_P_ST, pp, L.d, L.d, L.pitch_a, 64, 32, s128)) ||
+        (rc = make_tmap(tm + TM_A_MIR, pa, L.d, L.d, L.pitch_a, 32, 64, s0)) ||
+        (rc = make_tmap(tm + TM_P_MIR, pp, L.d, L.d, L.pitch_a, 32, 64, s0)))
       return rc;
   }
   const uint32_t pair_min_d = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_PAIR_MIN_D));
@@ -535,16 +640,16 @@ int build_tc_plan(Plan& pl) {
   cudaDeviceGetAttribute(&tc->sms, cudaDevAttrMultiProcessorCount, pl.device);
   cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), kMaxLaunches * sizeof(uint32_t));
   if (e != cudaSuccess) return cuda_fail(e);
-  e = cudaFuncSetAttribute(k_ns_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geo<1>::kSmemBytes);
+  e = cudaFuncSetAttribute(k_ns_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return cuda_fail(e);
-  e = cudaFuncSetAttribute(k_ns_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Geo<2>::kSmemBytes);
+  e = cudaFuncSetAttribute(k_ns_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return cuda_fail(e);
   // how many CTA pairs can be co-resident (one CTA per SM; the two CTAs of a pair share a TPC)
   {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)tc->sms / 2 * 2);
     cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = Geo<2>::kSmemBytes;
+    cfg.dynamicSmemBytes = kSmemBytes;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
