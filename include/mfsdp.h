@@ -202,16 +202,18 @@ int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precisio
  *   MFSDP_TUNE_SYM_BAND     row blocks per band of the symmetric (GRAM, POLY) tile order, single-CTA class.  16
  *   MFSDP_TUNE_SYM_BAND2    the same for the CTA-pair class.  8
  *   MFSDP_TUNE_RECT_GROUP   column tiles per panel of the rectangular (APPLY) tile order.  8
+ *   MFSDP_TUNE_WIDE_MIN_KB  CTA-pair tiles are 512 columns wide (else 256) in phases whose k loop has at least this
+ *                           many 64-element blocks.  8
  * Returns MFSDP_EINVAL for an unknown knob or value < 1; mfsdp_get_tune returns the value or a negative code. */
 enum { MFSDP_TUNE_PAIR_MIN_D = 0, MFSDP_TUNE_SYM_BAND = 1, MFSDP_TUNE_SYM_BAND2 = 2, MFSDP_TUNE_RECT_GROUP = 3,
-       MFSDP_TUNE_COUNT_ = 4 };
+       MFSDP_TUNE_WIDE_MIN_KB = 4, MFSDP_TUNE_COUNT_ = 5 };
 int mfsdp_tune(int knob, int value);
 int mfsdp_get_tune(int knob);
 
 /* Debug aid: tile trace of the tensor-core Newton-Schulz kernels.  dev_buf: DEVICE buffer of `bytes` bytes, 8-byte
  * aligned, zeroed by the caller and owned by the caller; NULL switches tracing off (the default).  While set, every
  * NS tile appends one record of six 64-bit words after the counter word dev_buf[0]:
- *   (launch index within the pass << 32 | tile index), (walking unit << 32 | SM id),
+ *   (phase index 3 * iteration + {0 GRAM, 1 POLY, 2 APPLY} << 32 | tile index within the launch), (walking unit << 32 | SM id),
  *   %globaltimer ns when the tile's accumulator was complete, %globaltimer ns when its first epilogue warp was done,
  *   the SM's clock64 at the first instant, (k blocks of the tile << 32 | UMMA N).
  * Records beyond the capacity are dropped (the counter keeps counting).  Returns MFSDP_EINVAL on a misaligned or

@@ -14,6 +14,6 @@ from .binding import (  # noqa: F401
     mfsdp_plan, mfsdp_validate_desc, mfsdp_flat_elems, mfsdp_workspace_bytes, mfsdp_workspace_view,
     mfsdp_debug_ws_offsets, mfsdp_muon_step, mfsdp_muon_momentum_pass, mfsdp_muon_ns_pass, mfsdp_muon_update_pass,
     mfsdp_muon_step_host, mfsdp_adamw_tail_step, mfsdp_strerror, mfsdp_version, mfsdp_launch_count,
-    mfsdp_tune, mfsdp_get_tune, mfsdp_debug_trace, TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP,
+    mfsdp_tune, mfsdp_get_tune, mfsdp_debug_trace, TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB,
     make_desc_array,
 )

@@ -180,7 +180,7 @@ def mfsdp_launch_count():
     return int(load().mfsdp_launch_count())
 
 
-TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP = 0, 1, 2, 3
+TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB = 0, 1, 2, 3, 4
 
 
 def mfsdp_tune(knob, value):

@@ -44,18 +44,22 @@ enum { TM_X0 = 0, TM_X1 = 1, TM_A = 2, TM_P = 3,            // operand loads: bo
 
 struct TcMat {                 // device, one per matrix
   uint64_t x_off[2], a_off, p_off;
-  uint32_t rows, cols, d, n_long, pitch_x, pitch_a, tall, pad;
+  uint32_t rows, cols, d, n_long, pitch_x, pitch_a, tall;
+  uint32_t reports_per_iter;   // completion reports (one per epilogue warp and tile) of one NS iteration of this matrix
 };
 // Output tile: origin (rows, cols of the OUTPUT buffer), k blocks, width in columns (multiple of 64; of 128 when
 // paired; <= 256 single CTA, <= 512 paired).
-struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; };
+// `need`: completion reports of the SAME matrix and iteration that must have been made before this tile's operands
+// may be read (= every tile of the matrix' earlier phases); `phase`: PH_*.
+struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; uint32_t need, phase; };
 
 struct NsTcPlan {
   CUtensorMap* d_tmaps = nullptr;   // TM_COUNT per matrix
   TcMat* d_mats = nullptr;
-  TcTile* d_tiles[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};   // [kCG - 1][phase]
-  uint32_t n_tiles[2][3] = {{0, 0, 0}, {0, 0, 0}};
-  uint32_t* d_counters = nullptr;   // one tile counter per launch of a pass (zeroed at the start of every pass)
+  TcTile* d_tiles[2] = {nullptr, nullptr};   // [kCG - 1]: the tiles of ONE iteration, GRAM then POLY then APPLY
+  uint32_t n_tiles[2] = {0, 0};
+  uint32_t* d_counters = nullptr;   // [2] tile counters (one per class) then [n_mat] completion reports; zeroed per pass
+  uint32_t n_mat = 0;
   int sms = 148;
   int max_pairs = 74;               // co-resident CTA pairs
 };
@@ -79,7 +83,6 @@ constexpr uint32_t kEpiBufBytes = 4096;        // one staging tile: 32 rows x 64
 constexpr uint32_t kEpiBytes = 4 * 2 * kEpiBufBytes;   // 4 epilogue warps x 2 buffers
 constexpr uint32_t kBarBytes = 256;
 constexpr uint32_t kSmemBytes = kStages * kStageBytes + kEpiBytes + kBarBytes + 1024 /*align slack*/;
-constexpr uint32_t kMaxLaunches = 64 * 3 * 2;   // ns_steps <= 64, three phases, two tile classes
 
 struct TcParams {
   const TcTile* tiles;
@@ -88,9 +91,10 @@ struct TcParams {
   const CUtensorMap* tmaps;
   uint8_t* ws;
   const float* inv_norm;
-  int phase, src, first;
+  uint32_t n_iter_tiles, ns_steps;   // the launch walks ns_steps x n_iter_tiles tiles (iteration-major)
   float a, b, c;
   uint32_t* counter;            // dynamic tile scheduler: next unclaimed tile of THIS launch (zero at launch)
+  uint32_t* done;               // [n_mat] completion reports of the pass so far (zero at the start of the pass)
   unsigned long long* trace;    // optional (mfsdp_debug_trace): [0] = record counter, then 6 words per tile
   uint32_t trace_cap, launch_idx;
 };
@@ -103,22 +107,33 @@ struct TileCfg {
   uint32_t out_rows, out_cols;  // bounds of the output buffer
 };
 
-__device__ __forceinline__ TileCfg decode(const TcParams& p, const TcTile& t, const TcMat& M) {
+// One claimed unit of work: tile j of iteration it.
+struct Work { TcTile t; uint32_t it, src, first; };
+__device__ __forceinline__ Work fetch(const TcParams& p, uint32_t ti) {
+  Work w;
+  w.it = ti / p.n_iter_tiles;
+  w.t = p.tiles[ti - w.it * p.n_iter_tiles];
+  w.src = w.it & 1u;
+  w.first = w.it == 0u;
+  return w;
+}
+
+__device__ __forceinline__ TileCfg decode(const TcParams& p, const TcTile& t, const TcMat& M, uint32_t src) {
   TileCfg c;
   const CUtensorMap* tm = p.tmaps + TM_COUNT * (size_t)t.mat;
   c.tmir = nullptr; c.tain = tm + TM_A_ST;
-  if (p.phase == PH_GRAM) {
-    c.ta = c.tb = tm + p.src; c.a_mn = c.b_mn = M.tall; c.a_ext = M.d; c.out_rows = c.out_cols = M.d;
+  if (t.phase == PH_GRAM) {
+    c.ta = c.tb = tm + src; c.a_mn = c.b_mn = M.tall; c.a_ext = M.d; c.out_rows = c.out_cols = M.d;
     c.tout = tm + TM_A_ST; c.tmir = tm + TM_A_MIR;
-  } else if (p.phase == PH_POLY) {
+  } else if (t.phase == PH_POLY) {
     c.ta = c.tb = tm + TM_A; c.a_mn = c.b_mn = 0; c.a_ext = M.d; c.out_rows = c.out_cols = M.d;
     c.tout = tm + TM_P_ST; c.tmir = tm + TM_P_MIR;
   } else if (!M.tall) {          // X_new (d x n) = P (K-major) * X (k x n, MN-major)
-    c.ta = tm + TM_P; c.a_mn = 0; c.a_ext = M.d; c.tb = tm + p.src; c.b_mn = 1;
-    c.out_rows = M.rows; c.out_cols = M.cols; c.tout = tm + TM_X0_ST + (p.src ^ 1);
+    c.ta = tm + TM_P; c.a_mn = 0; c.a_ext = M.d; c.tb = tm + src; c.b_mn = 1;
+    c.out_rows = M.rows; c.out_cols = M.cols; c.tout = tm + TM_X0_ST + (src ^ 1);
   } else {                       // X_new (n x d) = X (K-major) * P^T, P symmetric (K-major)
-    c.ta = tm + p.src; c.a_mn = 0; c.a_ext = M.rows; c.tb = tm + TM_P; c.b_mn = 0;
-    c.out_rows = M.rows; c.out_cols = M.cols; c.tout = tm + TM_X0_ST + (p.src ^ 1);
+    c.ta = tm + src; c.a_mn = 0; c.a_ext = M.rows; c.tb = tm + TM_P; c.b_mn = 0;
+    c.out_rows = M.rows; c.out_cols = M.cols; c.tout = tm + TM_X0_ST + (src ^ 1);
   }
   return c;
 }
@@ -144,11 +159,14 @@ struct Feed {
   uint32_t empty_lead0;                  // the leader's empty barriers as a shared::cluster address (paired) / = empty0
   uint32_t s = 0, ph = 0;
   __device__ __forceinline__ void advance() { if (++s == kFeed) { s = 0; ph ^= 1; } }
-  // leader producer: claim and publish.  Returns the tile index or kNoTile.
+  // leader producer: claim ...
   __device__ __forceinline__ uint32_t claim(uint32_t* counter, uint32_t n_tiles) {
+    const uint32_t ti = atomicAdd(counter, 1u);
+    return ti < n_tiles ? ti : kNoTile;
+  }
+  // ... and publish (after the tile's inputs are known to be complete).
+  __device__ __forceinline__ void publish(uint32_t ti) {
     ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);                // every consumer has read the slot's previous content
-    uint32_t ti = atomicAdd(counter, 1u);
-    if (ti >= n_tiles) ti = kNoTile;
     ptx::st_shared_u32(slots0 + 4 * s, ti);
     if constexpr (kCG == 2) {
       ptx::st_shared_cluster_u32(ptx::mapa(slots0 + 4 * s, 1), ti);
@@ -156,7 +174,11 @@ struct Feed {
     }
     ptx::mbar_arrive(full0 + 8 * s);
     advance();
-    return ti;
+  }
+  // has the next index been published? (non-blocking)
+  __device__ __forceinline__ bool ready() const {
+    if constexpr (kCG == 2) return ptx::mbar_try_wait_cluster(full0 + 8 * s, ph) != 0;
+    else return ptx::mbar_try_wait(full0 + 8 * s, ph) != 0;
   }
   // any other role: wait for the next index ...
   __device__ __forceinline__ uint32_t peek() const {
@@ -191,7 +213,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   feed.full0 = ptx::smem_u32(bars + 2 * kStages + 5);
   feed.empty0 = ptx::smem_u32(bars + 2 * kStages + 5 + kFeed);
   feed.slots0 = ptx::smem_u32(bars + 2 * kStages + 5 + 2 * kFeed);
-  const uint32_t epibar0 = ptx::smem_u32(bars + 2 * kStages + 7 + 2 * kFeed);   // one per epilogue warp (POLY A-tile loads)
   const uint32_t stage0 = ptx::smem_u32(smem);
   const uint32_t epi0 = stage0 + kStages * kStageBytes;
   const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -204,7 +225,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     for (uint32_t s = 0; s < 2; ++s) { ptx::mbar_init(tfull0 + 8 * s, 1); ptx::mbar_init(tempty0 + 8 * s, 4 * kCG); }
     // feed consumers per slot: UMMA issuer + 4 epilogue warps of the leader, producer + 4 epilogue warps of the peer
     for (uint32_t s = 0; s < kFeed; ++s) { ptx::mbar_init(feed.full0 + 8 * s, 1); ptx::mbar_init(feed.empty0 + 8 * s, 5 * kCG); }
-    for (uint32_t s = 0; s < 4; ++s) ptx::mbar_init(epibar0 + 8 * s, 1);
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc<kTmemCols, kCG>(ptx::smem_u32(tmem_holder));
@@ -218,12 +238,38 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     if (lane == 0) {
       uint32_t stage = 0, phase = 0;
       const uint32_t full_lead0 = kCG == 2 ? ptx::mapa(full0, 0) : full0;
+      // the leader claims one tile ahead: the atomic's round trip overlaps with issuing the current tile's loads
+      uint32_t next_ti = rank == 0 ? feed.claim(p.counter, p.n_iter_tiles * p.ns_steps) : 0u;
       for (;;) {
-        const uint32_t ti = rank == 0 ? feed.claim(p.counter, p.n_tiles) : feed.next_single();
+        uint32_t ti;
+        if (rank == 0) {
+          ti = next_ti;
+          if (ti != kNoTile) {
+            // inputs of the tile = outputs of every tile of the same matrix in the preceding phases: wait until all
+            // of them have been reported complete (tiles are claimed in phase order, so those tiles are running or
+            // done, never waiting on a later one)
+            const Work w0 = fetch(p, ti);
+            const uint32_t need = w0.it * p.mats[w0.t.mat].reports_per_iter + w0.t.need;
+            const uint32_t* flag = p.done + w0.t.mat;
+            if (ptx::ld_acquire_gpu(flag) < need) {
+              const long long t0 = clock64();
+              while (ptx::ld_acquire_gpu(flag) < need) {
+                __nanosleep(64);
+                if (clock64() - t0 > 4000000000ll) __trap();
+              }
+            }
+          }
+          feed.publish(ti);
+          if (ti != kNoTile) next_ti = feed.claim(p.counter, p.n_iter_tiles * p.ns_steps);
+        } else {
+          ti = feed.next_single();
+        }
         if (ti == kNoTile) break;
-        const TcTile t = p.tiles[ti];
+        ptx::fence_proxy_async();          // reported (generic-proxy) completion -> this thread's TMA reads
+        const Work w = fetch(p, ti);
+        const TcTile t = w.t;
         const TcMat M = p.mats[t.mat];
-        const TileCfg c = decode(p, t, M);
+        const TileCfg c = decode(p, t, M, w.src);
         const uint32_t am0 = t.m0 + rank * kBM;
         // B boxes of this CTA: single CTA: nw / 64 consecutive boxes.  Paired: per 256-column half h its own half of
         // the panel, nh / 128 boxes (nh = width of the half), stored at box slot 2 h + j.
@@ -276,23 +322,25 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     // vector->uniform election loops); one elected lane issues the UMMAs and their commits. =====
     if (rank == 0) {
       const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem_base, 0);
-      uint32_t stage = 0, phase = 0, tile_no = 0;
+      uint32_t stage = 0, phase = 0, acc_next = 0;
       uint32_t acc_phase = 0;                                      // bit per accumulator
-      for (;; ++tile_no) {
+      for (;;) {
         const uint32_t ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
         __syncwarp();
         feed.release(lane == 0);
         if (ti == kNoTile) break;
-        const TcTile t = p.tiles[ti];
+        const Work w = fetch(p, ti);
+        const TcTile t = w.t;
         const TcMat M = p.mats[t.mat];
-        const TileCfg c = decode(p, t, M);
+        const TileCfg c = decode(p, t, M, w.src);
         // K-major: +32 B per 16-k step; MN-major: +16 rows of 128 B.  (descriptor address field is in 16-byte units)
         const uint32_t a_step = c.a_mn ? (2048u >> 4) : (32u >> 4), b_step = c.b_mn ? (2048u >> 4) : (32u >> 4);
         const uint32_t a_lbo = c.a_mn ? kBoxBytes : 16u, b_lbo = c.b_mn ? kBoxBytes : 16u;
-        // accumulators of this tile: paired -> halves h = 0 (, 1) in TMEM columns 256 h; single -> one accumulator,
-        // alternating between the two column ranges from tile to tile
-        const uint32_t n_acc = kCG == 2 ? (t.nw > kBN ? 2u : 1u) : 1u;
-        const uint32_t acc0 = kCG == 2 ? 0u : (tile_no & 1u);
+        // accumulators of this tile: wider than 256 columns -> both, halves h = 0, 1 in TMEM columns 256 h; else one,
+        // alternating from tile to tile (the epilogue of one such tile overlaps the main loop of the next)
+        const uint32_t n_acc = t.nw > kBN ? 2u : 1u;
+        const uint32_t acc0 = n_acc == 2 ? 0u : acc_next;
+        acc_next = n_acc == 2 ? 0u : acc_next ^ 1u;
         // The two accumulators of a paired tile are visited in turn; a visit covers kGroup ring stages (switching the
         // accumulator after every stage measured ~20 % slower UMMA issue than staying on one).
         for (uint32_t kb = 0; kb < t.nkb; kb += kGroup) {
@@ -346,54 +394,96 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
     // ===== epilogue: warps 2..5, warp w owns TMEM lanes 32 (w % 4) .. + 31 = 32 rows of the CTA's 128 =====
     const uint32_t q = warp & 3, ew = warp - 2;
     const uint32_t buf0 = epi0 + ew * 2 * kEpiBufBytes;          // two 4 KB staging tiles, used alternately
-    const uint32_t ldbar = epibar0 + 8 * ew;
-    uint32_t ld_phase = 0, n_store = 0, epi_phase = 0, tile_no = 0;
+    uint32_t n_store = 0, epi_phase = 0, acc_next = 0;
+    uint32_t pend_mat = kNoTile, pend_seq = 0;                   // tile whose completion has not been reported yet
     const uint32_t tempty_lead0 = kCG == 2 ? ptx::mapa(tempty0, 0) : tempty0;
     const uint32_t sw = (lane & 7) << 4;                         // 128-byte swizzle: 16-byte chunk j of row i sits at j ^ (i & 7)
     const uint32_t row_smem = lane * 128;
-    for (;; ++tile_no) {
+    // Completion report of this warp's share of a tile: its TMA stores have been performed, then a release at gpu
+    // scope.  `newer` = stores issued after the tile's last one: waiting for "all but the newest k <= newer groups"
+    // does not wait for those.  A report is deferred while the next accumulator is already waiting to be drained (then
+    // it is made after that tile's stores, by which time it costs nothing) and made at once otherwise.
+    auto report = [&](uint32_t newer) {
+      if (lane == 0) {
+        if (newer >= 8) ptx::bulk_wait<8>(); else if (newer >= 4) ptx::bulk_wait<4>();
+        else if (newer >= 2) ptx::bulk_wait<2>(); else if (newer >= 1) ptx::bulk_wait<1>(); else ptx::bulk_wait<0>();
+        ptx::fence_proxy_async();
+        ptx::red_release_gpu_add(p.done + pend_mat, 1u);
+      }
+      pend_mat = kNoTile;
+    };
+    for (;;) {
+      // the producer may be waiting for the pending report before it publishes the next tile: never block on the feed
+      // with a report outstanding
+      if (pend_mat != kNoTile && !__shfl_sync(0xffffffffu, (uint32_t)feed.ready(), 0)) report(n_store - pend_seq);
       const uint32_t ti = feed.peek();
       __syncwarp();
       feed.release(lane == 0);
       if (ti == kNoTile) break;
-      const TcTile t = p.tiles[ti];
+      const Work w = fetch(p, ti);
+      const TcTile t = w.t;
       const TcMat M = p.mats[t.mat];
-      const TileCfg c = decode(p, t, M);
-      const float inv = p.first ? p.inv_norm[t.mat] : 1.f;
-      const float alpha = p.phase == PH_GRAM ? inv * inv : inv;
+      const TileCfg c = decode(p, t, M, w.src);
+      const float inv = w.first ? p.inv_norm[t.mat] : 1.f;
+      const float alpha = t.phase == PH_GRAM ? inv * inv : inv;
       const uint32_t rb0 = t.m0 + rank * kBM;                    // first output row of this CTA
       const uint32_t rw0 = rb0 + q * 32;                         // ... of this warp
       const uint32_t r = rw0 + lane;                             // ... of this thread
       const bool rows_ok = rw0 < c.out_rows;                     // warp-uniform
-      const bool sym = p.phase != PH_APPLY;
-      const uint32_t n_acc = kCG == 2 ? (t.nw > kBN ? 2u : 1u) : 1u;
-      const uint32_t acc0 = kCG == 2 ? 0u : (tile_no & 1u);
+      const bool sym = t.phase != PH_APPLY;
+      const bool poly = t.phase == PH_POLY;
+      const uint32_t n_acc = t.nw > kBN ? 2u : 1u;
+      const uint32_t acc0 = n_acc == 2 ? 0u : acc_next;
+      acc_next = n_acc == 2 ? 0u : acc_next ^ 1u;
       unsigned long long t_ready = 0ull;
       long long c_ready = 0ll;
+      // chunks of 64 columns; chunk cc lives in accumulator acc0 + cc / 4.  Which chunks this warp writes:
+      const uint32_t n_chunks = min((uint32_t)t.nw, c.out_cols - t.n0 + 63u) >> 6;
+      auto writes = [&](uint32_t cc) {       // warp-uniform
+        // symmetric outputs: a 128-block below the diagonal is the mirror image of one that is written from above
+        return cc < n_chunks && rows_ok && !(sym && ((t.n0 + 64 * cc) >> 7) < (rb0 >> 7));
+      };
+      // POLY: this thread's 64 A values of a chunk (row r, 128 contiguous bytes), fetched one chunk ahead through L2
+      // (A was written by other SMs during this launch: no L1)
+      const __nv_bfloat16* arow = reinterpret_cast<const __nv_bfloat16*>(p.ws + M.a_off) + (size_t)r * M.pitch_a + t.n0;
+      const bool a_ok = poly && r < c.out_rows;
+      uint4 an[8];
+      auto fetch_a = [&](uint32_t cc) {
+        if (a_ok && writes(cc)) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) an[j] = ptx::ld_global_cg_v4(arow + 64 * cc + 8 * j);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) an[j] = make_uint4(0u, 0u, 0u, 0u);
+        }
+      };
+      uint32_t first_cc = 0;
+      while (first_cc < n_chunks && !writes(first_cc)) ++first_cc;
+      if (poly) fetch_a(first_cc);
 
       for (uint32_t h = 0; h < n_acc; ++h) {
         const uint32_t acc = acc0 + h;
-        const uint32_t nh = kCG == 2 ? min((uint32_t)t.nw - h * kBN, kBN) : (uint32_t)t.nw;
+        if (pend_mat != kNoTile && h == 0 &&
+            !__shfl_sync(0xffffffffu, ptx::mbar_try_wait(tfull0 + 8 * acc, (epi_phase >> acc) & 1u), 0))
+          report(n_store - pend_seq);                            // the accumulator is not ready anyway: report now
         ptx::mbar_wait(tfull0 + 8 * acc, (epi_phase >> acc) & 1u);
         epi_phase ^= 1u << acc;
         ptx::tc_fence_after();
         if (p.trace && h == 0) { t_ready = ptx::globaltimer(); c_ready = clock64(); }
         const uint32_t taddr0 = tmem_base + ((q * 32u) << 16) + acc * kBN;
-        const uint32_t colh = t.n0 + (kCG == 2 ? h * kBN : 0u);
-        for (uint32_t c0 = 0; c0 < nh; c0 += 64) {
-          const uint32_t col0 = colh + c0;
-          if (col0 >= c.out_cols) break;                         // warp-uniform
-          if (!rows_ok) continue;
-          // symmetric outputs: a 128-block below the diagonal is the mirror image of one that is written from above
-          if (sym && (col0 >> 7) < (rb0 >> 7)) continue;         // warp-uniform
-          const uint32_t buf = buf0 + (n_store & 1u) * kEpiBufBytes;
-          if (lane == 0) {
-            ptx::bulk_wait_read<1>();                            // the store issued two stores ago has released `buf`
-            if (p.phase == PH_POLY) {                            // A tile (32 rows x 64 cols) -> staging, for the b A term
-              ptx::mbar_arrive_expect_tx(ldbar, kEpiBufBytes);
-              ptx::tma_load_2d(buf, c.tain, (int)col0, (int)rw0, ldbar);
-            }
+        for (uint32_t cc = 4 * h; cc < 4 * h + 4; ++cc) {
+          if (!writes(cc)) continue;
+          const uint32_t c0 = 64 * (cc & 3u), col0 = t.n0 + 64 * cc;
+          uint4 a4[8];
+          if (poly) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) a4[j] = an[j];
+            uint32_t nx = cc + 1;
+            while (nx < n_chunks && !writes(nx)) ++nx;
+            fetch_a(nx);                                         // next chunk's A values: in flight during this chunk
           }
+          const uint32_t buf = buf0 + (n_store & 1u) * kEpiBufBytes;
+          if (lane == 0) ptx::bulk_wait_read<1>();               // the store issued two stores ago has released `buf`
           __syncwarp();
           uint32_t v[64];
           {
@@ -405,18 +495,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
             for (int j = 0; j < 32; ++j) { v[j] = lo[j]; v[32 + j] = hi[j]; }
           }
           uint32_t pk[32];                                       // the thread's 64 outputs as bf16 pairs
-          if (p.phase == PH_POLY) {
-            ptx::mbar_wait(ldbar, ld_phase);
-            ld_phase ^= 1u;
-            const bool on_diag = col0 < rw0 + 32u && rw0 < col0 + 64u;   // warp-uniform: the tile crosses the diagonal
+          if (poly) {
+            const bool on_diag = col0 < rw0 + 32u && rw0 < col0 + 64u;   // warp-uniform: the chunk crosses the diagonal
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-              uint32_t a4[4];
-              ptx::ld_shared_v4(buf + row_smem + (((uint32_t)j << 4) ^ sw), a4[0], a4[1], a4[2], a4[3]);
+              const uint32_t aw[4] = {a4[j].x, a4[j].y, a4[j].z, a4[j].w};
 #pragma unroll
               for (int i = 0; i < 4; ++i) {
-                float f0 = fmaf(p.c, __uint_as_float(v[8 * j + 2 * i]), p.b * __uint_as_float(a4[i] << 16));
-                float f1 = fmaf(p.c, __uint_as_float(v[8 * j + 2 * i + 1]), p.b * __uint_as_float(a4[i] & 0xffff0000u));
+                float f0 = fmaf(p.c, __uint_as_float(v[8 * j + 2 * i]), p.b * __uint_as_float(aw[i] << 16));
+                float f1 = fmaf(p.c, __uint_as_float(v[8 * j + 2 * i + 1]), p.b * __uint_as_float(aw[i] & 0xffff0000u));
                 if (on_diag) {                                   // the diagonal element: + a
                   if (col0 + 8 * j + 2 * i == r) f0 += p.a;
                   if (col0 + 8 * j + 2 * i + 1 == r) f1 += p.a;
@@ -459,11 +546,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
           if constexpr (kCG == 2) ptx::mbar_arrive_cluster(tempty_lead0 + 8 * acc); else ptx::mbar_arrive(tempty0 + 8 * acc);
         }
       }
+      if (pend_mat != kNoTile) report(n_store - pend_seq);       // the previous tile: its stores are at least a tile old
+      pend_mat = t.mat;
+      pend_seq = n_store;
       if (p.trace && q == 0 && lane == 0 && rank == 0) {         // one record per tile: when its (first) accumulator was
         const unsigned long long slot = atomicAdd(p.trace, 1ull);   // ready and when this warp had issued its stores
         if (slot < p.trace_cap) {
           unsigned long long* rec = p.trace + 1 + 6 * slot;
-          rec[0] = ((unsigned long long)p.launch_idx << 32) | ti;
+          rec[0] = ((unsigned long long)(3u * w.it + t.phase) << 32) | ti;
           rec[1] = ((unsigned long long)unit << 32) | ptx::smid();
           rec[2] = t_ready;
           rec[3] = ptx::globaltimer();
@@ -472,7 +562,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
         }
       }
     }
-    if (lane == 0) ptx::bulk_wait_all();                         // every store of this warp has reached global memory
+    if (pend_mat != kNoTile) report(n_store - pend_seq);
   }
 
   __syncwarp();
@@ -524,24 +614,25 @@ int make_tmap(CUtensorMap* out, void* base, uint32_t rows, uint32_t cols, uint32
 // the tiles that share it as long as the next sharer follows soon enough.  The list is therefore ordered so that a
 // window covers a compact block of the output (`band` row blocks x the column tiles that go with them) and sharers
 // are few entries apart: column-panel sharers adjacent, row-panel sharers `band` entries apart.
-uint16_t tile_w(uint32_t remaining, uint32_t cg) {        // width of a tile that has `remaining` columns to cover
+uint16_t tile_w(uint32_t remaining, uint32_t cg, uint32_t bn) {   // width of a tile that has `remaining` columns to cover
   const uint32_t gran = 64 * cg;
-  return (uint16_t)std::min(kBN * cg, (remaining + gran - 1) / gran * gran);
+  return (uint16_t)std::min(bn, (remaining + gran - 1) / gran * gran);
 }
 // rectangular output (APPLY): column panels of `group` tiles stay L2-resident while all row blocks sweep over them.
-void tiles_rect(std::vector<TcTile>& v, uint32_t mat, uint32_t out_rows, uint32_t out_cols, uint32_t nkb, uint32_t cg) {
-  const uint32_t bm = kBM * cg, bn = kBN * cg;
+void tiles_rect(std::vector<TcTile>& v, uint32_t mat, uint32_t out_rows, uint32_t out_cols, uint32_t nkb, uint32_t cg,
+                uint32_t bn, uint32_t phase) {
+  const uint32_t bm = kBM * cg;
   const uint32_t tm = (out_rows + bm - 1) / bm, tn = (out_cols + bn - 1) / bn;
   const uint32_t group = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_RECT_GROUP));
   for (uint32_t g0 = 0; g0 < tn; g0 += group)
     for (uint32_t i = 0; i < tm; ++i)
       for (uint32_t j = g0; j < std::min(tn, g0 + group); ++j)
-        v.push_back(TcTile{mat, i * bm, j * bn, (uint16_t)nkb, tile_w(out_cols - j * bn, cg)});
+        v.push_back(TcTile{mat, i * bm, j * bn, (uint16_t)nkb, tile_w(out_cols - j * bn, cg, bn), 0u, phase});
 }
 // symmetric output (GRAM, POLY): upper row blocks only; bands of `band` row blocks, inside a band column-major
 // (all row blocks of the band for one column step of a tile width, then the next step).
-void tiles_sym(std::vector<TcTile>& v, uint32_t mat, uint32_t d, uint32_t nkb, uint32_t cg) {
-  const uint32_t bm = kBM * cg, bn = kBN * cg;
+void tiles_sym(std::vector<TcTile>& v, uint32_t mat, uint32_t d, uint32_t nkb, uint32_t cg, uint32_t bn, uint32_t phase) {
+  const uint32_t bm = kBM * cg;
   const uint32_t tm = (d + bm - 1) / bm;
   const uint32_t band = (uint32_t)std::max(1, tune_value(cg == 2 ? MFSDP_TUNE_SYM_BAND2 : MFSDP_TUNE_SYM_BAND));
   for (uint32_t b0 = 0; b0 < tm; b0 += band) {
@@ -553,7 +644,7 @@ void tiles_sym(std::vector<TcTile>& v, uint32_t mat, uint32_t d, uint32_t nkb, u
         const uint32_t lo = std::max(c0, i * bm);
         const uint32_t hi = std::min(d, c0 + bn);
         if (lo >= hi) continue;
-        v.push_back(TcTile{mat, i * bm, lo, (uint16_t)nkb, tile_w(hi - lo, cg)});
+        v.push_back(TcTile{mat, i * bm, lo, (uint16_t)nkb, tile_w(hi - lo, cg, bn), 0u, phase});
       }
   }
 }
@@ -571,7 +662,7 @@ int dev_upload(T** dptr, const std::vector<T>& h) {
 }
 
 template <int kCG>
-cudaError_t launch_phase(const TcParams& p, uint32_t units, cudaStream_t st) {
+cudaError_t launch_class(const TcParams& p, uint32_t units, cudaStream_t st) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(units * kCG);
   cfg.blockDim = dim3(kThreads);
@@ -592,7 +683,7 @@ int build_tc_plan(Plan& pl) {
   uint8_t* ws = static_cast<uint8_t*>(pl.workspace);
   std::vector<CUtensorMap> maps(TM_COUNT * lay.mats.size());
   std::vector<TcMat> mats(lay.mats.size());
-  std::vector<TcTile> tiles[2][3];
+  std::vector<TcTile> tiles[2];
   // big matrices first so that the static round-robin over units ends with the cheap tiles
   std::vector<uint32_t> order(lay.mats.size());
   for (uint32_t i = 0; i < order.size(); ++i) order[i] = i;
@@ -605,7 +696,7 @@ int build_tc_plan(Plan& pl) {
     TcMat& m = mats[i];
     m.x_off[0] = L.x_off[0]; m.x_off[1] = L.x_off[1]; m.a_off = L.a_off; m.p_off = L.p_off;
     m.rows = L.rows; m.cols = L.cols; m.d = L.d; m.n_long = L.n_long; m.pitch_x = L.pitch_x; m.pitch_a = L.pitch_a;
-    m.tall = L.tall; m.pad = 0;
+    m.tall = L.tall; m.reports_per_iter = 0;
     CUtensorMap* tm = &maps[TM_COUNT * i];
     void *x0 = ws + L.x_off[0], *x1 = ws + L.x_off[1], *pa = ws + L.a_off, *pp = ws + L.p_off;
     const CUtensorMapSwizzle s128 = CU_TENSOR_MAP_SWIZZLE_128B, s0 = CU_TENSOR_MAP_SWIZZLE_NONE;
@@ -622,23 +713,40 @@ int build_tc_plan(Plan& pl) {
         (rc = make_tmap(tm + TM_P_MIR, pp, L.d, L.d, L.pitch_a, 32, 64, s0)))
       return rc;
   }
+  // One iteration's tiles per class, phase-major (all GRAM tiles, then POLY, then APPLY): a launch walks this list
+  // ns_steps times.  Paired tiles are 512 columns wide (one pass over the A operand feeds two accumulators) when the
+  // k loop is long enough to hide the non-overlapped part of their epilogue, else 256 wide (double-buffered).
   const uint32_t pair_min_d = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_PAIR_MIN_D));
-  for (uint32_t i : order) {
-    const MatLayout& L = lay.mats[i];
-    const uint32_t cg = L.d >= pair_min_d ? 2u : 1u;
-    tiles_sym(tiles[cg - 1][PH_GRAM], i, L.d, (L.n_long + kBK - 1) / kBK, cg);
-    tiles_sym(tiles[cg - 1][PH_POLY], i, L.d, (L.d + kBK - 1) / kBK, cg);
-    tiles_rect(tiles[cg - 1][PH_APPLY], i, L.rows, L.cols, (L.d + kBK - 1) / kBK, cg);
+  const uint32_t wide_min_kb = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_WIDE_MIN_KB));
+  std::vector<uint32_t> cls(lay.mats.size());
+  for (uint32_t ph = 0; ph < 3; ++ph)
+    for (uint32_t i : order) {
+      const MatLayout& L = lay.mats[i];
+      const uint32_t cg = cls[i] = L.d >= pair_min_d ? 2u : 1u;
+      const uint32_t nkb = ((ph == PH_GRAM ? L.n_long : L.d) + kBK - 1) / kBK;
+      const uint32_t bn = cg == 2 && nkb >= wide_min_kb ? 2 * kBN : kBN;
+      if (ph == PH_APPLY) tiles_rect(tiles[cg - 1], i, L.rows, L.cols, nkb, cg, bn, ph);
+      else tiles_sym(tiles[cg - 1], i, L.d, nkb, cg, bn, ph);
+    }
+  // dependencies: a tile needs every completion report of its matrix' earlier phases (4 epilogue warps per CTA report)
+  for (int g = 0; g < 2; ++g) {
+    const uint32_t per_tile = 4u * (uint32_t)(g + 1);
+    std::vector<uint32_t> cnt[3];
+    for (int ph = 0; ph < 3; ++ph) cnt[ph].assign(lay.mats.size(), 0u);
+    for (const TcTile& t : tiles[g]) cnt[t.phase][t.mat] += per_tile;
+    for (TcTile& t : tiles[g]) t.need = (t.phase >= 1 ? cnt[0][t.mat] : 0u) + (t.phase >= 2 ? cnt[1][t.mat] : 0u);
+    for (size_t i = 0; i < lay.mats.size(); ++i)
+      if (cls[i] == (uint32_t)g + 1) mats[i].reports_per_iter = cnt[0][i] + cnt[1][i] + cnt[2][i];
   }
   int rc;
   if ((rc = dev_upload(&tc->d_tmaps, maps)) || (rc = dev_upload(&tc->d_mats, mats))) return rc;
-  for (int g = 0; g < 2; ++g)
-    for (int ph = 0; ph < 3; ++ph) {
-      tc->n_tiles[g][ph] = (uint32_t)tiles[g][ph].size();
-      if ((rc = dev_upload(&tc->d_tiles[g][ph], tiles[g][ph]))) return rc;
-    }
+  for (int g = 0; g < 2; ++g) {
+    tc->n_tiles[g] = (uint32_t)tiles[g].size();
+    if ((rc = dev_upload(&tc->d_tiles[g], tiles[g]))) return rc;
+  }
+  tc->n_mat = (uint32_t)lay.mats.size();
   cudaDeviceGetAttribute(&tc->sms, cudaDevAttrMultiProcessorCount, pl.device);
-  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), kMaxLaunches * sizeof(uint32_t));
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), (2 + (size_t)tc->n_mat) * sizeof(uint32_t));
   if (e != cudaSuccess) return cuda_fail(e);
   e = cudaFuncSetAttribute(k_ns_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return cuda_fail(e);
@@ -667,8 +775,7 @@ int build_tc_plan(Plan& pl) {
 void destroy_ns_tc(NsTcPlan* p) {
   if (!p) return;
   cudaFree(p->d_tmaps); cudaFree(p->d_mats); cudaFree(p->d_counters);
-  for (int g = 0; g < 2; ++g)
-    for (int ph = 0; ph < 3; ++ph) cudaFree(p->d_tiles[g][ph]);
+  for (int g = 0; g < 2; ++g) cudaFree(p->d_tiles[g]);
   delete p;
 }
 
@@ -686,31 +793,28 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
   p.a = (float)hp.a; p.b = (float)hp.b; p.c = (float)hp.c;
   get_trace(&p.trace, &p.trace_cap);
   p.launch_idx = 0;
+  p.ns_steps = (uint32_t)hp.ns_steps;
+  p.done = tc.d_counters + 2;
   {
-    const cudaError_t e = cudaMemsetAsync(tc.d_counters, 0, kMaxLaunches * sizeof(uint32_t), st);
+    const cudaError_t e = cudaMemsetAsync(tc.d_counters, 0, (2 + (size_t)tc.n_mat) * sizeof(uint32_t), st);
     if (e != cudaSuccess) return cuda_fail(e);
   }
-  for (int it = 0; it < hp.ns_steps; ++it) {
-    p.src = it & 1;
-    p.first = (it == 0);
-    for (int ph = 0; ph < 3; ++ph) {
-      p.phase = ph;
-      // the two tile classes touch disjoint matrices: their launches of one phase are independent
-      for (int g = 1; g >= 0; --g) {
-        p.tiles = tc.d_tiles[g][ph];
-        p.n_tiles = tc.n_tiles[g][ph];
-        if (p.n_tiles == 0) continue;
-        p.counter = tc.d_counters + p.launch_idx;
-        cudaError_t e;
-        if (g == 1) e = launch_phase<2>(p, std::min<uint32_t>(p.n_tiles, (uint32_t)tc.max_pairs), st);
-        else e = launch_phase<1>(p, std::min<uint32_t>(p.n_tiles, (uint32_t)tc.sms), st);
-        if (e != cudaSuccess) return cuda_fail(e);
-        ++p.launch_idx;
-        count_launch();
-        const int rc = check_last_launch();
-        if (rc) return rc;
-      }
-    }
+  // ONE launch per tile class for the whole pass (all iterations, all phases); the two classes touch disjoint matrices
+  for (int g = 1; g >= 0; --g) {
+    p.tiles = tc.d_tiles[g];
+    p.n_iter_tiles = tc.n_tiles[g];
+    if (p.n_iter_tiles == 0) continue;
+    p.counter = tc.d_counters + g;
+    const uint64_t total = (uint64_t)p.n_iter_tiles * p.ns_steps;
+    if (total >= 0xffffffffull) return MFSDP_EINVAL;
+    cudaError_t e;
+    if (g == 1) e = launch_class<2>(p, (uint32_t)std::min<uint64_t>(total, (uint64_t)tc.max_pairs), st);
+    else e = launch_class<1>(p, (uint32_t)std::min<uint64_t>(total, (uint64_t)tc.sms), st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    ++p.launch_idx;
+    count_launch();
+    const int rc = check_last_launch();
+    if (rc) return rc;
   }
   return MFSDP_OK;
 }
