@@ -39,6 +39,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--paper-setting", action="store_true",
+                    help="the paper's own Muon hyper-parameters (PAPER.md:121): momentum 0.5, 2 NS steps, lr 1e-3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -56,6 +58,32 @@ def ns_flops(rows, cols, K):
 def elementwise_bytes(rows, cols, wbytes):
     n = rows * cols
     return dict(mom=n * (wbytes + 4 + 4 + 2), upd=n * (wbytes + 2 + wbytes))
+
+
+def apply_setting(wl, args):
+    """--paper-setting: PAPER.md:121 "Muon uses lr 1e-3, weight decay 1e-2, momentum 0.5, 2 NS steps, match_rms_adamw"
+    (second timed workload on the same descriptors); AdamW betas (0.9, 0.999)."""
+    if args.paper_setting:
+        wl.muon.update(momentum=0.5, ns_steps=2, lr=1e-3, weight_decay=1e-2)
+        wl.adamw.update(beta2=0.999)
+        wl.name += "+paper_setting(mu0.5,K2)"
+    return wl
+
+
+def ncu_traffic(workload):
+    """DRAM bytes of one k_ns_tc launch (dram__bytes_read.sum + dram__bytes_write.sum of an `ncu --set full` capture of
+    this same command), copied by hand into profiles/ncu_traffic.csv: lines `workload,kernel,bytes`.  None if absent."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 3 and f[0] == workload and f[1] == "k_ns_tc":
+            try:
+                return float(f[2])
+            except ValueError:
+                return None
+    return None
 
 
 def peaks():
@@ -130,20 +158,17 @@ def plan_for(wl, rank_override=None):
 
 
 def oracle_sample(wl, desc, budget_flops=2.5e12):
-    """A bounded sample of the resident set for the fp64 oracle: the distinct matrix shapes, smallest NS cost first,
-    one matrix per shape, until ~budget_flops dense fp64 flops (about 10-30 s of dgemm on the host cores)."""
+    """A bounded sample of the resident set for the fp64 oracle: resident matrices, cheapest NS cost first, until
+    ~budget_flops dense fp64 flops (about 10-30 s of dgemm on the host cores); at least one matrix."""
     import workloads
     K = wl.muon["ns_steps"]
     mats = [d for d in desc if d["role"] == workloads.ROLE_MATRIX]
-    seen, sample, acc = set(), [], 0.0
+    sample, acc = [], 0.0
     for d in sorted(mats, key=lambda d: ns_flops(d["rows"], d["cols"], K)[1]):
-        key = (d["rows"], d["cols"])
-        if key in seen:
-            continue
         f = ns_flops(d["rows"], d["cols"], K)[1]
         if sample and acc + f > budget_flops:
             break
-        seen.add(key); sample.append(d); acc += f
+        sample.append(d); acc += f
     return sample
 
 
@@ -180,7 +205,10 @@ def time_oracle(wl, sample, steps=1):
 
 
 def sample_text(sample):
-    return "one matrix per shape: " + ", ".join("%dx%d" % (d["rows"], d["cols"]) for d in sample)
+    shapes = {}
+    for d in sample:
+        shapes[(d["rows"], d["cols"])] = shapes.get((d["rows"], d["cols"]), 0) + 1
+    return "cheapest resident matrices: " + ", ".join("%d x %dx%d" % (n, r, c) for (r, c), n in shapes.items())
 
 
 def run_reference(args):
@@ -189,7 +217,7 @@ def run_reference(args):
     if rank != 0:
         return
     import workloads
-    wl = workloads.get(args.config)
+    wl = apply_setting(workloads.get(args.config), args)
     pl = plan_for(wl)
     sample = oracle_sample(wl, pl["desc"], budget_flops=1.0e12)
     for _ in range(max(0, min(args.warmup, 1))):
@@ -262,7 +290,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     mf.load()
 
-    wl = workloads.get(args.config)
+    wl = apply_setting(workloads.get(args.config), args)
     order = rank_order_by_load(mf, wl)
     plan_rank = choose_plan_rank(order, wl.rank, rank, world)
     pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, plan_rank)
@@ -366,8 +394,9 @@ def run_ours(args):
                             n_mat_el * wbytes > 256e6 else "working set may fit L2 (not flushed)",
                             ns_flops_alg=f_alg, ns_flops_dense=f_dense),
                 gpu_launches=launches_all, clocks=clocks)
-    line["roofline"] = dict(bound="tensor", kernel="k_ns_tc (15 phase launches per step)", achieved=ns_tflops,
-                            peak=pk["tc_sustained"], unit="TFLOP/s", frac=ns_tflops / pk["tc_sustained"], traffic=None,
+    line["roofline"] = dict(bound="tensor", kernel="k_ns_tc (one launch per tile class walks all iterations and phases)",
+                            achieved=ns_tflops, peak=pk["tc_sustained"], unit="TFLOP/s",
+                            frac=ns_tflops / pk["tc_sustained"], traffic=ncu_traffic(wl.name),
                             peak_source=pk["src"] + ", sustained bf16", frac_of_burst=ns_tflops / pk["tc_burst"],
                             dense_equiv_tflops=f_dense / (t_ns * 1e-3) / 1e12, ms=t_ns)
     line["passes"] = dict(

@@ -201,7 +201,7 @@ int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precisio
  *                           256 x 256 tiles); smaller ones on single CTAs (128 x N tiles).  default 768
  *   MFSDP_TUNE_SYM_BAND     row blocks per band of the symmetric (GRAM, POLY) tile order, single-CTA class.  16
  *   MFSDP_TUNE_SYM_BAND2    the same for the CTA-pair class.  8
- *   MFSDP_TUNE_RECT_GROUP   column tiles per panel of the rectangular (APPLY) tile order.  8
+ *   MFSDP_TUNE_RECT_GROUP   column tiles per panel of the rectangular (APPLY) tile order.  4
  *   MFSDP_TUNE_WIDE_MIN_KB  CTA-pair tiles are 512 columns wide (else 256) in phases whose k loop has at least this
  *                           many 64-element blocks.  8
  * Returns MFSDP_EINVAL for an unknown knob or value < 1; mfsdp_get_tune returns the value or a negative code. */

@@ -28,7 +28,7 @@ void tune_init() {
   static const char* names[MFSDP_TUNE_COUNT_] = {"MFSDP_TUNE_PAIR_MIN_D", "MFSDP_TUNE_SYM_BAND",
                                                  "MFSDP_TUNE_SYM_BAND2", "MFSDP_TUNE_RECT_GROUP",
                                                  "MFSDP_TUNE_WIDE_MIN_KB"};
-  static const int dflt[MFSDP_TUNE_COUNT_] = {768, 16, 8, 8, 8};
+  static const int dflt[MFSDP_TUNE_COUNT_] = {768, 16, 8, 4, 8};
   for (int k = 0; k < MFSDP_TUNE_COUNT_; ++k) {
     const char* e = getenv(names[k]);
     const int v = e && *e ? atoi(e) : 0;

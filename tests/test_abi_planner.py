@@ -162,3 +162,30 @@ def test_step_entry_points_reject_bad_arguments_without_a_gpu():
         rc = lib.mfsdp_muon_step(pr.desc, n, 1024, 1024, 1024, 1024, 1 << 30, ctypes.byref(hp), None)
         assert rc == mf.EARCH, "no device must mean MFSDP_EARCH, never a CPU fallback"
         assert "no CPU fallback" in mf.mfsdp_strerror(mf.EARCH)
+
+
+def test_tune_knobs_roundtrip_and_reject_bad_values():
+    """mfsdp_tune / mfsdp_get_tune are host-only: defaults, round trip, error codes (no device needed)."""
+    knobs = [mf.TUNE_PAIR_MIN_D, mf.TUNE_SYM_BAND, mf.TUNE_SYM_BAND2, mf.TUNE_RECT_GROUP, mf.TUNE_WIDE_MIN_KB]
+    old = [mf.mfsdp_get_tune(k) for k in knobs]
+    assert all(v >= 1 for v in old)
+    try:
+        for k in knobs:
+            mf.mfsdp_tune(k, 3)
+            assert mf.mfsdp_get_tune(k) == 3
+        for bad in ((-1, 1), (len(knobs), 1), (0, 0), (0, -5)):
+            with pytest.raises(mf.MfsdpError) as e:
+                mf.mfsdp_tune(*bad)
+            assert e.value.code == mf.EINVAL
+        with pytest.raises(mf.MfsdpError):
+            mf.mfsdp_get_tune(99)
+    finally:
+        for k, v in zip(knobs, old):
+            mf.mfsdp_tune(k, v)
+
+
+def test_debug_trace_rejects_bad_buffers():
+    lib = mf.load()
+    assert lib.mfsdp_debug_trace(ctypes.c_void_p(8), 16) == mf.EINVAL       # too small
+    assert lib.mfsdp_debug_trace(ctypes.c_void_p(12), 4096) == mf.EINVAL    # not 8-byte aligned
+    assert lib.mfsdp_debug_trace(None, 0) == 0                              # off

@@ -245,3 +245,31 @@ def test_launch_counter_counts_kernels():
     n0 = mf.mfsdp_launch_count()
     sess.muon_step()
     assert mf.mfsdp_launch_count() > n0
+
+
+def test_tile_trace_covers_every_tile_once():
+    """mfsdp_debug_trace: one record per tile and iteration, phases in dependency order per matrix (a tile of phase
+    f + 1 never completes its accumulator before the first tile of phase f of the same launch did)."""
+    wl = workloads.get("medium")
+    sess = gh.Session(wl, precision=mf.NS_BF16)
+    sess.load_grads(0)
+    sess.muon_step()                                     # builds the launch tables
+    cap = 1 << 16
+    buf = torch.zeros(1 + 6 * cap, dtype=torch.int64, device="cuda")
+    mf.mfsdp_debug_trace(buf)
+    try:
+        mf.mfsdp_muon_ns_pass(sess.desc, sess.ws, sess.hp)
+        torch.cuda.synchronize()
+    finally:
+        mf.mfsdp_debug_trace(None)
+    n = int(buf[0].item())
+    assert 0 < n <= cap
+    rec = buf[1:1 + 6 * n].cpu().numpy().reshape(n, 6)
+    phase = rec[:, 0] >> 32
+    K = sess.hp.ns_steps
+    assert set(phase.tolist()) == set(range(3 * K))
+    counts = np.bincount(phase, minlength=3 * K).reshape(K, 3)
+    assert (counts == counts[0]).all(), "every iteration walks the same tile list"
+    assert (rec[:, 3] >= rec[:, 2]).all()
+    first_ready = np.array([rec[phase == f, 2].min() for f in range(3 * K)])
+    assert (np.diff(first_ready) > 0).all()
