@@ -94,6 +94,22 @@ def test_c3_ragged_512():
     assert 150 <= n_tall <= 280       # the transposed path is really exercised
 
 
+def test_vocab_embedding_shape():
+    """50,257 x 768 (GPT-2 vocabulary embedding on Muon): odd row count, GRAM k loop of 786 blocks, APPLY
+    with 197 row blocks; full oracle comparison plus the per-phase probes."""
+    wl = workloads.get("vocab")
+    sess = gh.Session(wl)
+    sess.load_grads(0)
+    W_old = [sess.seg64(sess.W, d) for d in sess.mats]
+    M_old = [np.zeros((d.rows, d.cols)) for d in sess.mats]
+    sess.muon_step()
+    rng = np.random.default_rng(3)
+    for i in range(len(sess.mats)):
+        eo, _ = gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i])
+        assert eo <= 3e-2
+        gh.probe_last_iteration(sess, i, rng, 2e-2)
+
+
 def _band_by_probes(O, rng, lo=0.55, hi=1.35):
     """O has singular values in the quintic's band ([0.68, 1.20] for sigma0 >= 0.002; tiny singular values
     of a heavy-tailed gradient may sit below).  ||O v|| <= sigma_max ||v|| for any v; and ||O||_F^2 / m is the mean

@@ -165,6 +165,46 @@ def test_both_tile_classes_bf16(pair_min_d, wname, min_d):
         gh.probe_last_iteration(sess, i, rng, 2e-2)
 
 
+@pytest.mark.parametrize("min_d", [1, 768])
+@pytest.mark.parametrize("precision", [mf.NS_BF16, mf.NS_FP32])
+def test_edge_shapes(pair_min_d, precision, min_d):
+    """1 x 1, single rows / columns, exact tile multiples and one past them, 16 x 4096 and 4096 x 16; bf16 mode with
+    everything forced onto CTA pairs and with the default split, and fp32 mode."""
+    if precision == mf.NS_FP32 and min_d == 1:
+        pytest.skip("the tile-class knob only affects the bf16 tensor-core path")
+    pair_min_d(min_d)
+    wl = workloads.edge_shapes(precision=precision)
+    sess, errs = _full_step_check(wl)
+    assert max(errs) <= gh.TOL_O[precision]
+    sess.load_grads(1)                                    # a second step on non-zero momentum
+    W_old, M_old = _snapshot(sess)
+    sess.muon_step()
+    for i in range(len(sess.mats)):
+        gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i])
+
+
+def test_empty_and_tail_only_tables_are_no_ops():
+    empty = mf.make_desc_array([])
+    hp = mf.MuonHParams(precision=mf.NS_BF16, **workloads.get("c1").muon)
+    ws = gh.aligned_bytes(max(1024, mf.mfsdp_workspace_bytes(empty, mf.NS_BF16)))
+    dummy = torch.zeros(64, device="cuda")
+    n0 = mf.mfsdp_launch_count()
+    mf.mfsdp_muon_step(empty, dummy, dummy, dummy, ws, hp)
+    mf.mfsdp_adamw_tail_step(empty, dummy, dummy, dummy, dummy, mf.AdamWHParams(step=1, **workloads.get("c1").adamw))
+    torch.cuda.synchronize()
+    assert mf.mfsdp_launch_count() == n0
+    # tails only: the Muon entry points launch nothing, AdamW moves the tail
+    wl = workloads.Workload("tails_only", [(0, 1, 300, 1, mf.BF16, 0), (1, 1, 5000, 1, mf.BF16, 0)], seed=3)
+    sess = gh.Session(wl)
+    sess.load_grads(0)
+    n0 = mf.mfsdp_launch_count()
+    sess.muon_step()
+    assert mf.mfsdp_launch_count() == n0
+    P0 = sess.P.clone()
+    sess.adamw_step(1)
+    assert not torch.equal(sess.P, P0)
+
+
 def test_medium_ragged_default_split_bf16():
     """Default threshold: the set is split between the two tile classes inside one step."""
     wl = workloads.get("medium")

@@ -112,8 +112,26 @@ def medium_ragged(seed=11, dtype=BF16, precision=NS_BF16):
     return Workload("medium_ragged", params, seed=seed, precision=precision, dtype=dtype)
 
 
+def edge_shapes(seed=13, dtype=BF16, precision=NS_BF16):
+    """Degenerate and boundary shapes: scalars, single rows / columns, exact tile multiples and one past them, very
+    thin matrices with a long k loop."""
+    shapes = [(1, 1), (1, 24), (24, 1), (7, 3), (128, 128), (129, 257), (255, 513), (256, 512), (16, 4096), (4096, 16)]
+    params = [(i // 4, 2, r, c, dtype, 0) for i, (r, c) in enumerate(shapes)]
+    params += [(0, 1, 1, 1, dtype, 0), (2, 1, 8, 1, dtype, 0)]
+    params.sort(key=lambda p: p[0])
+    return Workload("edge_shapes", params, seed=seed, precision=precision, dtype=dtype)
+
+
+def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
+    """The paper's convergence model puts the 50,257 x 768 embedding and the untied LM head on Muon:
+    a very tall matrix with an odd row count (GRAM k loop of 786 blocks) next to one ordinary matrix."""
+    params = [(0, 2, 50257, 768, dtype, 0), (1, 2, 768, 3072, dtype, 0), (1, 1, 768, 1, dtype, 0)]
+    return Workload("vocab_embedding", params, seed=seed, precision=precision, dtype=dtype)
+
+
 CONFIGS = {"c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
-           "small": small_ragged, "medium": medium_ragged}
+           "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes,
+           "vocab": vocab_embedding}
 
 
 def get(name):
