@@ -149,6 +149,7 @@ int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision,
  *   M              DEVICE i/o. rank-flat momentum, always float, same element offsets.
  *   workspace      DEVICE.     >= mfsdp_workspace_bytes, 1024-byte aligned; contents need not be preserved
  *                              between calls; after the call it holds O and ||U||^2 (mfsdp_workspace_view).
+ *                              May be NULL (and W, G, M too) when the table holds no matrix: the call is a no-op.
  *                              The library caches, per (table, workspace pointer, precision), a few KB..MB of
  *                              launch tables (TMA tensor maps, tile lists) in device memory of its own.
  *   hp             HOST in.
@@ -169,9 +170,11 @@ int mfsdp_muon_ns_pass(const mfsdp_desc_t* desc, size_t n_desc, void* workspace,
 int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, void* W, void* workspace, size_t ws_bytes,
                            const mfsdp_muon_hparams_t* hp, void* cuda_stream);
 
-/* The same step with HOST buffers (pinned or pageable): copies G (and W, M when `upload_state` != 0) to the
- * caller's device staging buffers dW/dG/dM, runs mfsdp_muon_step, copies W and M back, all on `cuda_stream`, and
- * synchronises the stream before returning.  Used for the end-to-end measurement. */
+/* The same step with HOST buffers (pinned for overlap; pageable works, serialised by the driver): copies G (and W, M
+ * when `upload_state` != 0) to the caller's device staging buffers dW/dG/dM (128-byte aligned), runs the step on
+ * `cuda_stream`, copies W and M back and synchronises the stream before returning.  Two internal copy streams carry
+ * the upload of W and the download of M underneath the Newton-Schulz pass; everything is ordered after the work
+ * already queued on `cuda_stream`.  Used for the end-to-end measurement. */
 int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, const void* hG, void* hM,
                          void* dW, void* dG, void* dM, int upload_state,
                          void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);

@@ -14,6 +14,7 @@ namespace mfsdp {
 // ---- bookkeeping ------------------------------------------------------------------------------------------------
 namespace {
 std::mutex g_mu;
+std::mutex g_host_mu;   // serialises mfsdp_muon_step_host (one set of copy streams)
 uint64_t g_launches = 0;
 std::string g_cuda_err = "no CUDA error recorded";
 std::vector<Plan*> g_plans;
@@ -212,7 +213,13 @@ int muon_front(const mfsdp_desc_t* desc, size_t n_desc, void* workspace, size_t 
   int rc = check_hp(hp);
   if (rc) return rc;
   if (n_desc && !desc) return MFSDP_EINVAL;
-  if (!workspace || !aligned(workspace, kBufAlign)) return MFSDP_EINVAL;
+  if (!workspace) {           // allowed only when the table holds no matrix (nothing to do: *pl stays null)
+    for (size_t i = 0; i < n_desc; ++i)
+      if (desc[i].role == MFSDP_ROLE_MATRIX) return MFSDP_EINVAL;
+    *pl = nullptr;
+    return MFSDP_OK;
+  }
+  if (!aligned(workspace, kBufAlign)) return MFSDP_EINVAL;
   rc = get_plan(desc, n_desc, hp->precision, workspace, true, pl);
   if (rc) return rc;
   if (ws_bytes < (*pl)->lay.total_bytes) return MFSDP_ECAP;
@@ -266,7 +273,7 @@ extern "C" int mfsdp_muon_momentum_pass(const mfsdp_desc_t* desc, size_t n_desc,
   Plan* pl = nullptr;
   const int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
-  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   if (!G || !M || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
   return launch_momentum(*pl, G, M, *hp, static_cast<cudaStream_t>(cuda_stream));
 }
@@ -276,7 +283,7 @@ extern "C" int mfsdp_muon_ns_pass(const mfsdp_desc_t* desc, size_t n_desc, void*
   Plan* pl = nullptr;
   const int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
-  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   return ns_dispatch(*pl, *hp, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -285,7 +292,7 @@ extern "C" int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, v
   Plan* pl = nullptr;
   const int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
-  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   if (!W || !aligned(W, 128)) return MFSDP_EINVAL;
   return launch_update(*pl, W, *hp, static_cast<cudaStream_t>(cuda_stream));
 }
@@ -295,7 +302,7 @@ extern "C" int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W,
   Plan* pl = nullptr;
   int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
-  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   if (!W || !G || !M || !aligned(W, 128) || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if ((rc = launch_momentum(*pl, G, M, *hp, st))) return rc;
@@ -303,28 +310,79 @@ extern "C" int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W,
   return launch_update(*pl, W, *hp, st);
 }
 
+namespace mfsdp {
+namespace {
+// Copy engines of mfsdp_muon_step_host: one stream per direction next to the caller's compute stream, so that the
+// uploads of W and the download of M run under the Newton-Schulz pass (PCIe is full duplex).
+struct HostPipe {
+  cudaStream_t in = nullptr, out = nullptr;
+  cudaEvent_t start = nullptr, gm_in = nullptr, w_in = nullptr, mom = nullptr, m_out = nullptr;
+  int device = -1;
+};
+HostPipe g_pipe;
+int host_pipe(HostPipe** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(e);
+  if (g_pipe.device != dev) {            // (re)create for the current device; the old objects are left to the driver
+    HostPipe p;
+    if ((e = cudaStreamCreateWithFlags(&p.in, cudaStreamNonBlocking)) != cudaSuccess ||
+        (e = cudaStreamCreateWithFlags(&p.out, cudaStreamNonBlocking)) != cudaSuccess)
+      return cuda_fail(e);
+    cudaEvent_t* evs[5] = {&p.start, &p.gm_in, &p.w_in, &p.mom, &p.m_out};
+    for (cudaEvent_t* ev : evs)
+      if ((e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
+    p.device = dev;
+    g_pipe = p;
+  }
+  *out = &g_pipe;
+  return MFSDP_OK;
+}
+}  // namespace
+}  // namespace mfsdp
+
 extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, const void* hG, void* hM,
                                     void* dW, void* dG, void* dM, int upload_state, void* workspace,
                                     size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
   Plan* pl = nullptr;
   int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
-  if (pl->lay.mats.empty()) return MFSDP_OK;
+  if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   if (!hW || !hG || !hM || !dW || !dG || !dM) return MFSDP_EINVAL;
+  if (!aligned(dW, 128) || !aligned(dG, 128) || !aligned(dM, 128)) return MFSDP_EINVAL;
   uint64_t elems = 0;
   if ((rc = mfsdp_flat_elems(desc, n_desc, &elems, nullptr))) return rc;
   const size_t es = pl->lay.mat_dtype == MFSDP_BF16 ? 2 : 4;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  cudaError_t e = cudaMemcpyAsync(dG, hG, elems * es, cudaMemcpyHostToDevice, st);
-  if (e != cudaSuccess) return cuda_fail(e);
-  if (upload_state) {
-    if ((e = cudaMemcpyAsync(dW, hW, elems * es, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
-    if ((e = cudaMemcpyAsync(dM, hM, elems * 4, cudaMemcpyHostToDevice, st)) != cudaSuccess) return cuda_fail(e);
-  }
-  if ((rc = mfsdp_muon_step(desc, n_desc, dW, dG, dM, workspace, ws_bytes, hp, cuda_stream))) return rc;
-  if ((e = cudaMemcpyAsync(hW, dW, elems * es, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
-  if ((e = cudaMemcpyAsync(hM, dM, elems * 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess) return cuda_fail(e);
-  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e);
+  std::lock_guard<std::mutex> lock(g_host_mu);
+  HostPipe* hpipe = nullptr;
+  if ((rc = host_pipe(&hpipe))) return rc;
+  HostPipe& q = *hpipe;
+  cudaError_t e;
+#define MFSDP_TRY(call) do { if ((e = (call)) != cudaSuccess) return cuda_fail(e); } while (0)
+  // in:  G, M (needed by the momentum pass), then W (needed only by the update pass: rides under Newton-Schulz)
+  MFSDP_TRY(cudaEventRecord(q.start, st));
+  MFSDP_TRY(cudaStreamWaitEvent(q.in, q.start, 0));
+  MFSDP_TRY(cudaMemcpyAsync(dG, hG, elems * es, cudaMemcpyHostToDevice, q.in));
+  if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dM, hM, elems * 4, cudaMemcpyHostToDevice, q.in));
+  MFSDP_TRY(cudaEventRecord(q.gm_in, q.in));
+  if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dW, hW, elems * es, cudaMemcpyHostToDevice, q.in));
+  MFSDP_TRY(cudaEventRecord(q.w_in, q.in));
+  // compute on the caller's stream
+  MFSDP_TRY(cudaStreamWaitEvent(st, q.gm_in, 0));
+  if ((rc = launch_momentum(*pl, dG, dM, *hp, st))) return rc;
+  MFSDP_TRY(cudaEventRecord(q.mom, st));
+  // out: M is final after the momentum pass: its download rides under Newton-Schulz too
+  MFSDP_TRY(cudaStreamWaitEvent(q.out, q.mom, 0));
+  MFSDP_TRY(cudaMemcpyAsync(hM, dM, elems * 4, cudaMemcpyDeviceToHost, q.out));
+  MFSDP_TRY(cudaEventRecord(q.m_out, q.out));
+  if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
+  MFSDP_TRY(cudaStreamWaitEvent(st, q.w_in, 0));
+  if ((rc = launch_update(*pl, dW, *hp, st))) return rc;
+  MFSDP_TRY(cudaMemcpyAsync(hW, dW, elems * es, cudaMemcpyDeviceToHost, st));
+  MFSDP_TRY(cudaStreamWaitEvent(st, q.m_out, 0));
+  MFSDP_TRY(cudaStreamSynchronize(st));
+#undef MFSDP_TRY
   return MFSDP_OK;
 }
 
