@@ -234,8 +234,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   const uint32_t tmem_base = *tmem_holder;
 
   if (warp == 0) {
-    // ===== TMA producer (both CTAs of a pair; the bytes of both are counted on the leader's full barrier) =====
-    if (lane == 0) {
+    // ===== TMA producer (both CTAs of a pair; the bytes of both are counted on the leader's full barrier).  Like the
+    // UMMA warp it runs converged with one elected lane issuing (uniform-register operands without election loops:
+    // the single-lane version spent ~700 cycles per k block issuing 4-6 loads); claiming a tile and waiting for its
+    // dependencies is lane 0's business. =====
+    {
       uint32_t stage = 0, phase = 0;
       const uint32_t full_lead0 = kCG == 2 ? ptx::mapa(full0, 0) : full0;
       // Short tiles: the leader claims one tile ahead, so that the atomic's round trip overlaps with issuing the current
@@ -245,8 +248,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       constexpr uint32_t kUnclaimed = 0xfffffffeu, kAheadMaxKb = 32;
       uint32_t next_ti = kUnclaimed;
       for (;;) {
-        uint32_t ti;
+        uint32_t ti = 0;
         if (rank == 0) {
+          if (lane == 0) {
           ti = next_ti == kUnclaimed ? feed.claim(p.counter, p.n_iter_tiles * p.ns_steps) : next_ti;
           next_ti = kUnclaimed;
           bool ahead = false;
@@ -268,8 +272,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
           }
           feed.publish(ti);
           if (ahead) next_ti = feed.claim(p.counter, p.n_iter_tiles * p.ns_steps);
+          }
+          ti = __shfl_sync(0xffffffffu, ti, 0);
         } else {
-          ti = feed.next_single();
+          ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
+          __syncwarp();
+          feed.release(lane == 0);
         }
         if (ti == kNoTile) break;
         ptx::fence_proxy_async();          // reported (generic-proxy) completion -> this thread's TMA reads
@@ -301,6 +309,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
         const uint32_t tx = (a_boxes + n_b) * kBoxBytes * kCG;
         for (uint32_t kb = 0; kb < t.nkb; ++kb) {
           ptx::mbar_wait(empty0 + 8 * stage, phase ^ 1);
+          if (ptx::elect_one()) {
           if (rank == 0) ptx::mbar_arrive_expect_tx(full0 + 8 * stage, tx);
           const uint32_t fb = full_lead0 + 8 * stage;
           const uint32_t sa = stage0 + stage * kStageBytes, sb = sa + kABytes;
@@ -319,6 +328,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
               else ptx::tma_load_2d(dst, c.tb, c.b_mn ? mn : k0, c.b_mn ? k0 : mn, fb);
             }
           }
+          }
+          __syncwarp();
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
       }
