@@ -313,3 +313,34 @@ def test_tile_trace_covers_every_tile_once():
     assert (rec[:, 3] >= rec[:, 2]).all()
     first_ready = np.array([rec[phase == f, 2].min() for f in range(3 * K)])
     assert (np.diff(first_ready) > 0).all()
+
+
+@pytest.mark.parametrize("wname", ["small", "medium", "edge"])
+def test_no_write_outside_the_buffers(wname):
+    """Guard bands around W, M and the workspace stay intact (the TMA stores are clipped by the tensor maps, the
+    elementwise passes by the segment tables), and the gradient is never written."""
+    wl = workloads.get(wname)
+    sess = gh.Session(wl, precision=mf.NS_BF16)
+    sess.load_grads(0)
+    guard = 1 << 16
+
+    def banded(t, pattern):
+        raw = torch.full((t.numel() * t.element_size() + 2 * guard + 1024,), pattern, dtype=torch.uint8, device="cuda")
+        off = guard + ((-(raw.data_ptr() + guard)) % 1024)
+        view = raw[off:off + t.numel() * t.element_size()].view(t.dtype)
+        view.copy_(t.reshape(-1))
+        return raw, off, view
+
+    rawW, offW, W = banded(sess.W, 0xA5)
+    rawM, offM, M = banded(sess.M, 0x5A)
+    raws, offs, ws = banded(sess.ws, 0xC3)
+    G0 = sess.G.clone()
+    mf.mfsdp_muon_step(sess.desc, W, sess.G, M, ws, sess.hp)
+    torch.cuda.synchronize()
+    for raw, off, view, pat in ((rawW, offW, W, 0xA5), (rawM, offM, M, 0x5A), (raws, offs, ws, 0xC3)):
+        n = view.numel() * view.element_size()
+        assert bool((raw[:off] == pat).all()) and bool((raw[off + n:] == pat).all())
+    assert torch.equal(sess.G, G0)
+    # and the result equals the one computed in the ordinary buffers
+    sess.muon_step()
+    assert torch.equal(W, sess.W) and torch.equal(M, sess.M)
