@@ -127,8 +127,9 @@ __device__ __forceinline__ uint4 ld_global_cg_v4(const void* p) {
   asm volatile("ld.global.cg.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
   return v;
 }
-// orders this thread's earlier generic-proxy accesses (and what it acquired) before its later async-proxy (TMA) accesses
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// orders this thread's earlier generic-proxy accesses (and what it acquired) before its later async-proxy (TMA)
+// accesses, and vice versa, for GLOBAL memory (the only space the inter-CTA dependencies go through)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
 // ---- thread-block clusters (CTA pairs) ------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t cluster_ctarank() {
