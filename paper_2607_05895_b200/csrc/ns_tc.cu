@@ -51,7 +51,7 @@ struct TcMat {                 // device, one per matrix
 // paired; <= 256 single CTA, <= 512 paired).
 // `need`: completion reports of the SAME matrix and iteration that must have been made before this tile's operands
 // may be read (= every tile of the matrix' earlier phases); `phase`: PH_*.
-struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; uint32_t need, phase; };
+struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; uint32_t need, phase, reports_per_iter, pad; };
 
 struct NsTcPlan {
   CUtensorMap* d_tmaps = nullptr;   // TM_COUNT per matrix
@@ -77,7 +77,7 @@ constexpr uint32_t kStages = 4;
 #ifndef MFSDP_NS_GROUP
 #define MFSDP_NS_GROUP 2
 #endif
-constexpr uint32_t kThreads = 192;
+constexpr uint32_t kThreads = 224;   // producer, UMMA issuer, 4 epilogue warps, tile scheduler
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kEpiBufBytes = 4096;        // one staging tile: 32 rows x 64 cols (or 64 x 32 transposed) bf16
 constexpr uint32_t kEpiBytes = 4 * 2 * kEpiBufBytes;   // 4 epilogue warps x 2 buffers
@@ -213,6 +213,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   feed.full0 = ptx::smem_u32(bars + 2 * kStages + 5);
   feed.empty0 = ptx::smem_u32(bars + 2 * kStages + 5 + kFeed);
   feed.slots0 = ptx::smem_u32(bars + 2 * kStages + 5 + 2 * kFeed);
+  const uint32_t prod_done = ptx::smem_u32(bars + 2 * kStages + 7 + 2 * kFeed);   // tiles whose loads the producer has issued
   const uint32_t stage0 = ptx::smem_u32(smem);
   const uint32_t epi0 = stage0 + kStages * kStageBytes;
   const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -223,8 +224,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   if (threadIdx.x == 0) {
     for (uint32_t s = 0; s < kStages; ++s) { ptx::mbar_init(full0 + 8 * s, 1); ptx::mbar_init(empty0 + 8 * s, 1); }
     for (uint32_t s = 0; s < 2; ++s) { ptx::mbar_init(tfull0 + 8 * s, 1); ptx::mbar_init(tempty0 + 8 * s, 4 * kCG); }
-    // feed consumers per slot: UMMA issuer + 4 epilogue warps of the leader, producer + 4 epilogue warps of the peer
-    for (uint32_t s = 0; s < kFeed; ++s) { ptx::mbar_init(feed.full0 + 8 * s, 1); ptx::mbar_init(feed.empty0 + 8 * s, 5 * kCG); }
+    // feed consumers per slot: producer + UMMA issuer + 4 epilogue warps of the leader, producer + 4 epilogue warps of
+    // the peer
+    for (uint32_t s = 0; s < kFeed; ++s) { ptx::mbar_init(feed.full0 + 8 * s, 1); ptx::mbar_init(feed.empty0 + 8 * s, kCG == 2 ? 11 : 6); }
+    ptx::st_shared_volatile_u32(prod_done, 0u);
     ptx::fence_barrier_init();
   }
   if (warp == 1) ptx::tmem_alloc<kTmemCols, kCG>(ptx::smem_u32(tmem_holder));
@@ -236,49 +239,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   if (warp == 0) {
     // ===== TMA producer (both CTAs of a pair; the bytes of both are counted on the leader's full barrier).  Like the
     // UMMA warp it runs converged with one elected lane issuing (uniform-register operands without election loops:
-    // the single-lane version spent ~700 cycles per k block issuing 4-6 loads); claiming a tile and waiting for its
-    // dependencies is lane 0's business. =====
+    // the single-lane version spent ~700 cycles per k block issuing 4-6 loads).  Tiles come from the scheduler warp. =====
     {
-      uint32_t stage = 0, phase = 0;
+      uint32_t stage = 0, phase = 0, n_done = 0;
       const uint32_t full_lead0 = kCG == 2 ? ptx::mapa(full0, 0) : full0;
-      // Short tiles: the leader claims one tile ahead, so that the atomic's round trip overlaps with issuing the current
-      // tile's loads.  Long tiles are claimed when needed: claiming ahead widens the window of tiles in flight and
-      // measured 19 % more DRAM traffic on the Llama-70B set (the L2 reuse between neighbouring tiles relies on
-      // list neighbours starting close in time).
-      constexpr uint32_t kUnclaimed = 0xfffffffeu, kAheadMaxKb = 32;
-      uint32_t next_ti = kUnclaimed;
       for (;;) {
-        uint32_t ti = 0;
-        if (rank == 0) {
-          if (lane == 0) {
-          ti = next_ti == kUnclaimed ? feed.claim(p.counter, p.n_iter_tiles * p.ns_steps) : next_ti;
-          next_ti = kUnclaimed;
-          bool ahead = false;
-          if (ti != kNoTile) {
-            // inputs of the tile = outputs of every tile of the same matrix in the preceding phases: wait until all
-            // of them have been reported complete (tiles are claimed in phase order, so those tiles are running or
-            // done, never waiting on a later one)
-            const Work w0 = fetch(p, ti);
-            const uint32_t need = w0.it * p.mats[w0.t.mat].reports_per_iter + w0.t.need;
-            const uint32_t* flag = p.done + w0.t.mat;
-            ahead = w0.t.nkb < kAheadMaxKb;
-            if (ptx::ld_acquire_gpu(flag) < need) {
-              const long long t0 = clock64();
-              while (ptx::ld_acquire_gpu(flag) < need) {
-                __nanosleep(64);
-                if (clock64() - t0 > 4000000000ll) __trap();
-              }
-            }
-          }
-          feed.publish(ti);
-          if (ahead) next_ti = feed.claim(p.counter, p.n_iter_tiles * p.ns_steps);
-          }
-          ti = __shfl_sync(0xffffffffu, ti, 0);
-        } else {
-          ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
-          __syncwarp();
-          feed.release(lane == 0);
-        }
+        const uint32_t ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
+        __syncwarp();
+        feed.release(lane == 0);
         if (ti == kNoTile) break;
         ptx::fence_proxy_async();          // reported (generic-proxy) completion -> this thread's TMA reads
         const Work w = fetch(p, ti);
@@ -331,6 +299,49 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
           }
           __syncwarp();
           if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+        ++n_done;                                               // tells the scheduler that this tile's loads are issued
+        if (rank == 0 && lane == 0) ptx::st_shared_volatile_u32(prod_done, n_done);
+      }
+    }
+  } else if (warp == 6) {
+    // ===== tile scheduler (leader CTA, one lane): claims tiles, waits for their dependencies, publishes them.  It runs
+    // ahead of the producer, which takes the atomic, the descriptor fetch and the dependency check (~2 K cycles, three
+    // dependent trips to L2) off the load-issue path: by up to the feed depth on tiny tiles (< 8 k blocks), by one tile
+    // on medium ones (queueing more costs load balance at the end of a phase), not at all on long ones (>= 32 k
+    // blocks: it waits until the producer has issued the tile's last load -- claiming long tiles early widens the
+    // window of tiles in flight and measured 19 % more DRAM traffic on the Llama-70B set, because the L2 reuse between
+    // list neighbours relies on their starting close in time). =====
+    if (rank == 0 && lane == 0) {
+      constexpr uint32_t kLongKb = 32, kTinyKb = 8;
+      const uint32_t total = p.n_iter_tiles * p.ns_steps;
+      for (uint32_t n_pub = 0;; ++n_pub) {
+        const uint32_t ti = feed.claim(p.counter, total);
+        uint32_t wait_for = 0;                                   // producer progress required before the next claim
+        if (ti != kNoTile) {
+          // inputs of the tile = outputs of every tile of the same matrix in the preceding phases: wait until all of
+          // them have been reported complete (tiles are claimed in phase order and every unit works through its
+          // claims in order, so those tiles are running or done, never waiting on a later one)
+          const Work w0 = fetch(p, ti);
+          const uint32_t need = w0.it * w0.t.reports_per_iter + w0.t.need;
+          const uint32_t* flag = p.done + w0.t.mat;
+          wait_for = w0.t.nkb >= kLongKb ? n_pub + 1 : (w0.t.nkb >= kTinyKb ? n_pub : 0u);
+          if (ptx::ld_acquire_gpu(flag) < need) {
+            const long long t0 = clock64();
+            while (ptx::ld_acquire_gpu(flag) < need) {
+              __nanosleep(64);
+              if (clock64() - t0 > 4000000000ll) __trap();
+            }
+          }
+        }
+        feed.publish(ti);
+        if (ti == kNoTile) break;
+        if (ptx::ld_shared_volatile_u32(prod_done) < wait_for) {
+          const long long t0 = clock64();
+          while (ptx::ld_shared_volatile_u32(prod_done) < wait_for) {
+            __nanosleep(256);
+            if (clock64() - t0 > 4000000000ll) __trap();
+          }
         }
       }
     }
@@ -645,7 +656,7 @@ void tiles_rect(std::vector<TcTile>& v, uint32_t mat, uint32_t out_rows, uint32_
   for (uint32_t g0 = 0; g0 < tn; g0 += group)
     for (uint32_t i = 0; i < tm; ++i)
       for (uint32_t j = g0; j < std::min(tn, g0 + group); ++j)
-        v.push_back(TcTile{mat, i * bm, j * bn, (uint16_t)nkb, tile_w(out_cols - j * bn, cg, bn), 0u, phase});
+        v.push_back(TcTile{mat, i * bm, j * bn, (uint16_t)nkb, tile_w(out_cols - j * bn, cg, bn), 0u, phase, 0u, 0u});
 }
 // symmetric output (GRAM, POLY): upper row blocks only; bands of `band` row blocks, inside a band column-major
 // (all row blocks of the band for one column step of a tile width, then the next step).
@@ -662,7 +673,7 @@ void tiles_sym(std::vector<TcTile>& v, uint32_t mat, uint32_t d, uint32_t nkb, u
         const uint32_t lo = std::max(c0, i * bm);
         const uint32_t hi = std::min(d, c0 + bn);
         if (lo >= hi) continue;
-        v.push_back(TcTile{mat, i * bm, lo, (uint16_t)nkb, tile_w(hi - lo, cg, bn), 0u, phase});
+        v.push_back(TcTile{mat, i * bm, lo, (uint16_t)nkb, tile_w(hi - lo, cg, bn), 0u, phase, 0u, 0u});
       }
   }
 }
@@ -752,7 +763,10 @@ int build_tc_plan(Plan& pl) {
     std::vector<uint32_t> cnt[3];
     for (int ph = 0; ph < 3; ++ph) cnt[ph].assign(lay.mats.size(), 0u);
     for (const TcTile& t : tiles[g]) cnt[t.phase][t.mat] += per_tile;
-    for (TcTile& t : tiles[g]) t.need = (t.phase >= 1 ? cnt[0][t.mat] : 0u) + (t.phase >= 2 ? cnt[1][t.mat] : 0u);
+    for (TcTile& t : tiles[g]) {
+      t.need = (t.phase >= 1 ? cnt[0][t.mat] : 0u) + (t.phase >= 2 ? cnt[1][t.mat] : 0u);
+      t.reports_per_iter = cnt[0][t.mat] + cnt[1][t.mat] + cnt[2][t.mat];
+    }
     for (size_t i = 0; i < lay.mats.size(); ++i)
       if (cls[i] == (uint32_t)g + 1) mats[i].reports_per_iter = cnt[0][i] + cnt[1][i] + cnt[2][i];
   }
