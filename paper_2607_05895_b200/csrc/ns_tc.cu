@@ -20,10 +20,15 @@
 //            start as soon as that half has been drained.
 //   kCG = 1  small / ragged matrices: one CTA owns a 128 x (64..256) tile, two accumulator stages alternate
 //            between tiles (the epilogue of tile t overlaps the main loop of tile t + 1).
-// Kernel anatomy (192 threads per CTA): warp 0 = TMA producer (one lane), warp 1 = TMEM owner + UMMA issuer (one
-// lane, leader CTA only when paired), warps 2-5 = epilogue: TMEM -> registers -> fused scale / polynomial -> bf16
-// -> swizzled shared-memory staging -> TMA tensor stores (direct tile and, for the symmetric phases, the transposed
-// mirror tile); the b A term of POLY is TMA-loaded into the same staging buffer.  4-stage operand ring.
+// Kernel anatomy (224 threads per CTA): warp 0 = TMA producer, warp 1 = TMEM owner + UMMA issuer (leader CTA only when
+// paired) -- both run their loops converged with one elected lane issuing --, warps 2-5 = epilogue: TMEM -> registers
+// -> fused scale / polynomial -> bf16 -> swizzled shared-memory staging -> TMA tensor stores (direct tile and, for the
+// symmetric phases, the transposed mirror tile), warp 6 = tile scheduler (leader CTA, one lane).  4-stage operand ring.
+//
+// One launch per tile class walks the tiles of ALL iterations and phases: the scheduler claims tiles from a global
+// counter in list order, waits until the tile's inputs (every tile of the same matrix in the preceding phases) have
+// been reported complete through a per-matrix counter, and publishes the index to the other roles through a
+// shared-memory ring.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
