@@ -545,10 +545,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
                 pk[4 * j + i] = pack_bf16(f0, f1);
               }
             }
-          } else {
+          } else if (w.first) {                                  // iteration 0: the folded Frobenius normalisation
 #pragma unroll
             for (int j = 0; j < 32; ++j)
               pk[j] = pack_bf16(alpha * __uint_as_float(v[2 * j]), alpha * __uint_as_float(v[2 * j + 1]));
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) pk[j] = pack_bf16(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
           }
           // direct tile: row `lane` of the staging tile, swizzled; then one TMA store (clipped at the matrix edges)
 #pragma unroll
