@@ -9,7 +9,8 @@ namespace mfsdp {
 namespace {
 
 constexpr int kT = 64;    // output tile
-constexpr int kK = 16;    // k slab
+constexpr int kK = 32;    // k slab
+constexpr int kPer = kT * kK / 256;   // slab elements per thread and operand
 
 enum { PH_GRAM = 0, PH_POLY = 1, PH_APPLY = 2 };
 
@@ -44,17 +45,38 @@ __global__ void __launch_bounds__(256) k_ns_fp32(NsArgs g) {
   __shared__ float sA[kK][kT + 1];
   __shared__ float sB[kK][kT + 1];
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  float acc[4][4] = {};
-  for (uint32_t k0 = 0; k0 < Kd; k0 += kK) {
-    for (int t = threadIdx.x; t < kT * kK; t += 256) {
-      const int kk = t & (kK - 1), ii = t >> 4;           // A slab: 64 (i) x 16 (k)
-      const uint32_t i = i0 + ii, k = k0 + kk;
-      sA[kk][ii] = (i < Mo && k < Kd) ? Ap[i * sa_i + k * sa_k] : 0.f;
-      const int jj = t & (kT - 1), kb = t >> 6;           // B slab: 16 (k) x 64 (j)
-      const uint32_t j = j0 + jj, k2 = k0 + kb;
-      sB[kb][jj] = (j < No && k2 < Kd) ? Bp[k2 * sb_k + j * sb_j] : 0.f;
+  // Slab element e = threadIdx.x + 256 r of an operand -> (mn, k): the index that is contiguous in memory runs fastest
+  // across the threads (coalesced loads for both the plain and the transposed views).
+  const bool a_kfast = sa_k == 1, b_kfast = sb_k == 1;
+  float ra[kPer], rb[kPer];
+  auto fetch = [&](uint32_t k0) {
+#pragma unroll
+    for (int r = 0; r < kPer; ++r) {
+      const int e = threadIdx.x + 256 * r;
+      const int am = a_kfast ? e / kK : e % kT, ak = a_kfast ? e % kK : e / kT;
+      const uint32_t i = i0 + am, k = k0 + ak;
+      ra[r] = (i < Mo && k < Kd) ? Ap[i * sa_i + k * sa_k] : 0.f;
+      const int bm = b_kfast ? e / kK : e % kT, bk = b_kfast ? e % kK : e / kT;
+      const uint32_t j = j0 + bm, k2 = k0 + bk;
+      rb[r] = (j < No && k2 < Kd) ? Bp[k2 * sb_k + j * sb_j] : 0.f;
     }
+  };
+  auto stash = [&]() {
+#pragma unroll
+    for (int r = 0; r < kPer; ++r) {
+      const int e = threadIdx.x + 256 * r;
+      const int am = a_kfast ? e / kK : e % kT, ak = a_kfast ? e % kK : e / kT;
+      sA[ak][am] = ra[r];
+      const int bm = b_kfast ? e / kK : e % kT, bk = b_kfast ? e % kK : e / kT;
+      sB[bk][bm] = rb[r];
+    }
+  };
+  float acc[4][4] = {};
+  fetch(0);
+  for (uint32_t k0 = 0; k0 < Kd; k0 += kK) {
+    stash();
     __syncthreads();
+    if (k0 + kK < Kd) fetch(k0 + kK);        // next slab in flight (registers) while this one is multiplied
 #pragma unroll
     for (int kk = 0; kk < kK; ++kk) {
       float av[4], bv[4];
