@@ -150,6 +150,10 @@ int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision,
  *   workspace      DEVICE.     >= mfsdp_workspace_bytes, 1024-byte aligned; contents need not be preserved
  *                              between calls; after the call it holds O and ||U||^2 (mfsdp_workspace_view).
  *                              May be NULL (and W, G, M too) when the table holds no matrix: the call is a no-op.
+ *   cuda_stream    cudaStream_t (NULL = the legacy default stream).  Work is enqueued, not awaited.  After one
+ *                              ordinary call with the same (table, workspace, precision) -- which builds the cached
+ *                              launch tables with cudaMalloc / cudaMemcpy -- the step is CUDA-graph capturable (one
+ *                              memset node and the kernel launches).
  *                              The library caches, per (table, workspace pointer, precision), a few KB..MB of
  *                              launch tables (TMA tensor maps, tile lists) in device memory of its own.
  *   hp             HOST in.

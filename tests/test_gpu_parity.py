@@ -344,3 +344,32 @@ def test_no_write_outside_the_buffers(wname):
     # and the result equals the one computed in the ordinary buffers
     sess.muon_step()
     assert torch.equal(W, sess.W) and torch.equal(M, sess.M)
+
+
+def test_step_is_cuda_graph_capturable():
+    """After one eager call (which builds the cached launch tables) the whole step -- one memset and five kernel
+    launches -- can be captured into a CUDA graph and replayed: same bits as the eager step."""
+    wl = workloads.get("medium")
+    a = gh.Session(wl, precision=mf.NS_BF16)
+    a.load_grads(0)
+    a.muon_step()
+    a.adamw_step(1)                                       # eager reference: state after step 1
+    b = gh.Session(wl, precision=mf.NS_BF16)
+    b.load_grads(0)
+    W0, M0, P0 = b.W.clone(), b.M.clone(), b.P.clone()
+    b.muon_step()                                         # warm-up: builds the tables for b's workspace
+    b.adamw_step(1)
+    b.W.copy_(W0); b.M.copy_(M0); b.P.copy_(P0); b.m.zero_(); b.v.zero_()
+    ahp = mf.AdamWHParams(step=1, **wl.adamw)
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            mf.mfsdp_muon_step(b.desc, b.W, b.G, b.M, b.ws, b.hp)
+            mf.mfsdp_adamw_tail_step(b.desc, b.P, b.Gt, b.m, b.v, ahp)
+    torch.cuda.current_stream().wait_stream(side)
+    b.W.copy_(W0); b.M.copy_(M0); b.P.copy_(P0); b.m.zero_(); b.v.zero_()   # capture does not execute
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M) and torch.equal(a.P, b.P)
