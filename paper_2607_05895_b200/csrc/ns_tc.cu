@@ -86,7 +86,7 @@ constexpr uint32_t kThreads = 224;   // producer, UMMA issuer, 4 epilogue warps,
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kEpiBufBytes = 4096;        // one staging tile: 32 rows x 64 cols (or 64 x 32 transposed) bf16
 constexpr uint32_t kEpiBytes = 4 * 2 * kEpiBufBytes;   // 4 epilogue warps x 2 buffers
-constexpr uint32_t kBarBytes = 256;
+constexpr uint32_t kBarBytes = 512;            // mbarriers, TMEM address, scheduler feed slots
 constexpr uint32_t kSmemBytes = kStages * kStageBytes + kEpiBytes + kBarBytes + 1024 /*align slack*/;
 
 struct TcParams {
@@ -169,12 +169,23 @@ struct Feed {
     const uint32_t ti = atomicAdd(counter, 1u);
     return ti < n_tiles ? ti : kNoTile;
   }
-  // ... and publish (after the tile's inputs are known to be complete).
-  __device__ __forceinline__ void publish(uint32_t ti) {
+  // ... and publish it with its descriptors (after the tile's inputs are known to be complete).  A slot is 16 words:
+  // the TcTile (word 7 = the claimed index or kNoTile), the iteration, and the matrix fields the roles need -- so that
+  // no consumer has to chase tile / matrix tables through global memory at the start of every tile.
+  __device__ __forceinline__ void publish(uint32_t ti, const Work& w, const TcMat& M) {
     ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);                // every consumer has read the slot's previous content
-    ptx::st_shared_u32(slots0 + 4 * s, ti);
+    uint32_t v[16];
+    v[0] = w.t.mat; v[1] = w.t.m0; v[2] = w.t.n0; v[3] = (uint32_t)w.t.nkb | ((uint32_t)w.t.nw << 16);
+    v[4] = w.t.need; v[5] = w.t.phase; v[6] = w.t.reports_per_iter; v[7] = ti;
+    v[8] = w.it; v[9] = M.rows; v[10] = M.cols; v[11] = M.d; v[12] = M.tall; v[13] = M.pitch_a;
+    v[14] = (uint32_t)M.a_off; v[15] = (uint32_t)(M.a_off >> 32);
+    const uint32_t slot = slots0 + 64 * s;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) ptx::st_shared_v4(slot + 16 * i, v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
     if constexpr (kCG == 2) {
-      ptx::st_shared_cluster_u32(ptx::mapa(slots0 + 4 * s, 1), ti);
+      const uint32_t rslot = ptx::mapa(slot, 1);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) ptx::st_shared_cluster_u32(rslot + 4 * i, v[i]);
       ptx::mbar_arrive_cluster(ptx::mapa(full0 + 8 * s, 1));
     }
     ptx::mbar_arrive(full0 + 8 * s);
@@ -188,7 +199,21 @@ struct Feed {
   // any other role: wait for the next index ...
   __device__ __forceinline__ uint32_t peek() const {
     if constexpr (kCG == 2) ptx::mbar_wait_cluster(full0 + 8 * s, ph); else ptx::mbar_wait(full0 + 8 * s, ph);
-    return ptx::ld_shared_u32(slots0 + 4 * s);
+    return ptx::ld_shared_u32(slots0 + 64 * s + 28);
+  }
+  // ... read its descriptors (before release) ...
+  __device__ __forceinline__ void read(Work& w, TcMat& M) const {
+    uint32_t a[4], b[4], c[4], d[4];
+    const uint32_t slot = slots0 + 64 * s;
+    ptx::ld_shared_v4(slot, a[0], a[1], a[2], a[3]);
+    ptx::ld_shared_v4(slot + 16, b[0], b[1], b[2], b[3]);
+    ptx::ld_shared_v4(slot + 32, c[0], c[1], c[2], c[3]);
+    ptx::ld_shared_v4(slot + 48, d[0], d[1], d[2], d[3]);
+    w.t.mat = a[0]; w.t.m0 = a[1]; w.t.n0 = a[2]; w.t.nkb = (uint16_t)(a[3] & 0xffffu); w.t.nw = (uint16_t)(a[3] >> 16);
+    w.t.need = b[0]; w.t.phase = b[1]; w.t.reports_per_iter = b[2]; w.t.pad = 0;
+    w.it = c[0]; w.src = c[0] & 1u; w.first = c[0] == 0u;
+    M.rows = c[1]; M.cols = c[2]; M.d = c[3]; M.tall = d[0]; M.pitch_a = d[1];
+    M.a_off = (uint64_t)d[2] | ((uint64_t)d[3] << 32);
   }
   // ... and report the slot as consumed (`arrive`: one thread per role, after every thread of the role has read it).
   __device__ __forceinline__ void release(bool arrive) {
@@ -196,11 +221,6 @@ struct Feed {
       if constexpr (kCG == 2) ptx::mbar_arrive_cluster(empty_lead0 + 8 * s); else ptx::mbar_arrive(empty_lead0 + 8 * s);
     }
     advance();
-  }
-  __device__ __forceinline__ uint32_t next_single() {      // single-thread roles
-    const uint32_t ti = peek();
-    release(true);
-    return ti;
   }
 };
 
@@ -217,8 +237,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
   Feed<kCG> feed;
   feed.full0 = ptx::smem_u32(bars + 2 * kStages + 5);
   feed.empty0 = ptx::smem_u32(bars + 2 * kStages + 5 + kFeed);
-  feed.slots0 = ptx::smem_u32(bars + 2 * kStages + 5 + 2 * kFeed);
-  const uint32_t prod_done = ptx::smem_u32(bars + 2 * kStages + 7 + 2 * kFeed);   // tiles whose loads the producer has issued
+  feed.slots0 = ptx::smem_u32(bars) + 256;          // kFeed slots of 64 bytes in the second half of the region
+  const uint32_t prod_done = ptx::smem_u32(bars + 2 * kStages + 5 + 2 * kFeed);   // tiles whose loads the producer has issued
   const uint32_t stage0 = ptx::smem_u32(smem);
   const uint32_t epi0 = stage0 + kStages * kStageBytes;
   const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -250,13 +270,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       const uint32_t full_lead0 = kCG == 2 ? ptx::mapa(full0, 0) : full0;
       for (;;) {
         const uint32_t ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
+        Work w;
+        TcMat M;
+        feed.read(w, M);
         __syncwarp();
         feed.release(lane == 0);
         if (ti == kNoTile) break;
         ptx::fence_proxy_async();          // reported (generic-proxy) completion -> this thread's TMA reads
-        const Work w = fetch(p, ti);
         const TcTile t = w.t;
-        const TcMat M = p.mats[t.mat];
         const TileCfg c = decode(p, t, M, w.src);
         const uint32_t am0 = t.m0 + rank * kBM;
         // B boxes of this CTA: single CTA: nw / 64 consecutive boxes.  Paired: per 256-column half h its own half of
@@ -323,11 +344,16 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       for (uint32_t n_pub = 0;; ++n_pub) {
         const uint32_t ti = feed.claim(p.counter, total);
         uint32_t wait_for = 0;                                   // producer progress required before the next claim
+        Work w0;
+        TcMat M0;
+        w0.it = 0; w0.t = TcTile{0u, 0u, 0u, 0, 0, 0u, 0u, 0u, 0u};
+        M0.rows = M0.cols = M0.d = M0.tall = M0.pitch_a = 0; M0.a_off = 0;
         if (ti != kNoTile) {
           // inputs of the tile = outputs of every tile of the same matrix in the preceding phases: wait until all of
           // them have been reported complete (tiles are claimed in phase order and every unit works through its
           // claims in order, so those tiles are running or done, never waiting on a later one)
-          const Work w0 = fetch(p, ti);
+          w0 = fetch(p, ti);
+          M0 = p.mats[w0.t.mat];
           const uint32_t need = w0.it * w0.t.reports_per_iter + w0.t.need;
           const uint32_t* flag = p.done + w0.t.mat;
           wait_for = w0.t.nkb >= kLongKb ? n_pub + 1 : (w0.t.nkb >= kTinyKb ? n_pub : 0u);
@@ -339,7 +365,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
             }
           }
         }
-        feed.publish(ti);
+        feed.publish(ti, w0, M0);
         if (ti == kNoTile) break;
         if (ptx::ld_shared_volatile_u32(prod_done) < wait_for) {
           const long long t0 = clock64();
@@ -360,12 +386,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       uint32_t acc_phase = 0;                                      // bit per accumulator
       for (;;) {
         const uint32_t ti = __shfl_sync(0xffffffffu, feed.peek(), 0);
+        Work w;
+        TcMat M;
+        feed.read(w, M);
         __syncwarp();
         feed.release(lane == 0);
         if (ti == kNoTile) break;
-        const Work w = fetch(p, ti);
         const TcTile t = w.t;
-        const TcMat M = p.mats[t.mat];
         const TileCfg c = decode(p, t, M, w.src);
         // K-major: +32 B per 16-k step; MN-major: +16 rows of 128 B.  (descriptor address field is in 16-byte units)
         const uint32_t a_step = c.a_mn ? (2048u >> 4) : (32u >> 4), b_step = c.b_mn ? (2048u >> 4) : (32u >> 4);
@@ -451,12 +478,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       // with a report outstanding
       if (pend_mat != kNoTile && !__shfl_sync(0xffffffffu, (uint32_t)feed.ready(), 0)) report(n_store - pend_seq);
       const uint32_t ti = feed.peek();
+      Work w;
+      TcMat M;
+      feed.read(w, M);
       __syncwarp();
       feed.release(lane == 0);
       if (ti == kNoTile) break;
-      const Work w = fetch(p, ti);
       const TcTile t = w.t;
-      const TcMat M = p.mats[t.mat];
       const TileCfg c = decode(p, t, M, w.src);
       const float inv = w.first ? p.inv_norm[t.mat] : 1.f;
       const float alpha = t.phase == PH_GRAM ? inv * inv : inv;
