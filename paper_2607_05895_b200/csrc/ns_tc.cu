@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
             const long long t0 = clock64();
             while (ptx::ld_acquire_gpu(flag) < need) {
               __nanosleep(64);
-              if (clock64() - t0 > 4000000000ll) __trap();
+              if (clock64() - t0 > 20000000000ll) __trap();
             }
           }
         }
@@ -371,7 +371,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
           const long long t0 = clock64();
           while (ptx::ld_shared_volatile_u32(prod_done) < wait_for) {
             __nanosleep(256);
-            if (clock64() - t0 > 4000000000ll) __trap();
+            if (clock64() - t0 > 20000000000ll) __trap();
           }
         }
       }

@@ -37,13 +37,13 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
       : "memory");
   return ok;
 }
-// Spins until the phase with the given parity has completed.  A wait that lasts longer than ~2 s of SM clocks can
+// Spins until the phase with the given parity has completed.  A wait that lasts longer than ~10 s of SM clocks can
 // only be a protocol bug: trap (the launch then fails with an error) instead of hanging the device.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
   while (!mbar_try_wait(bar, parity)) {
-    if (clock64() - t0 > 4000000000ll) __trap();
+    if (clock64() - t0 > 20000000000ll) __trap();
   }
 }
 // The same wait with acquire semantics at CLUSTER scope (data published by a thread of the peer CTA).
@@ -64,7 +64,7 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
   if (mbar_try_wait_cluster(bar, parity)) return;
   const long long t0 = clock64();
   while (!mbar_try_wait_cluster(bar, parity)) {
-    if (clock64() - t0 > 4000000000ll) __trap();
+    if (clock64() - t0 > 20000000000ll) __trap();
   }
 }
 __device__ __forceinline__ void st_shared_u32(uint32_t addr, uint32_t v) {
