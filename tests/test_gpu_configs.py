@@ -1,12 +1,11 @@
 """GPU parity at BASELINE.json's full sizes (`-m gpu`), in the launch configuration bench.py times.
 
 C2 and C3 are compared with the full fp64 oracle (C2: every matrix at step 1, one matrix per shape at later steps; M,
-||U||^2, the lock-step update and the AdamW tails on everything at every step).  C4 / C5 matrices are too large for a
-full fp64 NS in test time, so: momentum state, ||U||^2 and the lock-step update are checked on EVERY matrix by the
-oracle's elementwise functions; O is checked against the full oracle on the matrices it can do in seconds (the
-1024-row k/v projections); and every matrix gets the size-independent probe identities of
-gpu_harness.probe_last_iteration (one per GEMM phase + fused epilogue) and a singular-value band check by random
-probes."""
+||U||^2, the lock-step update and the AdamW tails on everything at every step).  C4 / C5: one matrix per DISTINCT
+shape of the resident set gets the full fp64 oracle (4096 x 4096, 1024 x 4096, 14336 x 4096, 4096 x 14336; 8192 x 8192,
+1024 x 8192, 28672 x 8192 -- about 4-5 minutes of dgemm on the box's host cores); every matrix gets momentum state,
+||U||^2 and the lock-step update from the oracle's elementwise functions, the size-independent probe identities of
+gpu_harness.probe_last_iteration (one per GEMM phase + fused epilogue) and a singular-value band check."""
 import numpy as np
 import pytest
 import torch
@@ -123,37 +122,45 @@ def _band_by_probes(O, rng, lo=0.55, hi=1.35):
     assert lo ** 2 <= mean_sq <= hi ** 2, mean_sq
 
 
-def _large_config(name, full_oracle_max_rows):
+def _large_config(name):
+    """One full fp64-oracle comparison (M, ||U||^2, O over the whole K-step chain, lock-step update) per DISTINCT shape
+    of the resident set -- the 4096- / 8192-row matrices that carry > 99 % of the flops included (north_star: "matching
+    the fp64 oracle ... on all five configs") -- and, on every other matrix, the oracle's elementwise functions for M,
+    ||U||^2 and the update plus the size-independent probes."""
     wl = workloads.get(name)
     sess = gh.Session(wl)
     sess.load_grads(0)
     rng = np.random.default_rng(11)
-    n_full = 0
+    seen = {}
     # W_old / M_old one matrix at a time (host memory): M starts at zero, W_old is the seeded input
     sess.muon_step()
     for i, d in enumerate(sess.mats):
         W_old = sess.seg(sess.hW, d).to(torch.float64).numpy()
         M_old = np.zeros((d.rows, d.cols))
-        if min(d.rows, d.cols) <= full_oracle_max_rows and n_full < 3:
-            gh.check_matrix_against_oracle(sess, i, W_old, M_old)
-            n_full += 1
+        if (d.rows, d.cols) not in seen:
+            eo, _ = gh.check_matrix_against_oracle(sess, i, W_old, M_old)
+            seen[(d.rows, d.cols)] = eo
             O = sess.read_O(i)
         else:
             O = _elementwise_checks(sess, i, W_old, M_old)
         _band_by_probes(O, rng)
         del O, W_old, M_old
         gh.probe_last_iteration(sess, i, rng, 2e-2)
-    assert n_full >= 1
+    print("%s: relF(O) vs fp64 oracle per distinct shape: %s" % (name, ", ".join(
+        "%dx%d %.2e" % (r, c, e) for (r, c), e in seen.items())))
+    assert max(seen.values()) <= 3e-2
     state = {}
     _adamw_check(sess, 1, state)
-    return sess
+    return sess, seen
 
 
 def test_c4_llama8b_rank0():
-    sess = _large_config("c4", 1024)
+    sess, seen = _large_config("c4")
     assert len(sess.mats) == 30
+    assert set(seen) == {(4096, 4096), (1024, 4096), (14336, 4096), (4096, 14336)}
 
 
 def test_c5_llama70b_heaviest():
-    sess = _large_config("c5", 1024)
+    sess, seen = _large_config("c5")
     assert len(sess.mats) == 13
+    assert set(seen) == {(8192, 8192), (1024, 8192), (28672, 8192)}
