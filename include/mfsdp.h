@@ -19,7 +19,15 @@
  *   * Asynchrony: the *_step functions enqueue work on `cuda_stream` (a cudaStream_t passed as void*, NULL = the
  *     legacy default stream) and return without synchronising.  G is read-only; W, M (P, m, v) are updated in place.
  *   * Errors: 0 on success, a negative MFSDP_E* code otherwise; nothing is printed, nothing throws or aborts.
- *   * Determinism: fixed reduction order and a static tile schedule -> same inputs give bit-identical outputs.
+ *   * Determinism: same inputs give bit-identical outputs, run to run.  The Newton-Schulz tiles are handed to the
+ *     SMs by a DYNAMIC scheduler (an atomic claim counter), so which unit computes a tile and when varies; every
+ *     output tile is computed by exactly one unit with a fixed k order, and every norm by a fixed-order reduction,
+ *     so the values do not depend on the schedule (tests/test_gpu_parity.py::test_run_to_run_determinism).
+ *   * Dynamic range: the Frobenius normalisation is folded into the first Newton-Schulz iteration (the Gram matrix
+ *     of the UNNORMALISED bf16/fp32 momentum update U is accumulated in fp32 and scaled by 1/||U||^2 afterwards), so
+ *     u_i u_j must stay inside fp32's normal range: supported rms(U) is about 1e-17 .. 1e+16 (gradients of real
+ *     training runs sit around 1e-6 .. 1e+2).  Inside that range the result is invariant to the scale of G exactly
+ *     like the definition (power-of-two scalings give bit-identical O; tested).
  *   * There is NO CPU fallback: on a machine without an sm_100 device the step functions return MFSDP_EARCH.
  */
 #ifndef MFSDP_H_
@@ -48,7 +56,8 @@ enum { MFSDP_PARAM_SKIP = 1u };                               /* mfsdp_param_t.f
 enum { MFSDP_DESC_TRANSPOSED = 1u };                          /* mfsdp_desc_t.flags bit0: rows > cols (NS runs on X^T) */
 enum { MFSDP_SEG_ALIGN = 64 };                                /* every segment starts on a 64-element boundary    */
 
-enum { MFSDP_OK = 0, MFSDP_EINVAL = -1, MFSDP_ECAP = -2, MFSDP_ELAYOUT = -3, MFSDP_EARCH = -4, MFSDP_ECUDA = -5 };
+enum { MFSDP_OK = 0, MFSDP_EINVAL = -1, MFSDP_ECAP = -2, MFSDP_ELAYOUT = -3, MFSDP_EARCH = -4, MFSDP_ECUDA = -5,
+       MFSDP_ECACHE = -6 };                                   /* launch-table cache full, see mfsdp_release_plans  */
 
 /* ---- records ------------------------------------------------------------------------------------------------ */
 /* One model parameter, in model order (planner input). */
@@ -153,12 +162,21 @@ int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision,
  *   cuda_stream    cudaStream_t (NULL = the legacy default stream).  Work is enqueued, not awaited.  After one
  *                              ordinary call with the same (table, workspace, precision) -- which builds the cached
  *                              launch tables with cudaMalloc / cudaMemcpy -- the step is CUDA-graph capturable (one
- *                              memset node and the kernel launches).
- *                              The library caches, per (table, workspace pointer, precision), a few KB..MB of
- *                              launch tables (TMA tensor maps, tile lists) in device memory of its own.
+ *                              memset node and the kernel launches).  The hyper-parameters are baked into the
+ *                              captured kernel arguments: re-capture when lr, momentum, ... change (for AdamW the
+ *                              bias correction depends on hp->step, so every step needs its own capture or an
+ *                              eager call).
+ *                              The library caches, per (device, table contents, WORKSPACE POINTER, precision), a few
+ *                              KB..MB of launch tables (TMA tensor maps hold the workspace address; tile lists) in
+ *                              device memory of its own.  Entries are never evicted (launches in flight and captured
+ *                              graphs reference them): keep the workspace pointer stable across steps.  After 1024
+ *                              distinct keys the call fails with MFSDP_ECACHE until mfsdp_release_plans() is called.
  *   hp             HOST in.
  * Returns MFSDP_EINVAL (null / misaligned pointer, bad hyper-parameter, mixed dtypes), MFSDP_ECAP (ws_bytes too
- * small), MFSDP_ELAYOUT, MFSDP_EARCH (current device is not compute capability 10.x), MFSDP_ECUDA. */
+ * small), MFSDP_ELAYOUT, MFSDP_EARCH (current device is not compute capability 10.x), MFSDP_ECUDA, MFSDP_ECACHE.
+ * Thread safety: step functions may be called from several host threads (the cache is locked; counters are atomic;
+ * mfsdp_strerror(MFSDP_ECUDA) is per calling thread).  mfsdp_tune, mfsdp_debug_trace and mfsdp_release_plans must not
+ * run concurrently with step calls. */
 int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
                     void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
 
@@ -199,21 +217,29 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  * out[4] = X row pitch in elements, out[5] = A/P row pitch in elements. */
 int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t index, size_t out[6]);
 
+/* Frees every cached launch table of the process after synchronising their devices (HOST).  The caller guarantees
+ * that no CUDA graph captured from a step call will be replayed afterwards.  Always MFSDP_OK. */
+int mfsdp_release_plans(void);
+
 /* ---- tuning knobs (HOST) -------------------------------------------------------------------------------------
  * Scheduling choices of the tensor-core Newton-Schulz path.  They change HOW tiles are formed and ordered, never
  * what is computed (tests run the parity suite under several settings).  Setting a knob synchronises the device
- * and drops the cached launch tables, which are rebuilt on the next step.  Initial values come from the
- * environment variables of the same names, else the defaults below.
+ * and drops the cached launch tables, which are rebuilt on the next step.  The values below are the only initial
+ * state (no environment variables).
  *   MFSDP_TUNE_PAIR_MIN_D   matrices with min(rows, cols) >= value run on CTA pairs (tcgen05 cta_group::2,
- *                           256 x 256 tiles); smaller ones on single CTAs (128 x N tiles).  default 768
+ *                           256 x 512 output tiles held as two 256-column TMEM accumulators, 256 x 256 in phases
+ *                           with a short k loop); smaller ones on single CTAs (128 x N tiles).  default 768
  *   MFSDP_TUNE_SYM_BAND     row blocks per band of the symmetric (GRAM, POLY) tile order, single-CTA class.  16
  *   MFSDP_TUNE_SYM_BAND2    the same for the CTA-pair class.  8
  *   MFSDP_TUNE_RECT_GROUP   column tiles per panel of the rectangular (APPLY) tile order.  4
  *   MFSDP_TUNE_WIDE_MIN_KB  CTA-pair tiles are 512 columns wide (else 256) in phases whose k loop has at least this
  *                           many 64-element blocks.  8
+ *   MFSDP_TUNE_FUSED_BELOW_D matrices with min(rows, cols) < value whose padded X fits 128 KB of shared memory run in
+ *                           the whole-matrix kernel (one CTA keeps X, A and P on chip for all K iterations); 1 switches
+ *                           that kernel off.  129
  * Returns MFSDP_EINVAL for an unknown knob or value < 1; mfsdp_get_tune returns the value or a negative code. */
 enum { MFSDP_TUNE_PAIR_MIN_D = 0, MFSDP_TUNE_SYM_BAND = 1, MFSDP_TUNE_SYM_BAND2 = 2, MFSDP_TUNE_RECT_GROUP = 3,
-       MFSDP_TUNE_WIDE_MIN_KB = 4, MFSDP_TUNE_COUNT_ = 5 };
+       MFSDP_TUNE_WIDE_MIN_KB = 4, MFSDP_TUNE_FUSED_BELOW_D = 5, MFSDP_TUNE_COUNT_ = 6 };
 int mfsdp_tune(int knob, int value);
 int mfsdp_get_tune(int knob);
 
@@ -228,8 +254,8 @@ int mfsdp_get_tune(int knob);
 int mfsdp_debug_trace(void* dev_buf, size_t bytes);
 
 /* ---- misc ----------------------------------------------------------------------------------------------------- */
-const char* mfsdp_strerror(int code);      /* static string; for MFSDP_ECUDA the last CUDA error text            */
-int mfsdp_version(void);                   /* ABI version, currently 1                                            */
+const char* mfsdp_strerror(int code);      /* static string; for MFSDP_ECUDA the calling thread's last CUDA error */
+int mfsdp_version(void);                   /* ABI version, currently 2                                            */
 /* Number of kernels the library launched since process start (for bench.py's gpu_launches claim). */
 uint64_t mfsdp_launch_count(void);
 

@@ -11,7 +11,7 @@ POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY = 0, 1
 METRIC_NUMEL, METRIC_NS_FLOPS = 0, 1
 SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE = 0, 1, 2
 NS_BF16, NS_FP32 = 0, 1
-OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE = 0, -1, -2, -3, -4, -5, -6
 
 
 class Param(C.Structure):            # mfsdp_param_t
@@ -65,7 +65,8 @@ class PlanResult:
 _SYMBOLS = ["mfsdp_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
-            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace"]
+            "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
+            "mfsdp_release_plans"]
 _lib = None
 
 
@@ -180,7 +181,11 @@ def mfsdp_launch_count():
     return int(load().mfsdp_launch_count())
 
 
-TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB = 0, 1, 2, 3, 4
+TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D = 0, 1, 2, 3, 4, 5
+
+
+def mfsdp_release_plans():
+    _check(load().mfsdp_release_plans(), "mfsdp_release_plans")
 
 
 def mfsdp_tune(knob, value):

@@ -1,9 +1,10 @@
 // C-ABI entry points of the step (include/mfsdp.h): argument checks, workspace layout, the per-table cache of
 // device launch tables, and the launch sequence.  No compute happens here and there is no CPU fallback.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
 #include <string>
 
@@ -13,44 +14,39 @@ namespace mfsdp {
 
 // ---- bookkeeping ------------------------------------------------------------------------------------------------
 namespace {
-std::mutex g_mu;
-std::mutex g_host_mu;   // serialises mfsdp_muon_step_host (one set of copy streams)
-uint64_t g_launches = 0;
-std::string g_cuda_err = "no CUDA error recorded";
+std::mutex g_mu;        // plan cache, lazily built launch tables, trace target
+std::mutex g_host_mu;   // serialises mfsdp_muon_step_host (one set of copy streams per device)
+std::atomic<uint64_t> g_launches{0};
+thread_local std::string g_cuda_err = "no CUDA error recorded";   // per calling thread (mfsdp_strerror)
 std::vector<Plan*> g_plans;
 std::vector<std::vector<uint8_t>> g_plan_keys;
-}  // namespace
+constexpr size_t kMaxPlans = 1024;   // cached launch tables; beyond it get_plan fails loudly (MFSDP_ECACHE)
 
-namespace {
-int g_tune[MFSDP_TUNE_COUNT_];
-bool g_tune_init = false;
-void tune_init() {
-  if (g_tune_init) return;
-  static const char* names[MFSDP_TUNE_COUNT_] = {"MFSDP_TUNE_PAIR_MIN_D", "MFSDP_TUNE_SYM_BAND",
-                                                 "MFSDP_TUNE_SYM_BAND2", "MFSDP_TUNE_RECT_GROUP",
-                                                 "MFSDP_TUNE_WIDE_MIN_KB"};
-  static const int dflt[MFSDP_TUNE_COUNT_] = {768, 16, 8, 4, 8};
-  for (int k = 0; k < MFSDP_TUNE_COUNT_; ++k) {
-    const char* e = getenv(names[k]);
-    const int v = e && *e ? atoi(e) : 0;
-    g_tune[k] = v >= 1 ? v : dflt[k];
-  }
-  g_tune_init = true;
-}
-}  // namespace
+// Scheduling knobs (mfsdp_tune): defaults only -- no environment variables, no other hidden state.
+std::atomic<int> g_tune[MFSDP_TUNE_COUNT_] = {{768}, {16}, {8}, {4}, {8}, {129}};
 
-namespace {
 unsigned long long* g_trace = nullptr;
 uint32_t g_trace_cap = 0;
-}  // namespace
-void get_trace(unsigned long long** buf, uint32_t* cap) { *buf = g_trace; *cap = g_trace_cap; }
 
-int tune_value(int knob) {
-  tune_init();
-  return knob >= 0 && knob < MFSDP_TUNE_COUNT_ ? g_tune[knob] : -1;
+void free_plan(Plan* pl) {
+  if (!pl) return;
+  cudaFree(pl->d_mats); cudaFree(pl->d_tails); cudaFree(pl->d_chunk_begin); cudaFree(pl->d_tail_chunk_begin);
+  cudaFree(pl->d_chunk_mat); cudaFree(pl->d_chunk_tail);
+  destroy_ns_tc(pl->tc);
+  delete pl;
+}
+}  // namespace
+
+std::mutex& plan_mutex() { return g_mu; }
+
+void get_trace(unsigned long long** buf, uint32_t* cap) {
+  std::lock_guard<std::mutex> lock(g_mu);
+  *buf = g_trace; *cap = g_trace_cap;
 }
 
-void count_launch(uint64_t n) { g_launches += n; }
+int tune_value(int knob) { return knob >= 0 && knob < MFSDP_TUNE_COUNT_ ? g_tune[knob].load() : -1; }
+
+void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 int cuda_fail(cudaError_t e) {
   g_cuda_err = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e);
   return MFSDP_ECUDA;
@@ -171,21 +167,16 @@ int get_plan(const mfsdp_desc_t* desc, size_t n_desc, int precision, void* works
     for (uint32_t c = cb[i]; c < cb[i + 1]; ++c) cm[c] = (uint32_t)i;
   for (size_t i = 0; i < lay.tails.size(); ++i)
     for (uint32_t c = tcb[i]; c < tcb[i + 1]; ++c) ct[c] = (uint32_t)i;
+  // A cached plan is never freed behind the caller's back (launches in flight and captured CUDA graphs reference its
+  // device tables): a full cache is an error the caller resolves with mfsdp_release_plans().
+  if (g_plans.size() >= kMaxPlans) { delete pl; return MFSDP_ECACHE; }
   if ((rc = upload(&pl->d_mats, lay.mats.data(), lay.mats.size())) ||
       (rc = upload(&pl->d_tails, lay.tails.data(), lay.tails.size())) ||
       (rc = upload(&pl->d_chunk_begin, cb.data(), cb.size())) ||
       (rc = upload(&pl->d_tail_chunk_begin, tcb.data(), tcb.size())) ||
       (rc = upload(&pl->d_chunk_mat, cm.data(), cm.size())) || (rc = upload(&pl->d_chunk_tail, ct.data(), ct.size()))) {
-    return rc;   // a failed cudaMalloc on a tiny table: leave the partial plan to process teardown
-  }
-  if (g_plans.size() >= 64) {          // bound the cache: drop the oldest entry
-    Plan* old = g_plans.front();
-    cudaFree(old->d_mats); cudaFree(old->d_tails); cudaFree(old->d_chunk_begin); cudaFree(old->d_tail_chunk_begin);
-    cudaFree(old->d_chunk_mat); cudaFree(old->d_chunk_tail);
-    destroy_ns_tc(old->tc);
-    delete old;
-    g_plans.erase(g_plans.begin());
-    g_plan_keys.erase(g_plan_keys.begin());
+    free_plan(pl);
+    return rc;
   }
   g_plans.push_back(pl);
   g_plan_keys.push_back(std::move(key));
@@ -319,12 +310,13 @@ struct HostPipe {
   cudaEvent_t start = nullptr, gm_in = nullptr, w_in = nullptr, mom = nullptr, m_out = nullptr;
   int device = -1;
 };
-HostPipe g_pipe;
+std::map<int, HostPipe> g_pipes;         // one per device, created on first use (guarded by g_host_mu)
 int host_pipe(HostPipe** out) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return cuda_fail(e);
-  if (g_pipe.device != dev) {            // (re)create for the current device; the old objects are left to the driver
+  HostPipe& g_pipe = g_pipes[dev];
+  if (g_pipe.device != dev) {
     HostPipe p;
     if ((e = cudaStreamCreateWithFlags(&p.in, cudaStreamNonBlocking)) != cudaSuccess ||
         (e = cudaStreamCreateWithFlags(&p.out, cudaStreamNonBlocking)) != cudaSuccess)
@@ -359,7 +351,10 @@ extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, voi
   if ((rc = host_pipe(&hpipe))) return rc;
   HostPipe& q = *hpipe;
   cudaError_t e;
-#define MFSDP_TRY(call) do { if ((e = (call)) != cudaSuccess) return cuda_fail(e); } while (0)
+  // On any failure the copies already queued may still be reading or writing the caller's host buffers: drain the
+  // three streams before returning, so that the caller may free or reuse them.
+  auto bail = [&](int code) { cudaStreamSynchronize(q.in); cudaStreamSynchronize(q.out); cudaStreamSynchronize(st); return code; };
+#define MFSDP_TRY(call) do { if ((e = (call)) != cudaSuccess) return bail(cuda_fail(e)); } while (0)
   // in:  G, M (needed by the momentum pass), then W (needed only by the update pass: rides under Newton-Schulz)
   MFSDP_TRY(cudaEventRecord(q.start, st));
   MFSDP_TRY(cudaStreamWaitEvent(q.in, q.start, 0));
@@ -370,15 +365,15 @@ extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, voi
   MFSDP_TRY(cudaEventRecord(q.w_in, q.in));
   // compute on the caller's stream
   MFSDP_TRY(cudaStreamWaitEvent(st, q.gm_in, 0));
-  if ((rc = launch_momentum(*pl, dG, dM, *hp, st))) return rc;
+  if ((rc = launch_momentum(*pl, dG, dM, *hp, st))) return bail(rc);
   MFSDP_TRY(cudaEventRecord(q.mom, st));
   // out: M is final after the momentum pass: its download rides under Newton-Schulz too
   MFSDP_TRY(cudaStreamWaitEvent(q.out, q.mom, 0));
   MFSDP_TRY(cudaMemcpyAsync(hM, dM, elems * 4, cudaMemcpyDeviceToHost, q.out));
   MFSDP_TRY(cudaEventRecord(q.m_out, q.out));
-  if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
+  if ((rc = ns_dispatch(*pl, *hp, st))) return bail(rc);
   MFSDP_TRY(cudaStreamWaitEvent(st, q.w_in, 0));
-  if ((rc = launch_update(*pl, dW, *hp, st))) return rc;
+  if ((rc = launch_update(*pl, dW, *hp, st))) return bail(rc);
   MFSDP_TRY(cudaMemcpyAsync(hW, dW, elems * es, cudaMemcpyDeviceToHost, st));
   MFSDP_TRY(cudaStreamWaitEvent(st, q.m_out, 0));
   MFSDP_TRY(cudaStreamSynchronize(st));
@@ -403,9 +398,8 @@ extern "C" int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, vo
 extern "C" int mfsdp_tune(int knob, int value) {
   if (knob < 0 || knob >= MFSDP_TUNE_COUNT_ || value < 1) return MFSDP_EINVAL;
   std::lock_guard<std::mutex> lock(g_mu);
-  tune_init();
-  if (g_tune[knob] == value) return MFSDP_OK;
-  g_tune[knob] = value;
+  if (g_tune[knob].load() == value) return MFSDP_OK;
+  g_tune[knob].store(value);
   bool any = false;
   for (Plan* pl : g_plans) any |= pl->tc != nullptr;
   if (any) {
@@ -425,8 +419,21 @@ extern "C" int mfsdp_debug_trace(void* dev_buf, size_t bytes) {
 
 extern "C" int mfsdp_get_tune(int knob) {
   if (knob < 0 || knob >= MFSDP_TUNE_COUNT_) return MFSDP_EINVAL;
-  std::lock_guard<std::mutex> lock(g_mu);
   return tune_value(knob);
+}
+
+extern "C" int mfsdp_release_plans(void) {
+  std::lock_guard<std::mutex> lock(g_mu);
+  int dev = 0;
+  const bool have_dev = cudaGetDevice(&dev) == cudaSuccess;
+  for (Plan* pl : g_plans) {             // launches still in flight may be reading the tables
+    if (have_dev && cudaSetDevice(pl->device) == cudaSuccess) cudaDeviceSynchronize();
+    free_plan(pl);
+  }
+  if (have_dev) cudaSetDevice(dev);
+  g_plans.clear();
+  g_plan_keys.clear();
+  return MFSDP_OK;
 }
 
 extern "C" const char* mfsdp_strerror(int code) {
@@ -437,9 +444,11 @@ extern "C" const char* mfsdp_strerror(int code) {
     case MFSDP_ELAYOUT: return "descriptor table violates the one-contiguous-segment layout";
     case MFSDP_EARCH: return "no compute-capability-10.x (sm_100) device; there is no CPU fallback";
     case MFSDP_ECUDA: return g_cuda_err.c_str();
+    case MFSDP_ECACHE: return "launch-table cache full (1024 distinct (table, workspace, precision) keys): keep the "
+                              "workspace pointer stable, or call mfsdp_release_plans()";
     default: return "unknown error code";
   }
 }
 
-extern "C" int mfsdp_version(void) { return 1; }
-extern "C" uint64_t mfsdp_launch_count(void) { return g_launches; }
+extern "C" int mfsdp_version(void) { return 2; }
+extern "C" uint64_t mfsdp_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
 #include <vector>
 
 #include "mfsdp.h"
@@ -86,8 +87,9 @@ void count_launch(uint64_t n = 1);
 int cuda_fail(cudaError_t e);          // records the error text, returns MFSDP_ECUDA
 int check_last_launch();               // cudaGetLastError -> code
 
-int tune_value(int knob);
-void get_trace(unsigned long long** buf, uint32_t* cap);   // mfsdp_debug_trace target (null when off)               // current value of an MFSDP_TUNE_* knob
+int tune_value(int knob);                                  // current value of an MFSDP_TUNE_* knob
+void get_trace(unsigned long long** buf, uint32_t* cap);   // mfsdp_debug_trace target (null when off)
+std::mutex& plan_mutex();                                  // guards the plan cache and lazily built launch tables
 
 inline uint64_t align_up_u64(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
 

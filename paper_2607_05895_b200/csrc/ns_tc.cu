@@ -749,7 +749,7 @@ int build_tc_plan(Plan& pl) {
   std::vector<CUtensorMap> maps(TM_COUNT * lay.mats.size());
   std::vector<TcMat> mats(lay.mats.size());
   std::vector<TcTile> tiles[2];
-  // big matrices first so that the static round-robin over units ends with the cheap tiles
+  // big matrices first so that every phase of the tile list ends with the cheap tiles (dynamic claims, list order)
   std::vector<uint32_t> order(lay.mats.size());
   for (uint32_t i = 0; i < order.size(); ++i) order[i] = i;
   std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) {
@@ -849,9 +849,12 @@ void destroy_ns_tc(NsTcPlan* p) {
 
 int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
   if (pl.lay.mats.empty()) return MFSDP_OK;
-  if (!pl.tc) {
-    const int rc = build_tc_plan(pl);
-    if (rc) { destroy_ns_tc(pl.tc); pl.tc = nullptr; return rc; }
+  {
+    std::lock_guard<std::mutex> lock(plan_mutex());     // two threads stepping the same table build it once
+    if (!pl.tc) {
+      const int rc = build_tc_plan(pl);
+      if (rc) { destroy_ns_tc(pl.tc); pl.tc = nullptr; return rc; }
+    }
   }
   NsTcPlan& tc = *pl.tc;
   TcParams p;

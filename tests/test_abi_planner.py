@@ -23,7 +23,7 @@ def test_library_exports_every_declared_symbol():
     for name in sorted(declared):
         assert hasattr(lib, name), "libmfsdp.so does not export %s" % name
     assert declared == set(mf.exported_symbols()), "binding and header disagree on the entry points"
-    assert mf.mfsdp_version() == 1
+    assert mf.mfsdp_version() == 2
 
 
 def test_struct_sizes_match_header_layout():
@@ -166,9 +166,10 @@ def test_step_entry_points_reject_bad_arguments_without_a_gpu():
 
 def test_tune_knobs_roundtrip_and_reject_bad_values():
     """mfsdp_tune / mfsdp_get_tune are host-only: defaults, round trip, error codes (no device needed)."""
-    knobs = [mf.TUNE_PAIR_MIN_D, mf.TUNE_SYM_BAND, mf.TUNE_SYM_BAND2, mf.TUNE_RECT_GROUP, mf.TUNE_WIDE_MIN_KB]
+    knobs = [mf.TUNE_PAIR_MIN_D, mf.TUNE_SYM_BAND, mf.TUNE_SYM_BAND2, mf.TUNE_RECT_GROUP, mf.TUNE_WIDE_MIN_KB,
+             mf.TUNE_FUSED_BELOW_D]
     old = [mf.mfsdp_get_tune(k) for k in knobs]
-    assert all(v >= 1 for v in old)
+    assert old == [768, 16, 8, 4, 8, 129]         # the header's defaults; no environment variable can change them
     try:
         for k in knobs:
             mf.mfsdp_tune(k, 3)
