@@ -26,8 +26,9 @@
  *   * Dynamic range: the Frobenius normalisation is folded into the first Newton-Schulz iteration (the Gram matrix
  *     of the UNNORMALISED bf16/fp32 momentum update U is accumulated in fp32 and scaled by 1/||U||^2 afterwards), so
  *     u_i u_j must stay inside fp32's normal range: supported rms(U) is about 1e-17 .. 1e+16 (gradients of real
- *     training runs sit around 1e-6 .. 1e+2).  Inside that range the result is invariant to the scale of G exactly
- *     like the definition (power-of-two scalings give bit-identical O; tested).
+ *     training runs sit around 1e-6 .. 1e+2).  Inside that range, and above the clamp ||U||_F >= eps, the result is
+ *     invariant to the scale of G exactly like the definition (power-of-two scalings give bit-identical O; tested);
+ *     below eps the clamp X0 = U / eps applies, as in the definition.
  *   * There is NO CPU fallback: on a machine without an sm_100 device the step functions return MFSDP_EARCH.
  */
 #ifndef MFSDP_H_
@@ -54,6 +55,8 @@ enum { MFSDP_NS_BF16 = 0,                                     /* bf16 operands, 
        MFSDP_NS_FP32 = 1 };                                   /* fp32 operands and accumulate (FFMA), no TF32     */
 enum { MFSDP_PARAM_SKIP = 1u };                               /* mfsdp_param_t.flags bit0 (PAPER.md:45 TP skip)   */
 enum { MFSDP_DESC_TRANSPOSED = 1u };                          /* mfsdp_desc_t.flags bit0: rows > cols (NS runs on X^T) */
+enum { MFSDP_STEP_KEEP_O = 1u };                              /* mfsdp_muon_hparams_t.flags bit0: mfsdp_muon_step also
+                                                                 leaves O = X_K in the workspace (see mfsdp_muon_step) */
 enum { MFSDP_SEG_ALIGN = 64 };                                /* every segment starts on a 64-element boundary    */
 
 enum { MFSDP_OK = 0, MFSDP_EINVAL = -1, MFSDP_ECAP = -2, MFSDP_ELAYOUT = -3, MFSDP_EARCH = -4, MFSDP_ECUDA = -5,
@@ -97,6 +100,8 @@ typedef struct {
   int32_t ns_steps;      /* K >= 1 (north_star: 5; the paper's runs: 2)                             */
   int32_t scale_mode;    /* MFSDP_SCALE_*                                                                         */
   int32_t precision;     /* MFSDP_NS_BF16 | MFSDP_NS_FP32                                                         */
+  uint32_t flags;        /* MFSDP_STEP_*                                                                          */
+  uint32_t reserved;     /* 0                                                                                     */
 } mfsdp_muon_hparams_t;
 
 typedef struct {
@@ -157,7 +162,11 @@ int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision,
  *   G              DEVICE in.  rank-flat gradients, same dtype and offsets as W.
  *   M              DEVICE i/o. rank-flat momentum, always float, same element offsets.
  *   workspace      DEVICE.     >= mfsdp_workspace_bytes, 1024-byte aligned; contents need not be preserved
- *                              between calls; after the call it holds O and ||U||^2 (mfsdp_workspace_view).
+ *                              between calls; after the call it holds ||U||^2 and -- if hp->flags has
+ *                              MFSDP_STEP_KEEP_O, or the update could not be fused -- O (mfsdp_workspace_view).
+ *                              With bf16 weights and every cols % 8 == 0 (MFSDP_NS_BF16) the weight update runs
+ *                              inside the last Newton-Schulz epilogue straight from the accumulator tile, and O is
+ *                              written out only on request; the result is bit-identical to the separate passes.
  *                              May be NULL (and W, G, M too) when the table holds no matrix: the call is a no-op.
  *   cuda_stream    cudaStream_t (NULL = the legacy default stream).  Work is enqueued, not awaited.  After one
  *                              ordinary call with the same (table, workspace, precision) -- which builds the cached
@@ -221,6 +230,11 @@ int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precisio
  * that no CUDA graph captured from a step call will be replayed afterwards.  Always MFSDP_OK. */
 int mfsdp_release_plans(void);
 
+/* Which Newton-Schulz kernel class a rows x cols matrix runs in under MFSDP_NS_BF16 with the current knob values (HOST):
+ * 0 = whole-matrix kernel (X, A, P stay on chip: the A / P workspace buffers of mfsdp_debug_ws_offsets are NOT written),
+ * 1 = single-CTA tiles, 2 = CTA-pair tiles.  Negative code on rows == 0 or cols == 0. */
+int mfsdp_ns_class(uint32_t rows, uint32_t cols);
+
 /* ---- tuning knobs (HOST) -------------------------------------------------------------------------------------
  * Scheduling choices of the tensor-core Newton-Schulz path.  They change HOW tiles are formed and ordered, never
  * what is computed (tests run the parity suite under several settings).  Setting a knob synchronises the device
@@ -228,7 +242,9 @@ int mfsdp_release_plans(void);
  * state (no environment variables).
  *   MFSDP_TUNE_PAIR_MIN_D   matrices with min(rows, cols) >= value run on CTA pairs (tcgen05 cta_group::2,
  *                           256 x 512 output tiles held as two 256-column TMEM accumulators, 256 x 256 in phases
- *                           with a short k loop); smaller ones on single CTAs (128 x N tiles).  default 768
+ *                           with a short k loop); smaller ones on single CTAs (128 x N tiles).  default 1024
+ *                           (measured: GPT-2 768-row matrices run 14 % faster on single CTAs, 1024-row Llama k / v
+ *                           projections equally fast either way)
  *   MFSDP_TUNE_SYM_BAND     row blocks per band of the symmetric (GRAM, POLY) tile order, single-CTA class.  16
  *   MFSDP_TUNE_SYM_BAND2    the same for the CTA-pair class.  8
  *   MFSDP_TUNE_RECT_GROUP   column tiles per panel of the rectangular (APPLY) tile order.  4

@@ -11,6 +11,7 @@ POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY = 0, 1
 METRIC_NUMEL, METRIC_NS_FLOPS = 0, 1
 SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE = 0, 1, 2
 NS_BF16, NS_FP32 = 0, 1
+STEP_KEEP_O = 1
 OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE = 0, -1, -2, -3, -4, -5, -6
 
 
@@ -32,11 +33,13 @@ class Desc(C.Structure):             # mfsdp_desc_t
 class MuonHParams(C.Structure):      # mfsdp_muon_hparams_t
     _fields_ = [("lr", C.c_double), ("weight_decay", C.c_double), ("momentum", C.c_double), ("a", C.c_double),
                 ("b", C.c_double), ("c", C.c_double), ("eps", C.c_double), ("nesterov", C.c_int32),
-                ("ns_steps", C.c_int32), ("scale_mode", C.c_int32), ("precision", C.c_int32)]
+                ("ns_steps", C.c_int32), ("scale_mode", C.c_int32), ("precision", C.c_int32),
+                ("flags", C.c_uint32), ("reserved", C.c_uint32)]
 
     def __init__(self, lr=0.02, weight_decay=0.01, momentum=0.95, a=3.4445, b=-4.7750, c=2.0315, eps=1e-7,
-                 nesterov=1, ns_steps=5, scale_mode=SCALE_MATCH_RMS_ADAMW, precision=NS_BF16):
-        super().__init__(lr, weight_decay, momentum, a, b, c, eps, int(nesterov), ns_steps, scale_mode, precision)
+                 nesterov=1, ns_steps=5, scale_mode=SCALE_MATCH_RMS_ADAMW, precision=NS_BF16, flags=0):
+        super().__init__(lr, weight_decay, momentum, a, b, c, eps, int(nesterov), ns_steps, scale_mode, precision,
+                         flags, 0)
 
 
 class AdamWHParams(C.Structure):     # mfsdp_adamw_hparams_t
@@ -66,7 +69,7 @@ _SYMBOLS = ["mfsdp_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_work
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
             "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
-            "mfsdp_release_plans"]
+            "mfsdp_release_plans", "mfsdp_ns_class"]
 _lib = None
 
 
@@ -112,6 +115,7 @@ def load():
     lib.mfsdp_tune.argtypes = [i32, i32]
     lib.mfsdp_get_tune.argtypes = [i32]
     lib.mfsdp_debug_trace.argtypes = [vp, sz]
+    lib.mfsdp_ns_class.argtypes = [C.c_uint32, C.c_uint32]
     for name in _SYMBOLS:
         getattr(lib, name)          # AttributeError if the library does not export what the header declares
     _lib = lib
@@ -182,6 +186,13 @@ def mfsdp_launch_count():
 
 
 TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D = 0, 1, 2, 3, 4, 5
+
+
+def mfsdp_ns_class(rows, cols):
+    v = load().mfsdp_ns_class(int(rows), int(cols))
+    if v < 0:
+        _check(v, "mfsdp_ns_class")
+    return v
 
 
 def mfsdp_release_plans():

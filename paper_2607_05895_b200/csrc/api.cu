@@ -23,7 +23,7 @@ std::vector<std::vector<uint8_t>> g_plan_keys;
 constexpr size_t kMaxPlans = 1024;   // cached launch tables; beyond it get_plan fails loudly (MFSDP_ECACHE)
 
 // Scheduling knobs (mfsdp_tune): defaults only -- no environment variables, no other hidden state.
-std::atomic<int> g_tune[MFSDP_TUNE_COUNT_] = {{768}, {16}, {8}, {4}, {8}, {129}};
+std::atomic<int> g_tune[MFSDP_TUNE_COUNT_] = {{1024}, {16}, {8}, {4}, {8}, {129}};
 
 unsigned long long* g_trace = nullptr;
 uint32_t g_trace_cap = 0;
@@ -195,6 +195,7 @@ int check_hp(const mfsdp_muon_hparams_t* hp) {
   if (!(hp->eps > 0.0) || !(hp->lr == hp->lr) || !(hp->weight_decay == hp->weight_decay)) return MFSDP_EINVAL;
   if (hp->scale_mode < MFSDP_SCALE_MATCH_RMS_ADAMW || hp->scale_mode > MFSDP_SCALE_NONE) return MFSDP_EINVAL;
   if (hp->precision != MFSDP_NS_BF16 && hp->precision != MFSDP_NS_FP32) return MFSDP_EINVAL;
+  if ((hp->flags & ~(uint32_t)MFSDP_STEP_KEEP_O) || hp->reserved) return MFSDP_EINVAL;
   return MFSDP_OK;
 }
 
@@ -297,6 +298,8 @@ extern "C" int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W,
   if (!W || !G || !M || !aligned(W, 128) || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   if ((rc = launch_momentum(*pl, G, M, *hp, st))) return rc;
+  if (hp->precision == MFSDP_NS_BF16 && ns_tc_can_fuse_update(*pl))     // the update runs in the last APPLY epilogue
+    return launch_ns_tc(*pl, *hp, st, W, (hp->flags & MFSDP_STEP_KEEP_O) != 0);
   if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
   return launch_update(*pl, W, *hp, st);
 }
@@ -420,6 +423,11 @@ extern "C" int mfsdp_debug_trace(void* dev_buf, size_t bytes) {
 extern "C" int mfsdp_get_tune(int knob) {
   if (knob < 0 || knob >= MFSDP_TUNE_COUNT_) return MFSDP_EINVAL;
   return tune_value(knob);
+}
+
+extern "C" int mfsdp_ns_class(uint32_t rows, uint32_t cols) {
+  if (rows == 0 || cols == 0) return MFSDP_EINVAL;
+  return ns_class(rows, cols);
 }
 
 extern "C" int mfsdp_release_plans(void) {

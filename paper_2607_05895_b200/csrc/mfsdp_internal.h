@@ -79,8 +79,10 @@ int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaS
 int launch_adamw(const Plan& pl, void* P, const void* G, void* m, void* v, const mfsdp_adamw_hparams_t& hp,
                  cudaStream_t st);
 int launch_ns_fp32(const Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st);
-int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st);
+int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void* W = nullptr, bool keep_o = true);
+bool ns_tc_can_fuse_update(Plan& pl);   // bf16 weights, every cols % 8 == 0: the update runs in the last APPLY epilogue
 void destroy_ns_tc(NsTcPlan* p);
+int ns_class(uint32_t rows, uint32_t cols);   // 0 whole-matrix kernel, 1 single-CTA tiles, 2 CTA-pair tiles
 
 // ---- bookkeeping ---------------------------------------------------------------------------------------------
 void count_launch(uint64_t n = 1);

@@ -36,38 +36,10 @@
 #include <cstdlib>
 
 #include "mfsdp_internal.h"
+#include "ns_plan.h"
 #include "ptx_sm100.cuh"
 
 namespace mfsdp {
-
-enum { PH_GRAM = 0, PH_POLY = 1, PH_APPLY = 2 };
-// tensor maps per matrix
-enum { TM_X0 = 0, TM_X1 = 1, TM_A = 2, TM_P = 3,            // operand loads: box 64 x 64, 128-byte swizzle
-       TM_X0_ST = 4, TM_X1_ST = 5, TM_A_ST = 6, TM_P_ST = 7,  // epilogue tiles: box 64 cols x 32 rows, 128-byte swizzle
-       TM_A_MIR = 8, TM_P_MIR = 9,                            // mirror tiles: box 32 cols x 64 rows, no swizzle
-       TM_COUNT = 10 };
-
-struct TcMat {                 // device, one per matrix
-  uint64_t x_off[2], a_off, p_off;
-  uint32_t rows, cols, d, n_long, pitch_x, pitch_a, tall;
-  uint32_t reports_per_iter;   // completion reports (one per epilogue warp and tile) of one NS iteration of this matrix
-};
-// Output tile: origin (rows, cols of the OUTPUT buffer), k blocks, width in columns (multiple of 64; of 128 when
-// paired; <= 256 single CTA, <= 512 paired).
-// `need`: completion reports of the SAME matrix and iteration that must have been made before this tile's operands
-// may be read (= every tile of the matrix' earlier phases); `phase`: PH_*.
-struct TcTile { uint32_t mat, m0, n0; uint16_t nkb, nw; uint32_t need, phase, reports_per_iter, pad; };
-
-struct NsTcPlan {
-  CUtensorMap* d_tmaps = nullptr;   // TM_COUNT per matrix
-  TcMat* d_mats = nullptr;
-  TcTile* d_tiles[2] = {nullptr, nullptr};   // [kCG - 1]: the tiles of ONE iteration, GRAM then POLY then APPLY
-  uint32_t n_tiles[2] = {0, 0};
-  uint32_t* d_counters = nullptr;   // [2] tile counters (one per class) then [n_mat] completion reports; zeroed per pass
-  uint32_t n_mat = 0;
-  int sms = 148;
-  int max_pairs = 74;               // co-resident CTA pairs
-};
 
 namespace {
 
@@ -102,6 +74,7 @@ struct TcParams {
   uint32_t* done;               // [n_mat] completion reports of the pass so far (zero at the start of the pass)
   unsigned long long* trace;    // optional (mfsdp_debug_trace): [0] = record counter, then 6 words per tile
   uint32_t trace_cap, launch_idx;
+  UpdArgs ua;                   // weight update fused into the APPLY epilogue of the last iteration (ua.W != nullptr)
 };
 
 struct TileCfg {
@@ -494,6 +467,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       const bool rows_ok = rw0 < c.out_rows;                     // warp-uniform
       const bool sym = t.phase != PH_APPLY;
       const bool poly = t.phase == PH_POLY;
+      // last iteration's APPLY: W <- W (1 - lr wd) - lr s O right here, from the O tile held in registers (a4)
+      const bool upd = p.ua.W != nullptr && t.phase == PH_APPLY && w.it + 1 == p.ns_steps;   // warp-uniform
+      float coef = 0.f;
+      uint64_t w_elem = 0;
+      if (upd) {
+        const TcUpd* u = p.ua.upd + t.mat;
+        coef = (float)(p.ua.lr * u->scale[p.ua.scale_mode]);           // lr s, rounded once (as k_update does)
+        w_elem = u->elem_off;
+      }
       const uint32_t n_acc = t.nw > kBN ? 2u : 1u;
       const uint32_t acc0 = n_acc == 2 ? 0u : acc_next;
       acc_next = n_acc == 2 ? 0u : acc_next ^ 1u;
@@ -506,14 +488,24 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
         return cc < n_chunks && rows_ok && !(sym && ((t.n0 + 64 * cc) >> 7) < (rb0 >> 7));
       };
       // POLY: this thread's 64 A values of a chunk (row r, 128 contiguous bytes), fetched one chunk ahead through L2
-      // (A was written by other SMs during this launch: no L1)
-      const __nv_bfloat16* arow = reinterpret_cast<const __nv_bfloat16*>(p.ws + M.a_off) + (size_t)r * M.pitch_a + t.n0;
-      const bool a_ok = poly && r < c.out_rows;
+      // (A was written by other SMs during this launch: no L1).  Fused update: the thread's 64 W values likewise
+      // (bf16, row pitch = cols, cols % 8 == 0 so that a 16-byte vector never straddles the row end).
+      const __nv_bfloat16* arow = nullptr;
+      if (poly) arow = reinterpret_cast<const __nv_bfloat16*>(p.ws + M.a_off) + (size_t)r * M.pitch_a + t.n0;
+      else if (upd) arow = reinterpret_cast<const __nv_bfloat16*>(p.ua.W) + w_elem + (size_t)r * c.out_cols + t.n0;
+      const bool a_ok = (poly || upd) && r < c.out_rows;
       uint4 an[8];
       auto fetch_a = [&](uint32_t cc) {
         if (a_ok && writes(cc)) {
+          if (poly) {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) an[j] = ptx::ld_global_cg_v4(arow + 64 * cc + 8 * j);
+            for (int j = 0; j < 8; ++j) an[j] = ptx::ld_global_cg_v4(arow + 64 * cc + 8 * j);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+              an[j] = t.n0 + 64 * cc + 8 * j < c.out_cols ? *reinterpret_cast<const uint4*>(arow + 64 * cc + 8 * j)
+                                                         : make_uint4(0u, 0u, 0u, 0u);
+          }
         } else {
 #pragma unroll
           for (int j = 0; j < 8; ++j) an[j] = make_uint4(0u, 0u, 0u, 0u);
@@ -521,7 +513,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       };
       uint32_t first_cc = 0;
       while (first_cc < n_chunks && !writes(first_cc)) ++first_cc;
-      if (poly) fetch_a(first_cc);
+      if (poly || upd) fetch_a(first_cc);
 
       for (uint32_t h = 0; h < n_acc; ++h) {
         const uint32_t acc = acc0 + h;
@@ -537,7 +529,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
           if (!writes(cc)) continue;
           const uint32_t c0 = 64 * (cc & 3u), col0 = t.n0 + 64 * cc;
           uint4 a4[8];
-          if (poly) {
+          if (poly || upd) {
 #pragma unroll
             for (int j = 0; j < 8; ++j) a4[j] = an[j];
             uint32_t nx = cc + 1;
@@ -580,6 +572,26 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
           } else {
 #pragma unroll
             for (int j = 0; j < 32; ++j) pk[j] = pack_bf16(__uint_as_float(v[2 * j]), __uint_as_float(v[2 * j + 1]));
+          }
+          if (upd) {                                             // W <- fl(1 - lr wd) W - fl(lr s) O, O as stored (bf16)
+            if (a_ok) {
+              __nv_bfloat16* wrow = const_cast<__nv_bfloat16*>(arow) + 64 * cc;
+#pragma unroll
+              for (int j = 0; j < 8; ++j) {
+                if (col0 + 8 * j < c.out_cols) {
+                  const uint32_t ww[4] = {a4[j].x, a4[j].y, a4[j].z, a4[j].w};
+                  uint32_t nw[4];
+#pragma unroll
+                  for (int i = 0; i < 4; ++i) {
+                    const float o0 = __uint_as_float(pk[4 * j + i] << 16), o1 = __uint_as_float(pk[4 * j + i] & 0xffff0000u);
+                    const float w0 = __uint_as_float(ww[i] << 16), w1 = __uint_as_float(ww[i] & 0xffff0000u);
+                    nw[i] = pack_bf16(fmaf(-coef, o0, p.ua.decay * w0), fmaf(-coef, o1, p.ua.decay * w1));
+                  }
+                  *reinterpret_cast<uint4*>(wrow + 8 * j) = make_uint4(nw[0], nw[1], nw[2], nw[3]);
+                }
+              }
+            }
+            if (!p.ua.keep_o) continue;                          // O itself is not needed: nothing to store
           }
           // direct tile: row `lane` of the staging tile, swizzled; then one TMA store (clipped at the matrix edges)
 #pragma unroll
@@ -781,13 +793,26 @@ int build_tc_plan(Plan& pl) {
   // One iteration's tiles per class, phase-major (all GRAM tiles, then POLY, then APPLY): a launch walks this list
   // ns_steps times.  Paired tiles are 512 columns wide (one pass over the A operand feeds two accumulators) when the
   // k loop is long enough to hide the non-overlapped part of their epilogue, else 256 wide (double-buffered).
-  const uint32_t pair_min_d = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_PAIR_MIN_D));
   const uint32_t wide_min_kb = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_WIDE_MIN_KB));
+  const uint32_t fused_below_d = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_FUSED_BELOW_D));
+  // class 0 = whole-matrix kernel (ns_fused.cu: small d, X resident in shared memory), 1 = single-CTA tiles, 2 = CTA pairs
   std::vector<uint32_t> cls(lay.mats.size());
+  std::vector<FusedMat> fused[2];
+  for (uint32_t i : order) {                      // cost-sorted: the fused CTAs claim the expensive matrices first
+    const MatLayout& L = lay.mats[i];
+    FusedMat f;
+    int fc = 0;
+    cls[i] = (uint32_t)ns_class(L.rows, L.cols);
+    if (cls[i] == 0 && fused_eligible(L.rows, L.cols, fused_below_d, &f, &fc)) {
+      f.mat = i;
+      fused[fc].push_back(f);
+    }
+  }
   for (uint32_t ph = 0; ph < 3; ++ph)
     for (uint32_t i : order) {
       const MatLayout& L = lay.mats[i];
-      const uint32_t cg = cls[i] = L.d >= pair_min_d ? 2u : 1u;
+      const uint32_t cg = cls[i];
+      if (cg == 0) continue;
       const uint32_t nkb = ((ph == PH_GRAM ? L.n_long : L.d) + kBK - 1) / kBK;
       const uint32_t bn = cg == 2 && nkb >= wide_min_kb ? 2 * kBN : kBN;
       if (ph == PH_APPLY) tiles_rect(tiles[cg - 1], i, L.rows, L.cols, nkb, cg, bn, ph);
@@ -812,10 +837,31 @@ int build_tc_plan(Plan& pl) {
     tc->n_tiles[g] = (uint32_t)tiles[g].size();
     if ((rc = dev_upload(&tc->d_tiles[g], tiles[g]))) return rc;
   }
+  {
+    std::vector<TcUpd> upd(lay.mats.size());
+    tc->upd_ok = lay.mat_dtype == MFSDP_BF16;
+    for (size_t i = 0; i < lay.mats.size(); ++i) {
+      upd[i].elem_off = lay.mats[i].elem_off;
+      for (int k = 0; k < 3; ++k) upd[i].scale[k] = lay.mats[i].scale[k];
+      if (lay.mats[i].cols % 8u) tc->upd_ok = false;     // a 16-byte vector of a W row must not straddle the row end
+    }
+    if ((rc = dev_upload(&tc->d_upd, upd))) return rc;
+  }
+  for (int g = 0; g < 2; ++g) {
+    tc->n_fused[g] = (uint32_t)fused[g].size();
+    if ((rc = dev_upload(&tc->d_fused[g], fused[g]))) return rc;
+  }
+  if ((rc = fused_setup())) return rc;
   tc->n_mat = (uint32_t)lay.mats.size();
   cudaDeviceGetAttribute(&tc->sms, cudaDevAttrMultiProcessorCount, pl.device);
-  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), (2 + (size_t)tc->n_mat) * sizeof(uint32_t));
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), (kCounterWords + (size_t)tc->n_mat) * sizeof(uint32_t));
   if (e != cudaSuccess) return cuda_fail(e);
+  // the classes touch disjoint matrices: each runs on its own forked stream, joined before the pass returns
+  if ((e = cudaEventCreateWithFlags(&tc->fork, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
+  for (int k = 0; k < 3; ++k) {
+    if ((e = cudaStreamCreateWithFlags(&tc->side[k], cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e);
+    if ((e = cudaEventCreateWithFlags(&tc->join[k], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
+  }
   e = cudaFuncSetAttribute(k_ns_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
   if (e != cudaSuccess) return cuda_fail(e);
   e = cudaFuncSetAttribute(k_ns_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -840,14 +886,34 @@ int build_tc_plan(Plan& pl) {
 
 }  // namespace
 
+int ns_class(uint32_t rows, uint32_t cols) {
+  FusedMat f;
+  int fc = 0;
+  if (fused_eligible(rows, cols, (uint32_t)std::max(1, tune_value(MFSDP_TUNE_FUSED_BELOW_D)), &f, &fc)) return 0;
+  return std::min(rows, cols) >= (uint32_t)std::max(1, tune_value(MFSDP_TUNE_PAIR_MIN_D)) ? 2 : 1;
+}
+
 void destroy_ns_tc(NsTcPlan* p) {
   if (!p) return;
-  cudaFree(p->d_tmaps); cudaFree(p->d_mats); cudaFree(p->d_counters);
-  for (int g = 0; g < 2; ++g) cudaFree(p->d_tiles[g]);
+  cudaFree(p->d_tmaps); cudaFree(p->d_mats); cudaFree(p->d_counters); cudaFree(p->d_upd);
+  for (int g = 0; g < 2; ++g) { cudaFree(p->d_tiles[g]); cudaFree(p->d_fused[g]); }
+  if (p->fork) cudaEventDestroy(p->fork);
+  for (int k = 0; k < 3; ++k) {
+    if (p->join[k]) cudaEventDestroy(p->join[k]);
+    if (p->side[k]) cudaStreamDestroy(p->side[k]);
+  }
   delete p;
 }
 
-int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
+bool ns_tc_can_fuse_update(Plan& pl) {
+  std::lock_guard<std::mutex> lock(plan_mutex());
+  if (!pl.tc && build_tc_plan(pl)) { destroy_ns_tc(pl.tc); pl.tc = nullptr; return false; }
+  return pl.tc->upd_ok;
+}
+
+// W != nullptr (and ns_tc_can_fuse_update): the last APPLY epilogue also applies the weight update; O is then stored
+// only when keep_o is set.
+int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void* W, bool keep_o) {
   if (pl.lay.mats.empty()) return MFSDP_OK;
   {
     std::lock_guard<std::mutex> lock(plan_mutex());     // two threads stepping the same table build it once
@@ -864,28 +930,66 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
   p.a = (float)hp.a; p.b = (float)hp.b; p.c = (float)hp.c;
   get_trace(&p.trace, &p.trace_cap);
   p.launch_idx = 0;
+  p.ua.W = W && tc.upd_ok ? W : nullptr;
+  p.ua.upd = tc.d_upd;
+  p.ua.lr = hp.lr;
+  p.ua.decay = (float)(1.0 - hp.lr * hp.weight_decay);
+  p.ua.scale_mode = hp.scale_mode;
+  p.ua.keep_o = keep_o ? 1u : 0u;
   p.ns_steps = (uint32_t)hp.ns_steps;
-  p.done = tc.d_counters + 2;
+  p.done = tc.d_counters + kCounterWords;
   {
-    const cudaError_t e = cudaMemsetAsync(tc.d_counters, 0, (2 + (size_t)tc.n_mat) * sizeof(uint32_t), st);
+    const cudaError_t e = cudaMemsetAsync(tc.d_counters, 0, (kCounterWords + (size_t)tc.n_mat) * sizeof(uint32_t), st);
     if (e != cudaSuccess) return cuda_fail(e);
   }
-  // ONE launch per tile class for the whole pass (all iterations, all phases); the two classes touch disjoint matrices
-  for (int g = 1; g >= 0; --g) {
-    p.tiles = tc.d_tiles[g];
-    p.n_iter_tiles = tc.n_tiles[g];
-    if (p.n_iter_tiles == 0) continue;
-    p.counter = tc.d_counters + g;
-    const uint64_t total = (uint64_t)p.n_iter_tiles * p.ns_steps;
-    if (total >= 0xffffffffull) return MFSDP_EINVAL;
-    cudaError_t e;
-    if (g == 1) e = launch_class<2>(p, (uint32_t)std::min<uint64_t>(total, (uint64_t)tc.max_pairs), st);
-    else e = launch_class<1>(p, (uint32_t)std::min<uint64_t>(total, (uint64_t)tc.sms), st);
-    if (e != cudaSuccess) return cuda_fail(e);
-    ++p.launch_idx;
-    count_launch();
-    const int rc = check_last_launch();
+  // One launch per class for the whole pass (all iterations, all phases).  The classes touch disjoint matrices, so
+  // they run concurrently: the largest class stays on the caller's stream, the others are forked onto side streams
+  // and joined back.  The whole-matrix kernels go first: their CTAs leave the SMs after a few tens of microseconds and
+  // the persistent tile kernels pick the SMs up as they become free (tiles are claimed dynamically, so CTAs that
+  // start late simply claim later tiles).
+  struct Job { int kind; uint64_t work; };       // kind 0, 1 = fused class; 2 = single-CTA tiles; 3 = CTA-pair tiles
+  Job jobs[4];
+  int n_jobs = 0;
+  for (int c = 1; c >= 0; --c)
+    if (tc.n_fused[c]) jobs[n_jobs++] = Job{c, (uint64_t)tc.n_fused[c]};
+  for (int g = 1; g >= 0; --g)
+    if (tc.n_tiles[g]) jobs[n_jobs++] = Job{2 + g, (uint64_t)tc.n_tiles[g] * p.ns_steps * 64};
+  if (n_jobs == 0) return MFSDP_OK;
+  int main_job = 0;
+  for (int j = 1; j < n_jobs; ++j)
+    if (jobs[j].work > jobs[main_job].work) main_job = j;
+  cudaError_t e;
+  if (n_jobs > 1 && (e = cudaEventRecord(tc.fork, st)) != cudaSuccess) return cuda_fail(e);
+  int side_used = 0;
+  for (int j = 0; j < n_jobs; ++j) {
+    cudaStream_t js = st;
+    if (j != main_job) {
+      js = tc.side[side_used];
+      if ((e = cudaStreamWaitEvent(js, tc.fork, 0)) != cudaSuccess) return cuda_fail(e);
+    }
+    int rc = MFSDP_OK;
+    if (jobs[j].kind < 2) {
+      rc = launch_ns_fused(tc, jobs[j].kind, p.ws, p.inv_norm, hp, p.ua, js);
+    } else {
+      const int g = jobs[j].kind - 2;
+      p.tiles = tc.d_tiles[g];
+      p.n_iter_tiles = tc.n_tiles[g];
+      p.counter = tc.d_counters + g;
+      const uint64_t total = (uint64_t)p.n_iter_tiles * p.ns_steps;
+      if (total >= 0xffffffffull) return MFSDP_EINVAL;
+      if (g == 1) e = launch_class<2>(p, (uint32_t)std::min<uint64_t>(total, (uint64_t)tc.max_pairs), js);
+      else e = launch_class<1>(p, (uint32_t)std::min<uint64_t>(total, (uint64_t)tc.sms), js);
+      if (e != cudaSuccess) return cuda_fail(e);
+      ++p.launch_idx;
+      count_launch();
+      rc = check_last_launch();
+    }
     if (rc) return rc;
+    if (j != main_job) {
+      if ((e = cudaEventRecord(tc.join[side_used], js)) != cudaSuccess) return cuda_fail(e);
+      if ((e = cudaStreamWaitEvent(st, tc.join[side_used], 0)) != cudaSuccess) return cuda_fail(e);
+      ++side_used;
+    }
   }
   return MFSDP_OK;
 }

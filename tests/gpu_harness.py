@@ -40,6 +40,7 @@ class Session:
         self.precision = wl.precision if precision is None else precision
         kw = dict(wl.muon)
         kw.update(hp_over or {})
+        kw.setdefault("flags", mf.STEP_KEEP_O)       # the tests read O back after the whole step
         self.hp = mf.MuonHParams(precision=self.precision, **kw)
         self.n_mat_el, self.n_tail_el = mf.mfsdp_flat_elems(self.desc)
         self.tdt = workloads.TORCH_DTYPE[wl.dtype]
@@ -169,6 +170,8 @@ def probe_last_iteration(sess, i, rng, tol):
     where Y is the wide view of X_prev.  Each identity tests one GEMM phase + its fused epilogue."""
     d = sess.mats[i]
     hp = sess.hp
+    if sess.precision == mf.NS_BF16 and mf.mfsdp_ns_class(d.rows, d.cols) == 0:
+        return                 # whole-matrix kernel: A and P never leave the SM (nothing to probe; O is oracle-checked)
     Xp, A, P, Xl = sess.read_ns_buffers(i)
     tall = d.rows > d.cols
     Y = Xp.T if tall else Xp

@@ -29,7 +29,7 @@ def test_library_exports_every_declared_symbol():
 def test_struct_sizes_match_header_layout():
     assert ctypes.sizeof(mf.Param) == 24
     assert ctypes.sizeof(mf.Desc) == 40
-    assert ctypes.sizeof(mf.MuonHParams) == 7 * 8 + 4 * 4
+    assert ctypes.sizeof(mf.MuonHParams) == 7 * 8 + 6 * 4
     assert ctypes.sizeof(mf.AdamWHParams) == 5 * 8 + 8
 
 
@@ -169,7 +169,7 @@ def test_tune_knobs_roundtrip_and_reject_bad_values():
     knobs = [mf.TUNE_PAIR_MIN_D, mf.TUNE_SYM_BAND, mf.TUNE_SYM_BAND2, mf.TUNE_RECT_GROUP, mf.TUNE_WIDE_MIN_KB,
              mf.TUNE_FUSED_BELOW_D]
     old = [mf.mfsdp_get_tune(k) for k in knobs]
-    assert old == [768, 16, 8, 4, 8, 129]         # the header's defaults; no environment variable can change them
+    assert old == [1024, 16, 8, 4, 8, 129]         # the header's defaults; no environment variable can change them
     try:
         for k in knobs:
             mf.mfsdp_tune(k, 3)

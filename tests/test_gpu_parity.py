@@ -28,6 +28,28 @@ def pair_min_d():
     mf.mfsdp_tune(mf.TUNE_PAIR_MIN_D, old)
 
 
+@pytest.fixture
+def fused_below_d():
+    """Sets MFSDP_TUNE_FUSED_BELOW_D for one test (1 = whole-matrix kernel off) and restores the default."""
+    old = mf.mfsdp_get_tune(mf.TUNE_FUSED_BELOW_D)
+
+    def set_(v):
+        mf.mfsdp_tune(mf.TUNE_FUSED_BELOW_D, v)
+    yield set_
+    mf.mfsdp_tune(mf.TUNE_FUSED_BELOW_D, old)
+
+
+def _o_bits(sess):
+    """The bit patterns of every matrix' O = X_K in the workspace (rows x cols; the pitch padding is never written),
+    in table order."""
+    out = []
+    for i, d in enumerate(sess.mats):
+        o_off, pitch, _ = mf.mfsdp_workspace_view(sess.desc, sess.precision, sess.hp.ns_steps, i)
+        es, idt = (2, torch.int16) if sess.precision == mf.NS_BF16 else (4, torch.int32)
+        out.append(sess.ws[o_off:o_off + d.rows * pitch * es].view(idt).reshape(d.rows, pitch)[:, :d.cols].clone())
+    return out
+
+
 def _snapshot(sess):
     W_old = [sess.seg64(sess.W, d) for d in sess.mats]
     M_old = [sess.seg64(sess.M, d) for d in sess.mats]
@@ -183,6 +205,98 @@ def test_edge_shapes(pair_min_d, precision, min_d):
         gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i])
 
 
+@pytest.mark.parametrize("below_d", [129, 65, 1])
+@pytest.mark.parametrize("wname", ["fused", "small", "edge"])
+def test_whole_matrix_class_bf16(fused_below_d, wname, below_d):
+    """The whole-matrix kernel (one CTA keeps X, A, P on chip for all K iterations) on every shape it accepts -- both
+    size classes, tall / wide, ragged d and n, K = 5 and the odd / even buffer choice of K = 2 -- against the oracle;
+    and the same sets with the class narrowed (d < 65) and switched off (everything on the tile kernel)."""
+    fused_below_d(below_d)
+    wl = workloads.get(wname)
+    for K in (5, 2):
+        sess, errs = _full_step_check(wl, precision=mf.NS_BF16, hp_over=dict(ns_steps=K))
+        assert max(errs) <= 3e-2
+    sess.load_grads(1)                                    # a second step on non-zero momentum, same tables
+    W_old, M_old = _snapshot(sess)
+    sess.muon_step()
+    for i in range(len(sess.mats)):
+        gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i])
+
+
+def test_scale_invariance_power_of_two():
+    """O(alpha G) = O(G) for ||alpha U|| >> eps (oracle pin `test_ns_invariances`).  The kernels fold 1/||U|| into
+    iteration 0 and accumulate the Gram matrix of the UNNORMALISED U in fp32, so the invariance holds exactly --
+    bit-identical O -- for power-of-two scalings (include/mfsdp.h "Dynamic range"): 2^40 (|g| ~ 1e9), 2^12, 2^-6.
+    At 2^-40 the norm (~3e-14) is below eps = 1e-7 and the clamp of reading M3 applies, on the GPU as in the oracle:
+    X0 = U / eps, far from orthogonal, compared with the oracle by tolerance."""
+    wl = workloads.get("small")
+    ref = None
+    for shift in (0, 40, 12, -6, -40):
+        sess = gh.Session(wl)
+        sess.load_grads(0)
+        sess.G = (sess.G.float() * 2.0 ** shift).to(sess.G.dtype)
+        sess.hG = sess.G.cpu()
+        W_old, M_old = _snapshot(sess)
+        sess.muon_step()
+        bits = _o_bits(sess)
+        if ref is None or shift == -40:
+            for i in range(len(sess.mats)):
+                gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i])
+            if ref is None:
+                ref = bits
+            else:
+                assert max(float(sess.read_O(i).__abs__().max()) for i in range(len(sess.mats))) < 1e-3
+        else:
+            for a, b in zip(ref, bits):
+                assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("wname,min_d", [("medium", 1), ("medium", 100000), ("c2", 0), ("c3", 0)])
+def test_dependency_protocol_poison_stress(pair_min_d, wname, min_d):
+    """The inter-CTA protocol of the tile kernel (epilogue: TMA stores performed -> fence.proxy.async.global ->
+    red.release.gpu on the matrix' counter; scheduler: ld.acquire.gpu >= need -> publish; consumers: fence.proxy.async
+    before their TMA loads / ld.global.cg of A) checked by poisoning: before every pass the intermediates A, P and the
+    X ping-pong target are filled with NaN patterns, so a tile that read an operand before its producer's stores had
+    landed would pick up NaN (or, from the previous pass, nothing valid) and the result could not be bit-identical to
+    the reference pass.  20 passes, with a competing memory-bound kernel queued on another stream to perturb timing.
+    (compute-sanitizer is closed on this pool -- profiles/r02_sanitizer_closed.md -- so this is the tool-free check.)"""
+    if min_d:
+        pair_min_d(min_d)
+    wl = workloads.get(wname)
+    sess = gh.Session(wl, precision=mf.NS_BF16)
+    sess.load_grads(0)
+    mf.mfsdp_muon_momentum_pass(sess.desc, sess.G, sess.M, sess.ws, sess.hp)
+    torch.cuda.synchronize()
+    offs = [mf.mfsdp_debug_ws_offsets(sess.desc, sess.precision, i) for i in range(len(sess.mats))]
+    x0_keep = [(o[0], d.rows * o[4] * 2) for o, d in zip(offs, sess.mats)]
+    head = min(o[0] for o in offs)                        # ssq / inv_norm / partials live before the first X buffer
+    keep = sess.ws.clone()
+
+    def poison():
+        sess.ws[head:].view(torch.int16).fill_(0x7FC1)       # bf16 quiet NaN in every intermediate
+        for off, n in x0_keep:                            # X~ (the input of the pass) is restored
+            sess.ws[off:off + n].copy_(keep[off:off + n])
+
+    poison()
+    mf.mfsdp_muon_ns_pass(sess.desc, sess.ws, sess.hp)
+    torch.cuda.synchronize()
+    ref = _o_bits(sess)
+    for t in ref:
+        assert torch.isfinite(t.contiguous().view(torch.bfloat16).float()).all()
+    side = torch.cuda.Stream()
+    junk = torch.empty(1 << 27, device="cuda")
+    for rep in range(20):
+        poison()
+        torch.cuda.synchronize()
+        if rep % 2:
+            with torch.cuda.stream(side):
+                junk.add_(1.0)
+        mf.mfsdp_muon_ns_pass(sess.desc, sess.ws, sess.hp)
+        torch.cuda.synchronize()
+        for a, b in zip(ref, _o_bits(sess)):
+            assert torch.equal(a, b), "pass %d differs from the reference pass" % rep
+
+
 def test_empty_and_tail_only_tables_are_no_ops():
     empty = mf.make_desc_array([])
     hp = mf.MuonHParams(precision=mf.NS_BF16, **workloads.get("c1").muon)
@@ -233,16 +347,6 @@ def test_zero_gradient_gives_zero_update_no_nan():
             assert np.all(O == 0.0)
             assert sess.read_ssq(i) == 0.0
         assert torch.isfinite(sess.W.float()).all()
-
-
-def _o_bits(sess):
-    """The bytes of every matrix' O = X_K in the workspace (rows x pitch), in table order."""
-    out = []
-    for i, d in enumerate(sess.mats):
-        o_off, pitch, _ = mf.mfsdp_workspace_view(sess.desc, sess.precision, sess.hp.ns_steps, i)
-        es = 2 if sess.precision == mf.NS_BF16 else 4
-        out.append(sess.ws[o_off:o_off + d.rows * pitch * es].clone())
-    return out
 
 
 @pytest.mark.parametrize("wname,min_d", [("small", 0), ("medium", 0), ("medium", 1), ("medium", 100000), ("c2", 0)])
@@ -302,18 +406,27 @@ def test_paper_setting_parity():
                 assert ulps.max() <= 1 and (ulps > 0).mean() <= 2e-3
 
 
-def test_separate_passes_equal_fused_step():
-    wl = workloads.small_ragged()
-    a = gh.Session(wl)
-    a.load_grads(0)
-    a.muon_step()
+@pytest.mark.parametrize("wname", ["small", "medium", "fused", "c3"])
+def test_separate_passes_equal_fused_step(wname):
+    """mfsdp_muon_step == momentum pass + NS pass + update pass, bit for bit -- also where the step applies the weight
+    update inside the last Newton-Schulz epilogue (bf16 weights, every cols % 8 == 0: medium, c3) instead of running
+    k_update, with and without MFSDP_STEP_KEEP_O."""
+    wl = workloads.get(wname)
     b = gh.Session(wl)
     b.load_grads(0)
     mf.mfsdp_muon_momentum_pass(b.desc, b.G, b.M, b.ws, b.hp)
     mf.mfsdp_muon_ns_pass(b.desc, b.ws, b.hp)
     mf.mfsdp_muon_update_pass(b.desc, b.W, b.ws, b.hp)
     torch.cuda.synchronize()
-    assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M)
+    ref_o = _o_bits(b)
+    for flags in (mf.STEP_KEEP_O, 0):
+        a = gh.Session(wl, hp_over=dict(flags=flags))
+        a.load_grads(0)
+        a.muon_step()
+        assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M)
+        if flags:
+            for x, y in zip(_o_bits(a), ref_o):
+                assert torch.equal(x, y)
 
 
 def test_host_buffer_entry_point():

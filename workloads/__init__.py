@@ -122,6 +122,19 @@ def edge_shapes(seed=13, dtype=BF16, precision=NS_BF16):
     return Workload("edge_shapes", params, seed=seed, precision=precision, dtype=dtype)
 
 
+def fused_shapes(seed=19, dtype=BF16, precision=NS_BF16):
+    """Shapes of the whole-matrix Newton-Schulz class (min(rows, cols) <= 128, padded X <= 128 KB): the largest that
+    fit (128 x 512, 512 x 128), both size classes, d not a multiple of 16 / 64, n not a multiple of 64 / 128, tall and
+    wide twins, and neighbours just outside the class (129 x 200, 128 x 576) that stay on the tile kernel."""
+    shapes = [(128, 512), (512, 128), (64, 512), (512, 64), (100, 300), (300, 100), (128, 128), (16, 16), (127, 129),
+              (33, 500), (500, 33), (128, 448), (65, 257), (257, 65), (96, 192), (1, 200), (200, 1), (129, 200),
+              (128, 576), (72, 256)]
+    params = [(i // 5, 2, r, c, dtype, 0) for i, (r, c) in enumerate(shapes)]
+    params += [(0, 1, 129, 1, dtype, 0)]
+    params.sort(key=lambda p: p[0])
+    return Workload("fused_shapes", params, seed=seed, precision=precision, dtype=dtype, row_lognormal=True)
+
+
 def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
     """The paper's convergence model puts the 50,257 x 768 embedding and the untied LM head on Muon:
     a very tall matrix with an odd row count (GRAM k loop of 786 blocks) next to one ordinary matrix."""
@@ -130,7 +143,7 @@ def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
 
 
 CONFIGS = {"c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
-           "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes,
+           "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes, "fused": fused_shapes,
            "vocab": vocab_embedding}
 
 
