@@ -9,7 +9,10 @@ Follows PAPER.md Algorithm 1 line by line, plain Python ints 
       layouts by block."
   5: "Validate one contiguous local segment per parameter; return one MatrixShard layout
       per block."
-  (4: COSTAWARE needs workspace caps and a scorer the paper never defines -- out of scope.)
+  4: "COSTAWARE: use SCOPEGREEDY only if balance improves within workspace caps; else use
+      ROLEGREEDY."  ("COSTAWARE accepts the scope plan only when the balance gain
+      does not exceed workspace caps.")  The paper defines neither the caps nor the scorer's
+      formulas; reading P5 of DESIGN.md section 4 fixes them (cost_aware / score_plan below).
 
 PAPER.md:65 "The greedy load is owner-resident numel, a proxy for resident parameter/
 gradient bytes and Muon work" -> metric NUMEL.  BASELINE.json configs 4/5 "balances
@@ -27,6 +30,7 @@ ROLE_MATRIX = 0
 ROLE_TAIL = 1
 POLICY_ROLE_GREEDY = 0
 POLICY_SCOPE_GREEDY = 1
+POLICY_COST_AWARE = 2
 METRIC_NUMEL = 0
 METRIC_NS_FLOPS = 1
 PARAM_SKIP = 1
@@ -87,14 +91,120 @@ def _greedy(role_ids, roles, metric, loads, owner):
         loads[vec][lightest] += load
 
 
-def plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0):
-    """Algorithm 1 lines 1-3, 5.  Returns dict(roles, owner, loads, rank, desc)."""
+DTYPE_BYTES = {0: 2, 1: 4}     # BF16, F32 storage
+DEFAULT_CAPS = dict(owner_num=9, owner_den=8, ws_num=9, ws_den=8, abs_owner_bytes=0, abs_ws_bytes=0)
+
+
+def score_plan(params, world_size, owner):
+    """Resource scorer ("the resource scorer expands a completed plan into per-rank parameter, gradient,
+    optimizer-state, communication, and workspace estimates") and the per-block bandwidth model of PAPER.md:77-81.
+    Reading P5 (the paper prints no formulas for the scorer), all integers, bytes:
+      param[r]  = sum over roles owned by r of numel * sizeof(storage dtype)           (resident parameter shard)
+      grad[r]   = param[r]                                                              (gradient of the same roles, same dtype)
+      state[r]  = 4 * numel per owned matrix (fp32 Muon momentum, reading M9) + 8 * numel per owned tail (AdamW m, v)
+      comm[r]   = sum over blocks B of (W - 1) * O_{B,r}     (bytes r sends per materialisation of all blocks = bytes it
+                  receives per gradient reduction; the per-block maximum over r is the paper's C_B^owner)
+      ws[r]     = sum over owned matrices of 2 * (2 * rows * cols + 2 * d * d), d = min(rows, cols)
+                  (the owner-local step's Newton-Schulz workspace: X ping-pong + A + P in bf16, unpadded)
+      blk[r]    = max over blocks of O_{B,r}                 (largest owner segment r must hold unsharded)
+    and per block B, P_B = bytes of all its roles, O_{B,r} = bytes of it owned by r:
+      gamma_B = max_r O_{B,r} / (P_B / W);  C_B^FSDP = P_B (W-1)/W;  C_B^owner = (W-1) max_r O_{B,r}.
+    Returns dict(rank=[dict per rank], block=[dict per block in model order])."""
+    roles = build_roles(params)
+    if len(owner) != len(roles):
+        raise ValueError("owner[] does not match the roles")
+    W = world_size
+    rank = [dict(param=0, grad=0, state=0, comm=0, ws=0, blk=0) for _ in range(W)]
+    blocks = []
+    per_block = {}
+    for r, role in enumerate(roles):
+        o = owner[r]
+        if not 0 <= o < W:
+            raise ValueError("owner out of range")
+        nbytes = role["numel"] * DTYPE_BYTES[role["dtype"]]
+        rank[o]["param"] += nbytes
+        rank[o]["grad"] += nbytes
+        if role["kind"] == ROLE_MATRIX:
+            d = min(role["rows"], role["cols"])
+            rank[o]["state"] += 4 * role["numel"]
+            rank[o]["ws"] += 2 * (2 * role["rows"] * role["cols"] + 2 * d * d)
+        else:
+            rank[o]["state"] += 8 * role["numel"]
+        if role["block"] not in per_block:
+            per_block[role["block"]] = [0] * W
+            blocks.append(role["block"])
+        per_block[role["block"]][o] += nbytes
+    out_blocks = []
+    for b in blocks:
+        O = per_block[b]
+        P_B = sum(O)
+        mx = max(O)
+        for r in range(W):
+            rank[r]["comm"] += (W - 1) * O[r]
+            rank[r]["blk"] = max(rank[r]["blk"], O[r])
+        out_blocks.append(dict(block=b, param=P_B, max_owner=mx, gamma=float(mx * W) / float(P_B),
+                               c_fsdp=float(P_B * (W - 1)) / float(W), c_owner=float((W - 1) * mx)))
+    return dict(rank=rank, block=out_blocks)
+
+
+def cost_aware(params, world_size, metric=METRIC_NUMEL, caps=None):
+    """Algorithm 1 line 4 under reading P5.  Run ROLE-GREEDY and SCOPE-GREEDY; take the scope plan iff
+      (a) balance improves: max primary load (scope) < max primary load (role)  [same total, so max/avg improves], and
+      (b) it stays within the workspace caps, both relative to the memory-conservative role plan and absolute:
+            max_{B,r} O_{B,r}(scope) * owner_den <= owner_num * max_{B,r} O_{B,r}(role)
+            max_r ws[r](scope)       * ws_den    <= ws_num    * max_r ws[r](role)
+            max_{B,r} O_{B,r}(scope) <= abs_owner_bytes   (if non-zero),   max_r ws[r](scope) <= abs_ws_bytes (if non-zero);
+    else the role plan.  Default caps: 9/8 on both ratios, no absolute cap.
+    Returns (policy_used, owner, loads)."""
+    caps = dict(DEFAULT_CAPS, **(caps or {}))
+    role = _assign(params, world_size, POLICY_ROLE_GREEDY, metric)
+    scope = _assign(params, world_size, POLICY_SCOPE_GREEDY, metric)
+    take_scope = max(scope[1][0]) < max(role[1][0])
+    if take_scope:
+        sr = score_plan(params, world_size, role[0])["rank"]
+        ss = score_plan(params, world_size, scope[0])["rank"]
+        blk_r, blk_s = max(x["blk"] for x in sr), max(x["blk"] for x in ss)
+        ws_r, ws_s = max(x["ws"] for x in sr), max(x["ws"] for x in ss)
+        take_scope = (blk_s * caps["owner_den"] <= caps["owner_num"] * blk_r and
+                      ws_s * caps["ws_den"] <= caps["ws_num"] * ws_r and
+                      (caps["abs_owner_bytes"] == 0 or blk_s <= caps["abs_owner_bytes"]) and
+                      (caps["abs_ws_bytes"] == 0 or ws_s <= caps["abs_ws_bytes"]))
+    if take_scope:
+        return POLICY_SCOPE_GREEDY, scope[0], scope[1]
+    return POLICY_ROLE_GREEDY, role[0], role[1]
+
+
+def _assign(params, world_size, policy, metric):
+    """Algorithm 1 lines 1-3: (owner[], loads[2][W]) of ROLE- or SCOPE-GREEDY."""
+    roles = build_roles(params)
+    owner = [-1] * len(roles)
+    loads = [[0] * world_size, [0] * world_size]
+    if policy == POLICY_ROLE_GREEDY:
+        blocks = []
+        for r, role in enumerate(roles):
+            if not blocks or blocks[-1][0] != role["block"]:
+                blocks.append((role["block"], []))
+            blocks[-1][1].append(r)
+        for _, ids in blocks:                      # "per block ... carry loads forward"
+            _greedy(ids, roles, metric, loads, owner)
+    elif policy == POLICY_SCOPE_GREEDY:
+        _greedy(list(range(len(roles))), roles, metric, loads, owner)   # "pool all roles"
+    else:
+        raise ValueError("unknown policy")
+    return owner, loads
+
+
+def plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0, caps=None):
+    """Algorithm 1 lines 1-5.  Returns dict(roles, owner, loads, rank, desc, policy_used)."""
     if world_size < 1:
         raise ValueError("world_size < 1")
     roles = build_roles(params)
     owner = [-1] * len(roles)
     loads = [[0] * world_size, [0] * world_size]
-    if policy == POLICY_ROLE_GREEDY:
+    policy_used = policy
+    if policy == POLICY_COST_AWARE:
+        policy_used, owner, loads = cost_aware(params, world_size, metric, caps)
+    elif policy == POLICY_ROLE_GREEDY:
         blocks = []
         for r, role in enumerate(roles):
             if not blocks or blocks[-1][0] != role["block"]:
@@ -112,7 +222,7 @@ def plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, ran
         raise ValueError("rank out of range")
     desc = emit_desc(roles, owner, rank)
     validate_desc(desc)
-    return dict(roles=roles, owner=owner, loads=loads, rank=rank, desc=desc)
+    return dict(roles=roles, owner=owner, loads=loads, rank=rank, desc=desc, policy_used=policy_used)
 
 
 def _align_up(x, a):

@@ -5,9 +5,11 @@ comparison against the *paper's own* planner stays "parity unpinned" (DESIGN.md 
 import itertools
 import random
 
+import numpy as np
 import pytest
 
 from oracle import planner as P
+from oracle import planner as oplan
 
 
 def mat(block, rows, cols, dtype=1, flags=0):
@@ -164,3 +166,101 @@ def test_transformer_shaped_balance_is_in_the_papers_range():
     for policy in (P.POLICY_ROLE_GREEDY, P.POLICY_SCOPE_GREEDY):
         out = P.plan(params, 8, policy, P.METRIC_NUMEL)
         assert 1.0 <= P.balance(out["loads"][0]) <= 1.4
+
+
+# ---- resource scorer and COSTAWARE (Algorithm 1 line 4; reading P5) ---------------------------
+def test_score_plan_hand_example():
+    """Two blocks, two ranks, bytes by hand.  Block 0: 4x8 bf16 (64 B) on rank 0, 8x2 fp32 (64 B) on rank 1, a tail of
+    10 bf16 (20 B) on rank 0; block 1: 16x16 bf16 (512 B) on rank 1."""
+    params = [(0, 2, 4, 8, 0, 0), (0, 2, 8, 2, 1, 0), (0, 1, 10, 1, 0, 0), (1, 2, 16, 16, 0, 0)]
+    sc = oplan.score_plan(params, 2, [0, 1, 0, 1])
+    r0, r1 = sc["rank"]
+    assert (r0["param"], r1["param"]) == (84, 576) and (r0["grad"], r1["grad"]) == (84, 576)
+    assert (r0["state"], r1["state"]) == (4 * 32 + 8 * 10, 4 * 16 + 4 * 256)
+    assert (r0["ws"], r1["ws"]) == (2 * (2 * 32 + 2 * 16), 2 * (2 * 16 + 2 * 4) + 2 * (2 * 256 + 2 * 256))
+    assert (r0["comm"], r1["comm"]) == (84, 64 + 512) and (r0["blk"], r1["blk"]) == (84, 512)
+    b0, b1 = sc["block"]
+    assert (b0["param"], b0["max_owner"]) == (148, 84) and (b1["param"], b1["max_owner"]) == (512, 512)
+    assert b0["gamma"] == pytest.approx(84 * 2 / 148, rel=1e-15) and b0["c_fsdp"] == 74.0 and b0["c_owner"] == 84.0
+    assert b1["gamma"] == 2.0 and b1["c_fsdp"] == 256.0 and b1["c_owner"] == 512.0
+
+
+def test_bandwidth_model_closed_forms():
+    """"a block with one large owner can be bandwidth-poor (gamma_B ~ W); when the planner spreads matrix and
+    tail owners within the block (gamma_B ~ 1), the leading bandwidth term matches ordinary FSDP", and the second
+    equality of PAPER.md:79: C_B^owner = gamma_B P_B (W-1)/W."""
+    for W in (2, 8, 64):
+        one = oplan.score_plan([(0, 2, 32, 32, 0, 0)], W, [W - 1])["block"][0]
+        assert one["gamma"] == float(W) and one["c_owner"] == float((W - 1) * 32 * 32 * 2)
+        spread = oplan.score_plan([(0, 2, 8, 8, 0, 0)] * W, W, list(range(W)))["block"][0]
+        assert spread["gamma"] == 1.0 and spread["c_owner"] == spread["c_fsdp"]
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        W = int(rng.integers(1, 9))
+        params = [(int(b), 2, int(rng.integers(1, 30)), int(rng.integers(1, 30)), int(rng.integers(0, 2)), 0)
+                  for b in sorted(rng.integers(0, 4, size=int(rng.integers(1, 12))))]
+        owner = [int(rng.integers(0, W)) for _ in params]
+        sc = oplan.score_plan(params, W, owner)
+        total = sum(r * c * (2, 4)[dt] for (_, _, r, c, dt, _) in params)
+        assert sum(x["param"] for x in sc["rank"]) == total == sum(b["param"] for b in sc["block"])
+        assert sum(x["comm"] for x in sc["rank"]) == (W - 1) * total
+        for b in sc["block"]:
+            assert b["c_owner"] == pytest.approx(b["gamma"] * b["c_fsdp"], rel=1e-12) or W == 1
+            assert 1.0 - 1e-12 <= b["gamma"] <= W + 1e-12
+        for r in range(W):
+            assert sc["rank"][r]["blk"] == max([0] + [sum(rr * cc * (2, 4)[dt] for (bb, _, rr, cc, dt, _), o in
+                                                         zip(params, owner) if o == r and bb == b)
+                                                     for b in {p[0] for p in params}])
+
+
+def test_cost_aware_hand_traces():
+    """Algorithm 1 line 4 (reading P5), world 2, numel metric, bf16 column vectors.
+    A: block 0 = {2, 6 elements}, block 1 = {7}.  ROLE: 6 -> r0, 2 -> r1 | 7 -> r1 (lightest): loads (6, 9).  SCOPE:
+       7 -> r0, 6 -> r1, 2 -> r1: loads (7, 8) -- flatter, but rank 1 now owns 4 + 12 = 16 B of block 0 against a largest
+       owner segment of 14 B under ROLE: 16 * 8 > 9 * 14, the cap is exceeded -> ROLE is used.
+    B: block 0 = {2, 4}, block 1 = {8}.  ROLE loads (4, 10), SCOPE (8, 6); the largest owner segment is 16 B either way
+       and the step workspace falls (48 -> 36 B) -> SCOPE is used."""
+    A = [(0, 2, 2, 1, 0, 0), (0, 2, 6, 1, 0, 0), (1, 2, 7, 1, 0, 0)]
+    used, owner, loads = oplan.cost_aware(A, 2)
+    assert used == oplan.POLICY_ROLE_GREEDY and owner == [1, 0, 1] and loads[0] == [6, 9]
+    assert oplan.plan(A, 2, oplan.POLICY_SCOPE_GREEDY)["owner"] == [1, 1, 0]
+    used, owner, loads = oplan.cost_aware(A, 2, caps=dict(owner_num=8, owner_den=7))       # 16 * 7 <= 8 * 14: allowed
+    assert used == oplan.POLICY_SCOPE_GREEDY and owner == [1, 1, 0] and loads[0] == [7, 8]
+    used, _, _ = oplan.cost_aware(A, 2, caps=dict(owner_num=8, owner_den=7, abs_owner_bytes=15))
+    assert used == oplan.POLICY_ROLE_GREEDY                                                  # absolute cap 15 B < 16 B
+    B = [(0, 2, 2, 1, 0, 0), (0, 2, 4, 1, 0, 0), (1, 2, 8, 1, 0, 0)]
+    used, owner, loads = oplan.cost_aware(B, 2)
+    assert used == oplan.POLICY_SCOPE_GREEDY and owner == [1, 1, 0] and loads[0] == [8, 6]
+    used, _, _ = oplan.cost_aware(B, 2, caps=dict(abs_ws_bytes=35))                        # scope needs 36 B
+    assert used == oplan.POLICY_ROLE_GREEDY
+    p = oplan.plan(B, 2, oplan.POLICY_COST_AWARE, rank=1)
+    assert p["policy_used"] == oplan.POLICY_SCOPE_GREEDY and [d["rows"] for d in p["desc"]] == [2, 4]
+
+
+def test_cost_aware_is_one_of_the_two_plans_and_never_worse_balanced_than_role():
+    rng = np.random.default_rng(9)
+    for _ in range(60):
+        W = int(rng.integers(1, 7))
+        params = []
+        for b in range(int(rng.integers(1, 5))):
+            for _ in range(int(rng.integers(1, 6))):
+                if rng.random() < 0.7:
+                    params.append((b, 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)), 0, 0))
+                else:
+                    params.append((b, 1, int(rng.integers(1, 200)), 1, 0, 0))
+        for metric in (oplan.METRIC_NUMEL, oplan.METRIC_NS_FLOPS):
+            role = oplan.plan(params, W, oplan.POLICY_ROLE_GREEDY, metric)
+            scope = oplan.plan(params, W, oplan.POLICY_SCOPE_GREEDY, metric)
+            cost = oplan.plan(params, W, oplan.POLICY_COST_AWARE, metric)
+            assert cost["owner"] in (role["owner"], scope["owner"])
+            assert max(cost["loads"][0]) <= max(role["loads"][0])
+
+
+def test_llama_balance_ratios_in_the_papers_range():
+    """Context, not a pin (different model): Table 5 (PAPER.md:215-222) reports r/s/c = 1.07/1.02/1.07 ... 1.27/1.04/1.27;
+    on the Llama-3-8B shapes the three policies land in the same range, scope flattest, cost = role or scope."""
+    import workloads
+    wl = workloads.get("c4")
+    for W in (8, 64):
+        bal = [oplan.balance(oplan.plan(wl.params, W, pol, wl.metric)["loads"][0]) for pol in (0, 1, 2)]
+        assert 1.0 <= bal[1] <= bal[2] <= bal[0] <= 1.4
