@@ -45,7 +45,8 @@ extern "C" {
 enum { MFSDP_BF16 = 0, MFSDP_F32 = 1 };                       /* storage dtype of W / G (tails: P / G)            */
 enum { MFSDP_ROLE_MATRIX = 0, MFSDP_ROLE_TAIL = 1 };          /* PAPER.md:103 Alg. 1 line 1                       */
 enum { MFSDP_POLICY_ROLE_GREEDY = 0,                          /* PAPER.md:104 Alg. 1 line 2                       */
-       MFSDP_POLICY_SCOPE_GREEDY = 1 };                       /* PAPER.md:105 Alg. 1 line 3                       */
+       MFSDP_POLICY_SCOPE_GREEDY = 1,                         /* PAPER.md:105 Alg. 1 line 3                       */
+       MFSDP_POLICY_COST_AWARE = 2 };                         /* PAPER.md:106 Alg. 1 line 4 (mfsdp_plan_ex)       */
 enum { MFSDP_METRIC_NUMEL = 0,                                /* PAPER.md:65 "greedy load is owner-resident numel" */
        MFSDP_METRIC_NS_FLOPS = 1 };                           /* BASELINE.json C4/C5: m^2 (2n + m), m=min n=max    */
 enum { MFSDP_SCALE_MATCH_RMS_ADAMW = 0,                       /* 0.2 sqrt(max(rows, cols))       */
@@ -110,7 +111,7 @@ typedef struct {
 } mfsdp_adamw_hparams_t;
 
 /* ---- planner (HOST only, no CUDA) -----------------------------------------------------------------------------
- * Algorithm 1, lines 1-3 and 5.  Roles are built from params[] (line 1), assigned greedily
+ * Algorithm 1, lines 1-5.  Roles are built from params[] (line 1), assigned greedily
  * ("largest roles to the currently lightest ranks", ties: load desc, block asc, parameter index asc; lightest rank
  * ties -> lowest rank id), and the resident set of `rank` (rank < 0: the heaviest rank by primary load, ties ->
  * lowest id) is emitted as a descriptor table in (block, parameter) order and validated (line 5: one contiguous,
@@ -129,6 +130,55 @@ typedef struct {
 int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int world_size, int policy, int metric, int rank,
                int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
                mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out);
+
+/* Algorithm 1 line 4 ("COSTAWARE: use SCOPEGREEDY only if balance improves within workspace caps; else
+ * use ROLEGREEDY").  The paper defines neither the caps nor the scorer; reading P5: the scope plan
+ * is taken iff (a) its maximum primary load is strictly below the role plan's and (b), with O_{B,r} = bytes of block B
+ * owned by rank r and ws[r] = the step-workspace estimate of mfsdp_score_plan,
+ *   max_{B,r} O_{B,r}(scope) * owner_den <= owner_num * max_{B,r} O_{B,r}(role),
+ *   max_r ws[r](scope) * ws_den <= ws_num * max_r ws[r](role),
+ *   max_{B,r} O_{B,r}(scope) <= abs_owner_bytes and max_r ws[r](scope) <= abs_ws_bytes where those are non-zero. */
+typedef struct {
+  uint32_t owner_num, owner_den;     /* default 9 / 8 */
+  uint32_t ws_num, ws_den;           /* default 9 / 8 */
+  uint64_t abs_owner_bytes;          /* 0 = no absolute cap */
+  uint64_t abs_ws_bytes;             /* 0 = no absolute cap */
+} mfsdp_caps_t;
+
+/* mfsdp_plan with the caps of MFSDP_POLICY_COST_AWARE (caps == NULL: the defaults; ignored by the other policies) and
+ * the policy actually used (*policy_used, may be NULL: ROLE_GREEDY or SCOPE_GREEDY).  mfsdp_plan(policy = COST_AWARE)
+ * is this call with caps == NULL.  MFSDP_EINVAL additionally for a zero denominator. */
+int mfsdp_plan_ex(const mfsdp_param_t* params, size_t n_params, int world_size, int policy, int metric, int rank,
+                  const mfsdp_caps_t* caps, int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
+                  mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out, int* policy_used);
+
+/* Resource scorer ("expands a completed plan into per-rank parameter, gradient, optimizer-state,
+ * communication, and workspace estimates") and the per-block bandwidth model of PAPER.md:77-81 (HOST, integers; the
+ * formulas are DESIGN.md reading P5 -- the paper prints none):
+ *   param_bytes[r]  sum over roles owned by r of numel * sizeof(dtype);   grad_bytes[r] = param_bytes[r];
+ *   state_bytes[r]  4 * numel per owned matrix (fp32 Muon momentum) + 8 * numel per owned tail (AdamW m, v);
+ *   comm_bytes[r]   sum over blocks of (W - 1) * O_{B,r}  (sent per materialisation pass = received per gradient
+ *                   reduction pass; its per-block maximum over r is C_B^owner);
+ *   workspace_bytes[r]  sum over owned matrices of 2 * (2 rows cols + 2 d^2): X ping-pong + A + P in bf16, unpadded
+ *                   (mfsdp_workspace_bytes of the rank's table is this plus alignment padding and the norm scratch);
+ *   max_block_owner_bytes[r] = max_B O_{B,r}: the largest owner segment r holds unsharded.
+ * Per block B in model order: P_B, max_r O_{B,r}, gamma_B = max_r O_{B,r} / (P_B / W), C_B^FSDP = P_B (W-1)/W,
+ * C_B^owner = (W-1) max_r O_{B,r} = gamma_B C_B^FSDP.
+ *   owner, n_roles   HOST in.  owner rank per role as returned by mfsdp_plan (n_roles must match the roles of params).
+ *   rank_out         HOST out. [world_size]; may be NULL.
+ *   block_out, block_cap, n_blocks  HOST out. per-block records; block_out == NULL: only *n_blocks is written.
+ * Returns MFSDP_EINVAL (bad params / owner out of range / n_roles mismatch), MFSDP_ECAP (block_cap too small). */
+typedef struct {
+  uint64_t param_bytes, grad_bytes, state_bytes, comm_bytes, workspace_bytes, max_block_owner_bytes;
+} mfsdp_rank_score_t;
+typedef struct {
+  uint32_t block_id, reserved;
+  uint64_t param_bytes;              /* P_B */
+  uint64_t max_owner_bytes;          /* max_r O_{B,r} */
+  double gamma, c_fsdp, c_owner;
+} mfsdp_block_score_t;
+int mfsdp_score_plan(const mfsdp_param_t* params, size_t n_params, int world_size, const int32_t* owner, size_t n_roles,
+                     mfsdp_rank_score_t* rank_out, mfsdp_block_score_t* block_out, size_t block_cap, size_t* n_blocks);
 
 /* Validate a descriptor table against PAPER.md:71 / Alg. 1 line 5 (HOST).  0 or MFSDP_ELAYOUT / MFSDP_EINVAL. */
 int mfsdp_validate_desc(const mfsdp_desc_t* desc, size_t n_desc);

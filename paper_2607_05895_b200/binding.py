@@ -7,7 +7,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 
 BF16, F32 = 0, 1
 ROLE_MATRIX, ROLE_TAIL = 0, 1
-POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY = 0, 1
+POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY, POLICY_COST_AWARE = 0, 1, 2
 METRIC_NUMEL, METRIC_NS_FLOPS = 0, 1
 SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE = 0, 1, 2
 NS_BF16, NS_FP32 = 0, 1
@@ -50,6 +50,24 @@ class AdamWHParams(C.Structure):     # mfsdp_adamw_hparams_t
         super().__init__(lr, beta1, beta2, eps, weight_decay, step)
 
 
+class Caps(C.Structure):             # mfsdp_caps_t
+    _fields_ = [("owner_num", C.c_uint32), ("owner_den", C.c_uint32), ("ws_num", C.c_uint32), ("ws_den", C.c_uint32),
+                ("abs_owner_bytes", C.c_uint64), ("abs_ws_bytes", C.c_uint64)]
+
+    def __init__(self, owner_num=9, owner_den=8, ws_num=9, ws_den=8, abs_owner_bytes=0, abs_ws_bytes=0):
+        super().__init__(owner_num, owner_den, ws_num, ws_den, abs_owner_bytes, abs_ws_bytes)
+
+
+class RankScore(C.Structure):        # mfsdp_rank_score_t
+    _fields_ = [(n, C.c_uint64) for n in ("param_bytes", "grad_bytes", "state_bytes", "comm_bytes", "workspace_bytes",
+                                          "max_block_owner_bytes")]
+
+
+class BlockScore(C.Structure):       # mfsdp_block_score_t
+    _fields_ = [("block_id", C.c_uint32), ("reserved", C.c_uint32), ("param_bytes", C.c_uint64),
+                ("max_owner_bytes", C.c_uint64), ("gamma", C.c_double), ("c_fsdp", C.c_double), ("c_owner", C.c_double)]
+
+
 class MfsdpError(RuntimeError):
     def __init__(self, code, what):
         self.code = code
@@ -63,9 +81,10 @@ class PlanResult:
     rank_load: list      # [2 * world]: primary loads then tail loads
     desc: object         # ctypes array of Desc (the chosen rank's resident set)
     rank: int
+    policy_used: int = -1
 
 
-_SYMBOLS = ["mfsdp_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
+_SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
             "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
@@ -96,6 +115,10 @@ def load():
     psz = C.POINTER(C.c_size_t)
     lib.mfsdp_plan.argtypes = [pP, sz, i32, i32, i32, i32, C.POINTER(C.c_int32), psz, C.POINTER(C.c_uint64), pD, sz,
                                psz, C.POINTER(C.c_int)]
+    lib.mfsdp_plan_ex.argtypes = [pP, sz, i32, i32, i32, i32, C.POINTER(Caps), C.POINTER(C.c_int32), psz,
+                                  C.POINTER(C.c_uint64), pD, sz, psz, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    lib.mfsdp_score_plan.argtypes = [pP, sz, i32, C.POINTER(C.c_int32), sz, C.POINTER(RankScore), C.POINTER(BlockScore),
+                                     sz, psz]
     lib.mfsdp_validate_desc.argtypes = [pD, sz]
     lib.mfsdp_flat_elems.argtypes = [pD, sz, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.mfsdp_workspace_bytes.argtypes = [pD, sz, i32, psz]
@@ -218,13 +241,39 @@ def mfsdp_get_tune(knob):
     return v
 
 
-def mfsdp_plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0):
-    """params: list of (block_id, ndim, rows, cols, dtype, flags) tuples or Param.  Returns PlanResult."""
-    lib = load()
+def _param_array(params):
     n = len(params)
     arr = (Param * max(1, n))()
     for i, p in enumerate(params):
         arr[i] = p if isinstance(p, Param) else Param(*p)
+    return arr, n
+
+
+def mfsdp_plan_ex(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0, caps=None):
+    """params: list of (block_id, ndim, rows, cols, dtype, flags) tuples or Param; caps: Caps or None (defaults).
+    Returns PlanResult (policy_used = ROLE_GREEDY / SCOPE_GREEDY actually taken)."""
+    lib = load()
+    arr, n = _param_array(params)
+    cp = C.byref(caps) if caps is not None else None
+    n_roles, n_desc, rank_out, used = C.c_size_t(0), C.c_size_t(0), C.c_int(0), C.c_int(0)
+    rc = lib.mfsdp_plan_ex(arr, n, world_size, policy, metric, rank, cp, None, C.byref(n_roles), None, None, 0,
+                           C.byref(n_desc), C.byref(rank_out), C.byref(used))
+    _check(rc, "mfsdp_plan_ex(size query)")
+    owner = (C.c_int32 * max(1, n_roles.value))()
+    loads = (C.c_uint64 * (2 * world_size))()
+    desc = (Desc * max(1, n_desc.value))()
+    cap = n_desc.value
+    rc = lib.mfsdp_plan_ex(arr, n, world_size, policy, metric, rank, cp, owner, C.byref(n_roles), loads, desc, cap,
+                           C.byref(n_desc), C.byref(rank_out), C.byref(used))
+    _check(rc, "mfsdp_plan_ex")
+    desc._n = n_desc.value
+    return PlanResult(list(owner[:n_roles.value]), n_roles.value, list(loads), desc, rank_out.value, used.value)
+
+
+def mfsdp_plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUMEL, rank=0):
+    """params: list of (block_id, ndim, rows, cols, dtype, flags) tuples or Param.  Returns PlanResult."""
+    lib = load()
+    arr, n = _param_array(params)
     n_roles, n_desc, rank_out = C.c_size_t(0), C.c_size_t(0), C.c_int(0)
     rc = lib.mfsdp_plan(arr, n, world_size, policy, metric, rank, None, C.byref(n_roles), None, None, 0,
                         C.byref(n_desc), C.byref(rank_out))
@@ -238,6 +287,20 @@ def mfsdp_plan(params, world_size, policy=POLICY_ROLE_GREEDY, metric=METRIC_NUME
     _check(rc, "mfsdp_plan")
     desc._n = n_desc.value
     return PlanResult(list(owner[:n_roles.value]), n_roles.value, list(loads), desc, rank_out.value)
+
+
+def mfsdp_score_plan(params, world_size, owner):
+    """(list of RankScore per rank, list of BlockScore per block in model order) of a completed plan."""
+    lib = load()
+    arr, n = _param_array(params)
+    own = (C.c_int32 * max(1, len(owner)))(*owner)
+    nb = C.c_size_t(0)
+    _check(lib.mfsdp_score_plan(arr, n, world_size, own, len(owner), None, None, 0, C.byref(nb)), "mfsdp_score_plan(size)")
+    ranks = (RankScore * world_size)()
+    blocks = (BlockScore * max(1, nb.value))()
+    _check(lib.mfsdp_score_plan(arr, n, world_size, own, len(owner), ranks, blocks, nb.value, C.byref(nb)),
+           "mfsdp_score_plan")
+    return list(ranks), list(blocks[:nb.value])
 
 
 def mfsdp_validate_desc(desc):

@@ -114,19 +114,14 @@ extern "C" int mfsdp_flat_elems(const mfsdp_desc_t* d, size_t n, uint64_t* mat, 
   return MFSDP_OK;
 }
 
-extern "C" int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int world, int policy, int metric,
-                          int rank, int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
-                          mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out) {
-  if ((n_params && !params) || world < 1 || rank >= world || !n_desc) return MFSDP_EINVAL;
-  if (policy != MFSDP_POLICY_ROLE_GREEDY && policy != MFSDP_POLICY_SCOPE_GREEDY) return MFSDP_EINVAL;
-  if (metric != MFSDP_METRIC_NUMEL && metric != MFSDP_METRIC_NS_FLOPS) return MFSDP_EINVAL;
+namespace {
 
-  std::vector<Role> roles;
-  int rc = build_roles(params, n_params, roles);
-  if (rc) return rc;
-
-  std::vector<int32_t> owner(roles.size(), -1);
-  std::vector<uint64_t> loads[2] = {std::vector<uint64_t>((size_t)world, 0), std::vector<uint64_t>((size_t)world, 0)};
+// Algorithm 1 lines 2-3: owner[] and the two load vectors of ROLE- or SCOPE-GREEDY.
+void assign(const std::vector<Role>& roles, int world, int policy, int metric, std::vector<int32_t>& owner,
+            std::vector<uint64_t>* loads) {
+  owner.assign(roles.size(), -1);
+  loads[0].assign((size_t)world, 0);
+  loads[1].assign((size_t)world, 0);
   std::vector<uint32_t> ids;
   if (policy == MFSDP_POLICY_ROLE_GREEDY) {           // line 2: per block, carry loads forward
     size_t i = 0;
@@ -140,6 +135,122 @@ extern "C" int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int worl
     ids.resize(roles.size());
     for (size_t i = 0; i < roles.size(); ++i) ids[i] = (uint32_t)i;
     greedy(ids, roles, metric, world, loads, owner);
+  }
+}
+
+inline uint64_t dtype_bytes(uint32_t dtype) { return dtype == MFSDP_BF16 ? 2 : 4; }
+
+// Resource scorer (reading P5): per-rank and per-block records of a completed plan.
+void score(const std::vector<Role>& roles, const std::vector<int32_t>& owner, int world,
+           std::vector<mfsdp_rank_score_t>& rank, std::vector<mfsdp_block_score_t>& blocks) {
+  mfsdp_rank_score_t zero;
+  std::memset(&zero, 0, sizeof zero);
+  rank.assign((size_t)world, zero);
+  blocks.clear();
+  std::vector<uint64_t> O((size_t)world);
+  size_t i = 0;
+  while (i < roles.size()) {                          // roles are in model order: one run per block
+    const uint32_t blk = roles[i].block;
+    std::fill(O.begin(), O.end(), 0);
+    for (; i < roles.size() && roles[i].block == blk; ++i) {
+      const Role& r = roles[i];
+      const size_t o = (size_t)owner[i];
+      const uint64_t nbytes = r.numel * dtype_bytes(r.dtype);
+      rank[o].param_bytes += nbytes;
+      rank[o].grad_bytes += nbytes;
+      if (r.kind == MFSDP_ROLE_MATRIX) {
+        const uint64_t d = std::min(r.rows, r.cols);
+        rank[o].state_bytes += 4 * r.numel;
+        rank[o].workspace_bytes += 2 * (2 * (uint64_t)r.rows * r.cols + 2 * d * d);
+      } else {
+        rank[o].state_bytes += 8 * r.numel;
+      }
+      O[o] += nbytes;
+    }
+    uint64_t P = 0, mx = 0;
+    for (int r = 0; r < world; ++r) {
+      P += O[(size_t)r];
+      mx = std::max(mx, O[(size_t)r]);
+      rank[(size_t)r].comm_bytes += (uint64_t)(world - 1) * O[(size_t)r];
+      rank[(size_t)r].max_block_owner_bytes = std::max(rank[(size_t)r].max_block_owner_bytes, O[(size_t)r]);
+    }
+    mfsdp_block_score_t b;
+    std::memset(&b, 0, sizeof b);
+    b.block_id = blk; b.param_bytes = P; b.max_owner_bytes = mx;
+    b.gamma = (double)(mx * (uint64_t)world) / (double)P;
+    b.c_fsdp = (double)(P * (uint64_t)(world - 1)) / (double)world;
+    b.c_owner = (double)((uint64_t)(world - 1) * mx);
+    blocks.push_back(b);
+  }
+}
+
+}  // namespace
+
+extern "C" int mfsdp_score_plan(const mfsdp_param_t* params, size_t n_params, int world, const int32_t* owner,
+                                size_t n_roles, mfsdp_rank_score_t* rank_out, mfsdp_block_score_t* block_out,
+                                size_t block_cap, size_t* n_blocks) {
+  if ((n_params && !params) || world < 1 || (n_roles && !owner)) return MFSDP_EINVAL;
+  std::vector<Role> roles;
+  const int rc = build_roles(params, n_params, roles);
+  if (rc) return rc;
+  if (roles.size() != n_roles) return MFSDP_EINVAL;
+  std::vector<int32_t> own(owner, owner + n_roles);
+  for (int32_t o : own) if (o < 0 || o >= world) return MFSDP_EINVAL;
+  std::vector<mfsdp_rank_score_t> rank;
+  std::vector<mfsdp_block_score_t> blocks;
+  score(roles, own, world, rank, blocks);
+  if (n_blocks) *n_blocks = blocks.size();
+  if (rank_out) std::memcpy(rank_out, rank.data(), rank.size() * sizeof(mfsdp_rank_score_t));
+  if (block_out) {
+    if (block_cap < blocks.size()) return MFSDP_ECAP;
+    if (!blocks.empty()) std::memcpy(block_out, blocks.data(), blocks.size() * sizeof(mfsdp_block_score_t));
+  }
+  return MFSDP_OK;
+}
+
+extern "C" int mfsdp_plan_ex(const mfsdp_param_t* params, size_t n_params, int world, int policy, int metric, int rank,
+                             const mfsdp_caps_t* caps, int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
+                             mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out, int* policy_used) {
+  if ((n_params && !params) || world < 1 || rank >= world || !n_desc) return MFSDP_EINVAL;
+  if (policy != MFSDP_POLICY_ROLE_GREEDY && policy != MFSDP_POLICY_SCOPE_GREEDY && policy != MFSDP_POLICY_COST_AWARE)
+    return MFSDP_EINVAL;
+  if (metric != MFSDP_METRIC_NUMEL && metric != MFSDP_METRIC_NS_FLOPS) return MFSDP_EINVAL;
+  mfsdp_caps_t cp = {9, 8, 9, 8, 0, 0};
+  if (caps) cp = *caps;
+  if (policy == MFSDP_POLICY_COST_AWARE && (cp.owner_den == 0 || cp.ws_den == 0)) return MFSDP_EINVAL;
+
+  std::vector<Role> roles;
+  int rc = build_roles(params, n_params, roles);
+  if (rc) return rc;
+
+  std::vector<int32_t> owner;
+  std::vector<uint64_t> loads[2];
+  int used = policy;
+  if (policy == MFSDP_POLICY_COST_AWARE) {            // line 4: scope only if balance improves within the caps
+    std::vector<int32_t> owner_s;
+    std::vector<uint64_t> loads_s[2];
+    assign(roles, world, MFSDP_POLICY_ROLE_GREEDY, metric, owner, loads);
+    assign(roles, world, MFSDP_POLICY_SCOPE_GREEDY, metric, owner_s, loads_s);
+    auto vmax = [](const std::vector<uint64_t>& v) { uint64_t m = 0; for (uint64_t x : v) m = std::max(m, x); return m; };
+    bool take = vmax(loads_s[0]) < vmax(loads[0]);
+    if (take) {
+      std::vector<mfsdp_rank_score_t> sr, ss;
+      std::vector<mfsdp_block_score_t> tmp;
+      score(roles, owner, world, sr, tmp);
+      score(roles, owner_s, world, ss, tmp);
+      uint64_t blk_r = 0, blk_s = 0, ws_r = 0, ws_s = 0;
+      for (int r = 0; r < world; ++r) {
+        blk_r = std::max(blk_r, sr[(size_t)r].max_block_owner_bytes); blk_s = std::max(blk_s, ss[(size_t)r].max_block_owner_bytes);
+        ws_r = std::max(ws_r, sr[(size_t)r].workspace_bytes); ws_s = std::max(ws_s, ss[(size_t)r].workspace_bytes);
+      }
+      typedef unsigned __int128 u128;                 // bytes * small integers: no overflow worries
+      take = (u128)blk_s * cp.owner_den <= (u128)cp.owner_num * blk_r && (u128)ws_s * cp.ws_den <= (u128)cp.ws_num * ws_r &&
+             (cp.abs_owner_bytes == 0 || blk_s <= cp.abs_owner_bytes) && (cp.abs_ws_bytes == 0 || ws_s <= cp.abs_ws_bytes);
+    }
+    used = take ? MFSDP_POLICY_SCOPE_GREEDY : MFSDP_POLICY_ROLE_GREEDY;
+    if (take) { owner.swap(owner_s); loads[0].swap(loads_s[0]); loads[1].swap(loads_s[1]); }
+  } else {
+    assign(roles, world, policy, metric, owner, loads);
   }
 
   if (rank < 0) {                                     // P6: heaviest by primary load, ties -> lowest id
@@ -167,6 +278,7 @@ extern "C" int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int worl
 
   if (n_roles) *n_roles = roles.size();
   if (rank_out) *rank_out = rank;
+  if (policy_used) *policy_used = used;
   if (owner_out) for (size_t i = 0; i < roles.size(); ++i) owner_out[i] = owner[i];
   if (rank_load_out)
     for (int r = 0; r < world; ++r) { rank_load_out[r] = loads[0][r]; rank_load_out[world + r] = loads[1][r]; }
@@ -176,4 +288,11 @@ extern "C" int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int worl
     if (!out.empty()) std::memcpy(desc_out, out.data(), out.size() * sizeof(mfsdp_desc_t));
   }
   return MFSDP_OK;
+}
+
+extern "C" int mfsdp_plan(const mfsdp_param_t* params, size_t n_params, int world, int policy, int metric,
+                          int rank, int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
+                          mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out) {
+  return mfsdp_plan_ex(params, n_params, world, policy, metric, rank, nullptr, owner_out, n_roles, rank_load_out,
+                       desc_out, desc_cap, n_desc, rank_out, nullptr);
 }

@@ -33,9 +33,15 @@ def test_struct_sizes_match_header_layout():
     assert ctypes.sizeof(mf.AdamWHParams) == 5 * 8 + 8
 
 
-def _compare_plan(params, world, policy, metric, rank):
-    want = oplan.plan(params, world, policy, metric, rank)
-    got = mf.mfsdp_plan(params, world, policy, metric, rank)
+def _compare_plan(params, world, policy, metric, rank, caps=None):
+    want = oplan.plan(params, world, policy, metric, rank, caps=caps)
+    if caps is None:
+        got = mf.mfsdp_plan(params, world, policy, metric, rank)
+        got_ex = mf.mfsdp_plan_ex(params, world, policy, metric, rank)
+        assert got_ex.owner == got.owner and got_ex.policy_used == want["policy_used"]
+    else:
+        got = mf.mfsdp_plan_ex(params, world, policy, metric, rank, mf.Caps(**caps))
+        assert got.policy_used == want["policy_used"]
     assert got.n_roles == len(want["roles"])
     assert got.owner == want["owner"]
     assert got.rank == want["rank"]
@@ -47,7 +53,7 @@ def _compare_plan(params, world, policy, metric, rank):
 
 
 @pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4", "c5", "small"])
-@pytest.mark.parametrize("policy", [mf.POLICY_ROLE_GREEDY, mf.POLICY_SCOPE_GREEDY])
+@pytest.mark.parametrize("policy", [mf.POLICY_ROLE_GREEDY, mf.POLICY_SCOPE_GREEDY, mf.POLICY_COST_AWARE])
 @pytest.mark.parametrize("metric", [mf.METRIC_NUMEL, mf.METRIC_NS_FLOPS])
 def test_planner_matches_oracle_bit_exact_on_configs(name, policy, metric):
     wl = workloads.get(name)
@@ -68,10 +74,83 @@ def test_planner_matches_oracle_on_random_models():
                 else:
                     params.append((b, 1, int(rng.integers(1, 300)), 1, 0, int(rng.random() < 0.1)))
         world = int(rng.integers(1, 7))
-        policy = int(rng.integers(0, 2))
+        policy = int(rng.integers(0, 3))
         metric = int(rng.integers(0, 2))
         rank = int(rng.integers(-1, world))
         _compare_plan(params, world, policy, metric, rank)
+        if policy == mf.POLICY_COST_AWARE and trial % 2:
+            caps = dict(owner_num=int(rng.integers(1, 5)), owner_den=int(rng.integers(1, 5)),
+                        ws_num=int(rng.integers(1, 5)), ws_den=int(rng.integers(1, 5)),
+                        abs_owner_bytes=int(rng.integers(0, 3)) * int(rng.integers(1, 4000)),
+                        abs_ws_bytes=int(rng.integers(0, 3)) * int(rng.integers(1, 8000)))
+            _compare_plan(params, world, policy, metric, rank, caps=caps)
+
+
+def _compare_score(params, world, owner):
+    want = oplan.score_plan(params, world, owner)
+    ranks, blocks = mf.mfsdp_score_plan(params, world, owner)
+    assert len(ranks) == world and len(blocks) == len(want["block"])
+    for g, w in zip(ranks, want["rank"]):
+        assert (g.param_bytes, g.grad_bytes, g.state_bytes, g.comm_bytes, g.workspace_bytes, g.max_block_owner_bytes) == \
+            (w["param"], w["grad"], w["state"], w["comm"], w["ws"], w["blk"])
+    for g, w in zip(blocks, want["block"]):
+        assert (g.block_id, g.param_bytes, g.max_owner_bytes) == (w["block"], w["param"], w["max_owner"])
+        assert (g.gamma, g.c_fsdp, g.c_owner) == (w["gamma"], w["c_fsdp"], w["c_owner"])      # same IEEE operations
+    return ranks, blocks
+
+
+def test_score_plan_matches_oracle_bit_exact():
+    """mfsdp_score_plan (resource scorer + gamma_B / C_B model) against oracle.planner.score_plan on
+    the Llama-shaped plans of C4 / C5 under all three policies and on random models with random owners."""
+    for name in ("c2", "c4", "c5"):
+        wl = workloads.get(name)
+        for policy in (0, 1, 2):
+            pr = mf.mfsdp_plan(wl.params, wl.world, policy, wl.metric, 0)
+            ranks, blocks = _compare_score(wl.params, wl.world, pr.owner)
+            if wl.world > 1:
+                assert all(1.0 <= b.gamma <= wl.world for b in blocks)
+    rng = np.random.default_rng(77)
+    for trial in range(200):
+        params = []
+        for b in range(int(rng.integers(1, 6))):
+            for _ in range(int(rng.integers(0, 6))):
+                if rng.random() < 0.6:
+                    params.append((b, 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)), int(rng.integers(0, 2)), 0))
+                else:
+                    params.append((b, 1, int(rng.integers(1, 300)), 1, 0, int(rng.random() < 0.1)))
+        world = int(rng.integers(1, 7))
+        n_roles = len(oplan.build_roles(params))
+        _compare_score(params, world, [int(rng.integers(0, world)) for _ in range(n_roles)])
+
+
+def test_workspace_estimate_lower_bounds_the_real_workspace():
+    """The scorer's unpadded estimate 2 (2 rows cols + 2 d^2) per matrix vs mfsdp_workspace_bytes of the same rank's
+    table (adds 1024-byte alignment, row pitches and the norm scratch): never above it, within 2 % on the Llama sets."""
+    for name, slack in (("c4", 1.02), ("c5", 1.02), ("c3", 1.6)):
+        wl = workloads.get(name)
+        pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, wl.rank)
+        ranks, _ = mf.mfsdp_score_plan(wl.params, wl.world, pr.owner)
+        est = ranks[pr.rank].workspace_bytes
+        real = mf.mfsdp_workspace_bytes(pr.desc, mf.NS_BF16)
+        assert est <= real <= slack * est + 65536, (name, est, real)
+
+
+def test_score_and_plan_ex_errors():
+    lib = mf.load()
+    P = (mf.Param * 2)(mf.Param(0, 2, 4, 4, 0, 0), mf.Param(1, 2, 8, 4, 0, 0))
+    own = (ctypes.c_int32 * 2)(0, 1)
+    nb = ctypes.c_size_t(0)
+    assert lib.mfsdp_score_plan(P, 2, 2, own, 2, None, None, 0, ctypes.byref(nb)) == 0 and nb.value == 2
+    assert lib.mfsdp_score_plan(P, 2, 2, own, 1, None, None, 0, ctypes.byref(nb)) == mf.EINVAL     # n_roles mismatch
+    bad = (ctypes.c_int32 * 2)(0, 2)
+    assert lib.mfsdp_score_plan(P, 2, 2, bad, 2, None, None, 0, ctypes.byref(nb)) == mf.EINVAL     # owner out of range
+    B = (mf.BlockScore * 1)()
+    assert lib.mfsdp_score_plan(P, 2, 2, own, 2, None, B, 1, ctypes.byref(nb)) == mf.ECAP
+    nd = ctypes.c_size_t(0)
+    zero_den = mf.Caps(owner_den=0)
+    assert lib.mfsdp_plan_ex(P, 2, 2, mf.POLICY_COST_AWARE, 0, 0, ctypes.byref(zero_den), None, None, None, None, 0,
+                             ctypes.byref(nd), None, None) == mf.EINVAL
+    assert lib.mfsdp_plan_ex(P, 2, 2, 3, 0, 0, None, None, None, None, None, 0, ctypes.byref(nd), None, None) == mf.EINVAL
 
 
 def test_configured_resident_sets():
