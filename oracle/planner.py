@@ -273,3 +273,72 @@ def balance(load_vector):
     if total == 0:
         return 1.0
     return max(load_vector) * len(load_vector) / total
+
+
+# ---- owner-segment gradient reduction schedule ----------------------------------------------------------
+# "For gradient reduction, each rank contributes its local full-gradient buffer, but the reduced result is written
+# only to the nonempty owner segment.  The fast path uses deterministic native send/recv schedules ...  Cross-rank
+# validation checks that every rank derives the same deterministic schedule and segment sizes before communication
+# begins, turning mismatches into explicit errors rather than silent NCCL timeouts."
+# Reading F1 (the paper prints no schedule): one reduce-to-owner per role, blocks in REVERSE model
+# order (backward produces the last block's gradients first), roles of a block in parameter order; every record carries
+# the root (owner), the segment size, where the segment lives in the owner's rank-flat gradient buffer (the layout of
+# emit_desc) and which of the owner's per-matrix "gradient landed" flags it raises (tails: none).  The validation value
+# is the 64-bit FNV-1a hash of the records serialised as little-endian 32/64-bit integers.
+
+FNV_OFFSET = 0xCBF29CE484222325
+FNV_PRIME = 0x100000001B3
+
+
+def fnv1a64(data, h=FNV_OFFSET):
+    for byte in data:
+        h ^= byte
+        h = (h * FNV_PRIME) & 0xFFFFFFFFFFFFFFFF
+    return h
+
+
+def reduce_schedule(params, world_size, owner, reverse_blocks=True):
+    """Returns (ops, hash).  op = dict(seq, role, kind, block, param_id, owner, dtype, numel, owner_elem_off, flag)
+    where role indexes build_roles(params), owner_elem_off is the element offset of the segment in the owner's
+    rank-flat buffer of its kind (matrix space or tail space) and flag is the position of the matrix among the owner's
+    matrix descriptors (-1 for tails)."""
+    roles = build_roles(params)
+    if len(owner) != len(roles):
+        raise ValueError("owner[] does not match the roles")
+    off = [[0, 0] for _ in range(world_size)]        # running offsets per rank and kind, as emit_desc lays them out
+    n_mat = [0] * world_size
+    place = []
+    for r, role in enumerate(roles):
+        o = owner[r]
+        if not 0 <= o < world_size:
+            raise ValueError("owner out of range")
+        kind = role["kind"]
+        flag = -1
+        if kind == ROLE_MATRIX:
+            flag = n_mat[o]
+            n_mat[o] += 1
+        place.append((off[o][kind], flag))
+        off[o][kind] = _align_up(off[o][kind] + role["numel"], SEG_ALIGN)
+    blocks = []
+    for r, role in enumerate(roles):
+        if not blocks or blocks[-1][0] != role["block"]:
+            blocks.append((role["block"], []))
+        blocks[-1][1].append(r)
+    if reverse_blocks:
+        blocks = blocks[::-1]
+    ops = []
+    h = FNV_OFFSET
+    for _, ids in blocks:
+        for r in ids:
+            role = roles[r]
+            op = dict(seq=len(ops), role=r, kind=role["kind"], block=role["block"], param_id=role["index"],
+                      owner=owner[r], dtype=role["dtype"], numel=role["numel"], owner_elem_off=place[r][0],
+                      flag=place[r][1])
+            ops.append(op)
+            rec = b"".join(int(v & 0xFFFFFFFF).to_bytes(4, "little") for v in
+                           (op["seq"], op["role"], op["kind"], op["block"], op["param_id"], op["owner"], op["dtype"],
+                            op["flag"]))
+            rec += int(op["numel"]).to_bytes(8, "little") + int(op["owner_elem_off"]).to_bytes(8, "little")
+            h = fnv1a64(rec, h)
+    h = fnv1a64(int(world_size).to_bytes(4, "little") + len(ops).to_bytes(4, "little"), h)
+    return ops, h

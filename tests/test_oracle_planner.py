@@ -264,3 +264,45 @@ def test_llama_balance_ratios_in_the_papers_range():
     for W in (8, 64):
         bal = [oplan.balance(oplan.plan(wl.params, W, pol, wl.metric)["loads"][0]) for pol in (0, 1, 2)]
         assert 1.0 <= bal[1] <= bal[2] <= bal[0] <= 1.4
+
+
+# ---- gradient-reduction schedule and its validation hash (reading F1) -------------------------------------
+def test_fnv1a64_published_vectors():
+    """FNV-1a 64 test vectors of the algorithm's reference distribution: "" / "a" / "foobar"."""
+    assert oplan.fnv1a64(b"") == 0xCBF29CE484222325
+    assert oplan.fnv1a64(b"a") == 0xAF63DC4C8601EC8C
+    assert oplan.fnv1a64(b"foobar") == 0x85944171F73967E8
+
+
+def test_reduce_schedule_hand_trace():
+    """Two blocks, world 2.  Block 0: matrix 4x8 (rank 0), tail of 10 (rank 1), matrix 8x4 (rank 0); block 1: matrix
+    16x16 (rank 1).  Backward order: block 1 first.  Offsets follow emit_desc (64-element alignment per kind)."""
+    params = [(0, 2, 4, 8, 0, 0), (0, 1, 10, 1, 0, 0), (0, 2, 8, 4, 0, 0), (1, 2, 16, 16, 0, 0)]
+    ops, h = oplan.reduce_schedule(params, 2, [0, 1, 0, 1])
+    assert [(o["role"], o["owner"], o["numel"], o["owner_elem_off"], o["flag"]) for o in ops] == \
+        [(3, 1, 256, 0, 0), (0, 0, 32, 0, 0), (1, 1, 10, 0, -1), (2, 0, 32, 64, 1)]
+    assert [o["seq"] for o in ops] == [0, 1, 2, 3]
+    fwd, h2 = oplan.reduce_schedule(params, 2, [0, 1, 0, 1], reverse_blocks=False)
+    assert [o["role"] for o in fwd] == [0, 1, 2, 3] and h2 != h
+    # the offsets and flags are the ones of each owner's descriptor table
+    for rank in (0, 1):
+        desc = oplan.emit_desc(oplan.build_roles(params), [0, 1, 0, 1], rank)
+        mats = [d for d in desc if d["role"] == oplan.ROLE_MATRIX]
+        for o in ops:
+            if o["owner"] == rank and o["kind"] == oplan.ROLE_MATRIX:
+                assert mats[o["flag"]]["elem_off"] == o["owner_elem_off"] and mats[o["flag"]]["param_id"] == o["param_id"]
+
+
+def test_reduce_schedule_hash_detects_any_mismatch():
+    import workloads
+    wl = workloads.get("c4")
+    owner = oplan.plan(wl.params, 8, 0, wl.metric)["owner"]
+    ops, h = oplan.reduce_schedule(wl.params, 8, owner)
+    assert len(ops) == len(owner) and sorted(o["role"] for o in ops) == list(range(len(owner)))
+    assert sum(o["numel"] for o in ops) == sum(r["numel"] for r in oplan.build_roles(wl.params))
+    assert oplan.reduce_schedule(wl.params, 8, owner)[1] == h                       # deterministic
+    other = list(owner); other[5] = (other[5] + 1) % 8
+    assert oplan.reduce_schedule(wl.params, 8, other)[1] != h                       # different owner
+    p2 = list(wl.params); p2[3] = p2[3][:2] + (p2[3][2] + 64,) + p2[3][3:]
+    assert oplan.reduce_schedule(p2, 8, owner)[1] != h                              # different segment size
+    assert oplan.reduce_schedule(wl.params, 8, owner, reverse_blocks=False)[1] != h  # different order
