@@ -180,6 +180,28 @@ typedef struct {
 int mfsdp_score_plan(const mfsdp_param_t* params, size_t n_params, int world_size, const int32_t* owner, size_t n_roles,
                      mfsdp_rank_score_t* rank_out, mfsdp_block_score_t* block_out, size_t block_cap, size_t* n_blocks);
 
+/* Owner-segment gradient-reduction schedule ("each rank contributes its local full-gradient buffer, but
+ * the reduced result is written only to the nonempty owner segment"; "deterministic native send/recv
+ * schedules ... Cross-rank validation checks that every rank derives the same deterministic schedule and segment sizes
+ * before communication begins").  HOST, integers.  DESIGN.md reading F1: one reduce-to-owner per role (on one NVSwitch
+ * domain: ncclReduce with root = owner, or grouped send/recv), blocks in reverse model order when reverse_blocks != 0
+ * (backward produces the last block first), roles of a block in parameter order.  Every rank calls this with the same
+ * (params, world_size, owner) and compares *hash_out (FNV-1a 64 over the records) with its peers before it communicates;
+ * a mismatch is a configuration error to raise, not a hang to wait for.
+ *   owner_elem_off  where the reduced segment lands: element offset in the OWNER's rank-flat buffer of its kind (the
+ *                   elem_off of that rank's descriptor table, mfsdp_plan);
+ *   flag            position of the matrix among the owner's MATRIX descriptors = the index of its "gradient landed"
+ *                   flag for mfsdp_muon_step_gated (-1 for tails).
+ * ops_out == NULL: only *n_ops and *hash_out are written.  Errors as mfsdp_score_plan. */
+typedef struct {
+  uint32_t seq, role, kind, block_id, param_id, owner, dtype;
+  int32_t  flag;
+  uint64_t numel, owner_elem_off;
+} mfsdp_reduce_op_t;
+int mfsdp_reduce_schedule(const mfsdp_param_t* params, size_t n_params, int world_size, const int32_t* owner,
+                          size_t n_roles, int reverse_blocks, mfsdp_reduce_op_t* ops_out, size_t ops_cap, size_t* n_ops,
+                          uint64_t* hash_out);
+
 /* Validate a descriptor table against PAPER.md:71 / Alg. 1 line 5 (HOST).  0 or MFSDP_ELAYOUT / MFSDP_EINVAL. */
 int mfsdp_validate_desc(const mfsdp_desc_t* desc, size_t n_desc);
 
@@ -238,6 +260,25 @@ int mfsdp_workspace_view(const mfsdp_desc_t* desc, size_t n_desc, int precision,
  * run concurrently with step calls. */
 int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
                     void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+
+/* mfsdp_muon_step whose momentum pass starts on each matrix as soon as that matrix' gradient has landed (PAPER.md:47,
+ * 83: the gradient reduction "deposits the complete gradient on that owner"): the step may be
+ * enqueued while the reduction is still running on another stream.
+ *   ready   DEVICE in.  one uint32 per MATRIX descriptor, in table order.  The chunks of matrix i are processed once
+ *                       ready[i] >= epoch (acquire at system scope, so that writes of a copy engine, a peer GPU or
+ *                       the host made before the flag write are visible); G is read through L2 only.
+ *   epoch               the value the producer writes for this step (e.g. the step number; flags never need a reset).
+ * The producer -- the reduction's completion, or a host-to-device copy -- raises flag i with
+ * mfsdp_signal_ready(ready, i, epoch, producer_stream) AFTER the work that fills matrix i's gradient, on the stream
+ * that does that work.  The producer's work must not depend on SM resources that the waiting kernel occupies: enqueue
+ * the producer BEFORE this call (a kernel already running keeps its SMs), or use copy engines.  A wait longer than
+ * ~10 s of SM clocks traps (MFSDP_ECUDA on the next call) instead of hanging the device.  Newton-Schulz and the update
+ * start when the whole momentum pass is done (stream order).  Results are bit-identical to mfsdp_muon_step. */
+int mfsdp_muon_step_gated(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
+                          void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,
+                          const uint32_t* ready, uint32_t epoch, void* cuda_stream);
+/* Stream-ordered 32-bit write ready[index] = epoch (cuStreamWriteValue32: no kernel, no SM). */
+int mfsdp_signal_ready(uint32_t* ready, size_t index, uint32_t epoch, void* cuda_stream);
 
 /* Individual passes of the step, exposed so tests can check each kernel against the oracle and bench.py can time
  * them.  Same arguments and errors as mfsdp_muon_step.

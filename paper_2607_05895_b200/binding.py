@@ -68,6 +68,12 @@ class BlockScore(C.Structure):       # mfsdp_block_score_t
                 ("max_owner_bytes", C.c_uint64), ("gamma", C.c_double), ("c_fsdp", C.c_double), ("c_owner", C.c_double)]
 
 
+class ReduceOp(C.Structure):         # mfsdp_reduce_op_t
+    _fields_ = [("seq", C.c_uint32), ("role", C.c_uint32), ("kind", C.c_uint32), ("block_id", C.c_uint32),
+                ("param_id", C.c_uint32), ("owner", C.c_uint32), ("dtype", C.c_uint32), ("flag", C.c_int32),
+                ("numel", C.c_uint64), ("owner_elem_off", C.c_uint64)]
+
+
 class MfsdpError(RuntimeError):
     def __init__(self, code, what):
         self.code = code
@@ -84,7 +90,8 @@ class PlanResult:
     policy_used: int = -1
 
 
-_SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
+_SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_reduce_schedule", "mfsdp_muon_step_gated",
+            "mfsdp_signal_ready", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
             "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
@@ -119,6 +126,8 @@ def load():
                                   C.POINTER(C.c_uint64), pD, sz, psz, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     lib.mfsdp_score_plan.argtypes = [pP, sz, i32, C.POINTER(C.c_int32), sz, C.POINTER(RankScore), C.POINTER(BlockScore),
                                      sz, psz]
+    lib.mfsdp_reduce_schedule.argtypes = [pP, sz, i32, C.POINTER(C.c_int32), sz, i32, C.POINTER(ReduceOp), sz, psz,
+                                          C.POINTER(C.c_uint64)]
     lib.mfsdp_validate_desc.argtypes = [pD, sz]
     lib.mfsdp_flat_elems.argtypes = [pD, sz, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.mfsdp_workspace_bytes.argtypes = [pD, sz, i32, psz]
@@ -126,6 +135,8 @@ def load():
     lib.mfsdp_debug_ws_offsets.argtypes = [pD, sz, i32, sz, psz]
     pMH, pAH = C.POINTER(MuonHParams), C.POINTER(AdamWHParams)
     lib.mfsdp_muon_step.argtypes = [pD, sz, vp, vp, vp, vp, sz, pMH, vp]
+    lib.mfsdp_muon_step_gated.argtypes = [pD, sz, vp, vp, vp, vp, sz, pMH, vp, C.c_uint32, vp]
+    lib.mfsdp_signal_ready.argtypes = [vp, sz, C.c_uint32, vp]
     lib.mfsdp_muon_momentum_pass.argtypes = [pD, sz, vp, vp, vp, sz, pMH, vp]
     lib.mfsdp_muon_ns_pass.argtypes = [pD, sz, vp, sz, pMH, vp]
     lib.mfsdp_muon_update_pass.argtypes = [pD, sz, vp, vp, sz, pMH, vp]
@@ -342,6 +353,32 @@ def mfsdp_muon_step(desc, W, G, M, workspace, hp, stream=None):
     arr, n = _dn(desc)
     _check(load().mfsdp_muon_step(arr, n, _ptr(W), _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
                                   C.byref(hp), _stream(stream)), "mfsdp_muon_step")
+
+
+def mfsdp_muon_step_gated(desc, W, G, M, workspace, hp, ready, epoch, stream=None):
+    """ready: uint32/int32 CUDA tensor, one flag per matrix descriptor; the momentum pass of matrix i waits for
+    ready[i] >= epoch."""
+    arr, n = _dn(desc)
+    _check(load().mfsdp_muon_step_gated(arr, n, _ptr(W), _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
+                                        C.byref(hp), _ptr(ready), int(epoch), _stream(stream)), "mfsdp_muon_step_gated")
+
+
+def mfsdp_signal_ready(ready, index, epoch, stream=None):
+    _check(load().mfsdp_signal_ready(_ptr(ready), int(index), int(epoch), _stream(stream)), "mfsdp_signal_ready")
+
+
+def mfsdp_reduce_schedule(params, world_size, owner, reverse_blocks=True):
+    """(list of ReduceOp, 64-bit validation hash) of the owner-segment gradient reduction."""
+    lib = load()
+    arr, n = _param_array(params)
+    own = (C.c_int32 * max(1, len(owner)))(*owner)
+    n_ops, h = C.c_size_t(0), C.c_uint64(0)
+    _check(lib.mfsdp_reduce_schedule(arr, n, world_size, own, len(owner), int(reverse_blocks), None, 0, C.byref(n_ops),
+                                     C.byref(h)), "mfsdp_reduce_schedule(size)")
+    ops = (ReduceOp * max(1, n_ops.value))()
+    _check(lib.mfsdp_reduce_schedule(arr, n, world_size, own, len(owner), int(reverse_blocks), ops, n_ops.value,
+                                     C.byref(n_ops), C.byref(h)), "mfsdp_reduce_schedule")
+    return list(ops[:n_ops.value]), h.value
 
 
 def mfsdp_muon_momentum_pass(desc, G, M, workspace, hp, stream=None):

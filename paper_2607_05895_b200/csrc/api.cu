@@ -8,6 +8,8 @@
 #include <mutex>
 #include <string>
 
+#include <cuda.h>
+
 #include "mfsdp_internal.h"
 
 namespace mfsdp {
@@ -289,20 +291,57 @@ extern "C" int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, v
   return launch_update(*pl, W, *hp, static_cast<cudaStream_t>(cuda_stream));
 }
 
+namespace {
+int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M, void* workspace,
+                   size_t ws_bytes, const mfsdp_muon_hparams_t* hp, const uint32_t* ready, uint32_t epoch,
+                   void* cuda_stream);
+}  // namespace
+
 extern "C" int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
                                void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
+  return muon_step_impl(desc, n_desc, W, G, M, workspace, ws_bytes, hp, nullptr, 0u, cuda_stream);
+}
+
+extern "C" int mfsdp_muon_step_gated(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
+                                     void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,
+                                     const uint32_t* ready, uint32_t epoch, void* cuda_stream) {
+  if (!ready || (reinterpret_cast<uintptr_t>(ready) & 3)) return MFSDP_EINVAL;
+  return muon_step_impl(desc, n_desc, W, G, M, workspace, ws_bytes, hp, ready, epoch, cuda_stream);
+}
+
+extern "C" int mfsdp_signal_ready(uint32_t* ready, size_t index, uint32_t epoch, void* cuda_stream) {
+  if (!ready || (reinterpret_cast<uintptr_t>(ready) & 3)) return MFSDP_EINVAL;
+  typedef CUresult (*WriteFn)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+  static WriteFn fn = nullptr;
+  if (!fn) {
+    void* sym = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &sym, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess || !sym)
+      return cuda_fail(cudaErrorSymbolNotFound);
+    fn = reinterpret_cast<WriteFn>(sym);
+  }
+  const CUresult r = fn(static_cast<CUstream>(cuda_stream), reinterpret_cast<CUdeviceptr>(ready + index), epoch, 0);
+  return r == CUDA_SUCCESS ? MFSDP_OK : cuda_fail(cudaErrorUnknown);
+}
+
+namespace {
+int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M, void* workspace,
+                   size_t ws_bytes, const mfsdp_muon_hparams_t* hp, const uint32_t* ready, uint32_t epoch,
+                   void* cuda_stream) {
   Plan* pl = nullptr;
   int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
   if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   if (!W || !G || !M || !aligned(W, 128) || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  if ((rc = launch_momentum(*pl, G, M, *hp, st))) return rc;
+  if ((rc = launch_momentum(*pl, G, M, *hp, st, ready, epoch))) return rc;
   if (hp->precision == MFSDP_NS_BF16 && ns_tc_can_fuse_update(*pl))     // the update runs in the last APPLY epilogue
     return launch_ns_tc(*pl, *hp, st, W, (hp->flags & MFSDP_STEP_KEEP_O) != 0);
   if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
   return launch_update(*pl, W, *hp, st);
 }
+}  // namespace
 
 namespace mfsdp {
 namespace {

@@ -10,6 +10,8 @@
 // ~40 KB in flight per SM).
 #include <cuda_bf16.h>
 
+#include <algorithm>
+
 #include "mfsdp_internal.h"
 
 namespace mfsdp {
@@ -58,6 +60,29 @@ __device__ __forceinline__ F8 load8_ro(const __nv_bfloat16* p) {
   }
   return r;
 }
+// L2-only loads (gated pass: the gradient is written by another agent -- copy engine, peer GPU -- while this kernel runs)
+__device__ __forceinline__ F8 load8_cg(const float* p) {
+  F8 r;
+  const float4 a = __ldcg(reinterpret_cast<const float4*>(p));
+  const float4 b = __ldcg(reinterpret_cast<const float4*>(p + 4));
+  r.v[0] = a.x; r.v[1] = a.y; r.v[2] = a.z; r.v[3] = a.w; r.v[4] = b.x; r.v[5] = b.y; r.v[6] = b.z; r.v[7] = b.w;
+  return r;
+}
+__device__ __forceinline__ F8 load8_cg(const __nv_bfloat16* p) {
+  F8 r;
+  const uint4 u = __ldcg(reinterpret_cast<const uint4*>(p));
+  const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    r.v[2 * i] = __uint_as_float(w[i] << 16);
+    r.v[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+  }
+  return r;
+}
+__device__ __forceinline__ float load1_cg(const float* p) { return __ldcg(p); }
+__device__ __forceinline__ float load1_cg(const __nv_bfloat16* p) {
+  return __uint_as_float((uint32_t)__ldcg(reinterpret_cast<const unsigned short*>(p)) << 16);
+}
 __device__ __forceinline__ void store8(float* p, const F8& x) {
   *reinterpret_cast<float4*>(p) = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]);
   *reinterpret_cast<float4*>(p + 4) = make_float4(x.v[4], x.v[5], x.v[6], x.v[7]);
@@ -91,14 +116,32 @@ __device__ __forceinline__ double block_sum(double x, double* smem) {
 }
 
 // ---- a1: momentum + Nesterov + cast + partial squared norm ---------------------------------------------------------
-template <typename GT, typename XT>
+// kGated: the chunks of matrix i wait until ready[i] >= epoch (mfsdp_muon_step_gated), and G is read through L2.
+template <typename GT, typename XT, bool kGated>
 __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __restrict__ mats,
                                                          const uint32_t* __restrict__ chunk_mat, uint32_t n_chunks,
                                                          const GT* __restrict__ G, float* __restrict__ M,
                                                          uint8_t* __restrict__ ws, double* __restrict__ partial,
-                                                         float mu, float omm, int nesterov) {
+                                                         float mu, float omm, int nesterov,
+                                                         const uint32_t* __restrict__ ready, uint32_t epoch) {
   __shared__ double red[kEwThreads / 32];
   for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
+    if constexpr (kGated) {
+      if (threadIdx.x == 0) {
+        const uint32_t* flag = ready + chunk_mat[c];
+        uint32_t v;
+        asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+        if ((int32_t)(v - epoch) < 0) {
+          const long long t0 = clock64();
+          do {
+            __nanosleep(200);
+            if (clock64() - t0 > 20000000000ll) __trap();       // ~10 s: the producer never signalled
+            asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+          } while ((int32_t)(v - epoch) < 0);
+        }
+      }
+      __syncthreads();
+    }
     const MatLayout L = mats[chunk_mat[c]];
     const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
     const GT* g = G + L.elem_off;
@@ -113,7 +156,7 @@ __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __rest
 #pragma unroll
         for (int v = 0; v < kBatch; ++v) {
           const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
-          gv[v] = load8_ro(g + e0);
+          gv[v] = kGated ? load8_cg(g + e0) : load8_ro(g + e0);
           mv[v] = load8(m + e0);
         }
 #pragma unroll
@@ -136,7 +179,7 @@ __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __rest
         const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
         if (e0 >= L.numel) break;
         if (vec && e0 + 8 <= L.numel) {
-          const F8 gv = load8_ro(g + e0);
+          const F8 gv = kGated ? load8_cg(g + e0) : load8_ro(g + e0);
           F8 mv = load8(m + e0);
           F8 uv;
 #pragma unroll
@@ -151,7 +194,7 @@ __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __rest
         } else {
           const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
           for (uint64_t e = e0; e < e1; ++e) {
-            const float gs = omm * load1(g + e);
+            const float gs = omm * (kGated ? load1_cg(g + e) : load1(g + e));
             const float mn = fmaf(mu, m[e], gs);
             const float u = nesterov ? fmaf(mu, mn, gs) : mn;
             acc = fma((double)u, (double)u, acc);
@@ -294,19 +337,35 @@ int ew_grid(uint32_t n_chunks) {
 
 }  // namespace
 
-int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
+int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hparams_t& hp, cudaStream_t st,
+                    const uint32_t* ready, uint32_t epoch) {
   const WsLayout& lay = pl.lay;
   const uint32_t n_mat = (uint32_t)lay.mats.size();
   if (n_mat == 0) return MFSDP_OK;
   uint8_t* ws = static_cast<uint8_t*>(pl.workspace);
   double* partial = reinterpret_cast<double*>(ws + lay.partial_off);
   const float mu = (float)hp.momentum, omm = (float)(1.0 - hp.momentum);
-  const int grid = ew_grid(lay.n_chunks);
+  // Gated: CTAs spin while they wait for their matrix; at most 2 per SM, so that whatever produces the gradients
+  // (a copy kernel, a collective launched late) still finds room on every SM.
+  int grid = ew_grid(lay.n_chunks);
+  if (ready) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    grid = std::min(grid, 2 * sms);
+  }
   const bool gbf = lay.mat_dtype == MFSDP_BF16, xbf = pl.precision == MFSDP_NS_BF16;
-#define MOM(GT, XT)                                                                                             \
-  k_momentum<GT, XT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                      \
-                                                  static_cast<const GT*>(G), static_cast<float*>(M), ws, partial, \
-                                                  mu, omm, hp.nesterov)
+#define MOM(GT, XT)                                                                                                    \
+  do {                                                                                                                 \
+    if (ready)                                                                                                         \
+      k_momentum<GT, XT, true><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                   \
+                                                            static_cast<const GT*>(G), static_cast<float*>(M), ws,     \
+                                                            partial, mu, omm, hp.nesterov, ready, epoch);              \
+    else                                                                                                               \
+      k_momentum<GT, XT, false><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                  \
+                                                             static_cast<const GT*>(G), static_cast<float*>(M), ws,    \
+                                                             partial, mu, omm, hp.nesterov, nullptr, 0u);              \
+  } while (0)
   if (gbf && xbf) MOM(__nv_bfloat16, __nv_bfloat16);
   else if (gbf) MOM(__nv_bfloat16, float);
   else if (xbf) MOM(float, __nv_bfloat16);

@@ -74,7 +74,8 @@ struct Plan {
 int get_plan(const mfsdp_desc_t* desc, size_t n_desc, int precision, void* workspace, bool need_ws, Plan** out);
 
 // ---- kernels (host launchers); all return an MFSDP_* code ------------------------------------------------------
-int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hparams_t& hp, cudaStream_t st);
+int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hparams_t& hp, cudaStream_t st,
+                    const uint32_t* ready = nullptr, uint32_t epoch = 0);   // ready != nullptr: gated per matrix
 int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaStream_t st);
 int launch_adamw(const Plan& pl, void* P, const void* G, void* m, void* v, const mfsdp_adamw_hparams_t& hp,
                  cudaStream_t st);

@@ -208,6 +208,67 @@ extern "C" int mfsdp_score_plan(const mfsdp_param_t* params, size_t n_params, in
   return MFSDP_OK;
 }
 
+namespace {
+inline void fnv_bytes(uint64_t& h, const void* p, size_t n) {
+  const unsigned char* b = static_cast<const unsigned char*>(p);
+  for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 0x100000001B3ull; }
+}
+inline void fnv_u32(uint64_t& h, uint32_t v) { unsigned char b[4] = {(unsigned char)v, (unsigned char)(v >> 8), (unsigned char)(v >> 16), (unsigned char)(v >> 24)}; fnv_bytes(h, b, 4); }
+inline void fnv_u64(uint64_t& h, uint64_t v) { fnv_u32(h, (uint32_t)v); fnv_u32(h, (uint32_t)(v >> 32)); }
+}  // namespace
+
+extern "C" int mfsdp_reduce_schedule(const mfsdp_param_t* params, size_t n_params, int world, const int32_t* owner,
+                                     size_t n_roles, int reverse_blocks, mfsdp_reduce_op_t* ops_out, size_t ops_cap,
+                                     size_t* n_ops, uint64_t* hash_out) {
+  if ((n_params && !params) || world < 1 || (n_roles && !owner)) return MFSDP_EINVAL;
+  std::vector<Role> roles;
+  const int rc = build_roles(params, n_params, roles);
+  if (rc) return rc;
+  if (roles.size() != n_roles) return MFSDP_EINVAL;
+  for (size_t i = 0; i < n_roles; ++i) if (owner[i] < 0 || owner[i] >= world) return MFSDP_EINVAL;
+  // where each role's segment lives on its owner (the layout mfsdp_plan emits) and which landed-flag it raises
+  std::vector<uint64_t> off((size_t)world * 2, 0), place(roles.size());
+  std::vector<int32_t> n_mat((size_t)world, 0), flag(roles.size(), -1);
+  for (size_t i = 0; i < roles.size(); ++i) {
+    const size_t o = (size_t)owner[i];
+    if (roles[i].kind == MFSDP_ROLE_MATRIX) flag[i] = n_mat[o]++;
+    uint64_t& f = off[o * 2 + roles[i].kind];
+    place[i] = f;
+    f = align_up(f + roles[i].numel, MFSDP_SEG_ALIGN);
+  }
+  std::vector<std::pair<size_t, size_t>> blocks;      // [begin, end) role runs per block, model order
+  for (size_t i = 0; i < roles.size();) {
+    size_t j = i;
+    while (j < roles.size() && roles[j].block == roles[i].block) ++j;
+    blocks.push_back({i, j});
+    i = j;
+  }
+  if (reverse_blocks) std::reverse(blocks.begin(), blocks.end());
+  std::vector<mfsdp_reduce_op_t> ops;
+  uint64_t h = 0xCBF29CE484222325ull;
+  for (const auto& b : blocks)
+    for (size_t i = b.first; i < b.second; ++i) {
+      mfsdp_reduce_op_t op;
+      std::memset(&op, 0, sizeof op);
+      op.seq = (uint32_t)ops.size(); op.role = (uint32_t)i; op.kind = roles[i].kind; op.block_id = roles[i].block;
+      op.param_id = roles[i].first; op.owner = (uint32_t)owner[i]; op.dtype = roles[i].dtype; op.flag = flag[i];
+      op.numel = roles[i].numel; op.owner_elem_off = place[i];
+      ops.push_back(op);
+      fnv_u32(h, op.seq); fnv_u32(h, op.role); fnv_u32(h, op.kind); fnv_u32(h, op.block_id); fnv_u32(h, op.param_id);
+      fnv_u32(h, op.owner); fnv_u32(h, op.dtype); fnv_u32(h, (uint32_t)op.flag);
+      fnv_u64(h, op.numel); fnv_u64(h, op.owner_elem_off);
+    }
+  fnv_u32(h, (uint32_t)world);
+  fnv_u32(h, (uint32_t)ops.size());
+  if (n_ops) *n_ops = ops.size();
+  if (hash_out) *hash_out = h;
+  if (ops_out) {
+    if (ops_cap < ops.size()) return MFSDP_ECAP;
+    if (!ops.empty()) std::memcpy(ops_out, ops.data(), ops.size() * sizeof(mfsdp_reduce_op_t));
+  }
+  return MFSDP_OK;
+}
+
 extern "C" int mfsdp_plan_ex(const mfsdp_param_t* params, size_t n_params, int world, int policy, int metric, int rank,
                              const mfsdp_caps_t* caps, int32_t* owner_out, size_t* n_roles, uint64_t* rank_load_out,
                              mfsdp_desc_t* desc_out, size_t desc_cap, size_t* n_desc, int* rank_out, int* policy_used) {

@@ -269,3 +269,45 @@ def test_debug_trace_rejects_bad_buffers():
     assert lib.mfsdp_debug_trace(ctypes.c_void_p(8), 16) == mf.EINVAL       # too small
     assert lib.mfsdp_debug_trace(ctypes.c_void_p(12), 4096) == mf.EINVAL    # not 8-byte aligned
     assert lib.mfsdp_debug_trace(None, 0) == 0                              # off
+
+
+def test_reduce_schedule_matches_oracle_bit_exact():
+    """mfsdp_reduce_schedule (reading F1) against oracle.planner.reduce_schedule: records and the
+    FNV-1a validation hash, on the Llama plans and on random models, both block orders."""
+    def compare(params, world, owner, rev):
+        want, wh = oplan.reduce_schedule(params, world, owner, rev)
+        got, gh_ = mf.mfsdp_reduce_schedule(params, world, owner, rev)
+        assert gh_ == wh and len(got) == len(want)
+        for g, w in zip(got, want):
+            assert (g.seq, g.role, g.kind, g.block_id, g.param_id, g.owner, g.dtype, g.flag, g.numel, g.owner_elem_off) == \
+                (w["seq"], w["role"], w["kind"], w["block"], w["param_id"], w["owner"], w["dtype"], w["flag"], w["numel"],
+                 w["owner_elem_off"])
+    for name in ("c2", "c4", "c5"):
+        wl = workloads.get(name)
+        pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, 0)
+        for rev in (True, False):
+            compare(wl.params, wl.world, pr.owner, rev)
+    rng = np.random.default_rng(31)
+    for trial in range(150):
+        params = []
+        for b in range(int(rng.integers(1, 6))):
+            for _ in range(int(rng.integers(0, 6))):
+                if rng.random() < 0.6:
+                    params.append((b, 2, int(rng.integers(1, 40)), int(rng.integers(1, 40)), int(rng.integers(0, 2)), 0))
+                else:
+                    params.append((b, 1, int(rng.integers(1, 300)), 1, 0, int(rng.random() < 0.1)))
+        world = int(rng.integers(1, 7))
+        n_roles = len(oplan.build_roles(params))
+        compare(params, world, [int(rng.integers(0, world)) for _ in range(n_roles)], bool(trial % 2))
+
+
+def test_gated_step_and_signal_reject_bad_arguments_without_a_gpu():
+    lib = mf.load()
+    wl = workloads.get("c1")
+    pr = mf.mfsdp_plan(wl.params, 1)
+    hp = mf.MuonHParams(precision=mf.NS_FP32)
+    assert lib.mfsdp_muon_step_gated(pr.desc, pr.desc._n, 1024, 1024, 1024, 1024, 1 << 30, ctypes.byref(hp), None, 1,
+                                     None) == mf.EINVAL                      # no flags
+    assert lib.mfsdp_muon_step_gated(pr.desc, pr.desc._n, 1024, 1024, 1024, 1024, 1 << 30, ctypes.byref(hp), 1026, 1,
+                                     None) == mf.EINVAL                      # misaligned flags
+    assert lib.mfsdp_signal_ready(None, 0, 1, None) == mf.EINVAL

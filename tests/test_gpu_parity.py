@@ -429,6 +429,55 @@ def test_separate_passes_equal_fused_step(wname):
                 assert torch.equal(x, y)
 
 
+@pytest.mark.parametrize("wname", ["medium", "small"])
+@pytest.mark.parametrize("consumer_first", [True, False])
+def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
+    """SURVEY 8(f) f1 in the form one GPU can test: the gradients of the resident matrices arrive in 3 waves (here:
+    host-to-device copies on another stream; in the real system the owner-segment reduction of PAPER.md:83), each wave
+    followed by mfsdp_signal_ready on the producing stream; mfsdp_muon_step_gated is enqueued BEFORE the first byte has
+    arrived (consumer_first) -- its momentum kernel waits per matrix -- or after.  Device gradient buffer poisoned with
+    NaN beforehand.  Two consecutive steps (epochs 1, 2; the flags are never reset).  Bit-identical to the ungated step."""
+    import time
+    wl = workloads.get(wname)
+    a = gh.Session(wl)
+    b = gh.Session(wl)
+    n_mat = len(b.mats)
+    ready = torch.zeros(n_mat, dtype=torch.int32, device="cuda")
+    side = torch.cuda.Stream()
+    waves = [list(range(n_mat))[k::3] for k in range(3)][::-1]          # interleaved, last third first
+    for epoch in (1, 2):
+        a.load_grads(epoch - 1)
+        a.muon_step()
+        hG = workloads.fill_flat(wl, b.descs, workloads.KIND_G, step=epoch - 1).pin_memory()
+        b.G = torch.full_like(a.G, float("nan"))
+        torch.cuda.synchronize()
+
+        def produce():
+            with torch.cuda.stream(side):
+                for wave in waves:
+                    for i in wave:
+                        d = b.mats[i]
+                        sl = slice(d.elem_off, d.elem_off + d.rows * d.cols)
+                        b.G[sl].copy_(hG[sl], non_blocking=True)
+                        mf.mfsdp_signal_ready(ready, i, epoch, side)
+                    if consumer_first:
+                        side.synchronize()
+                        time.sleep(0.02)                                # the momentum kernel is waiting meanwhile
+
+        def consume():
+            mf.mfsdp_muon_step_gated(b.desc, b.W, b.G, b.M, b.ws, b.hp, ready, epoch)
+
+        if consumer_first:
+            consume(); produce()
+        else:
+            produce(); consume()
+        torch.cuda.synchronize()
+        assert int(ready.min().item()) == epoch
+        assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M)
+        for x, y in zip(_o_bits(a), _o_bits(b)):
+            assert torch.equal(x, y)
+
+
 def test_host_buffer_entry_point():
     wl = workloads.small_ragged()
     a = gh.Session(wl)

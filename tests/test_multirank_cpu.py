@@ -60,3 +60,59 @@ def test_single_rank_keeps_workload_choice():
     assert bench.choose_plan_rank([5, 3, 1], 0, 0, 1) == 0
     assert bench.choose_plan_rank([5, 3, 1], -1, 0, 1) == 5
     assert bench.choose_plan_rank([5, 3, 1], 0, 1, 2) == 3
+
+
+# ---- cross-rank validation of the gradient-reduction schedule -------------------------------------------
+def _sched_worker(rank, world, port, out, perturb):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import paper_2607_05895_b200 as mf
+    from paper_2607_05895_b200 import dist as mdist
+    import workloads
+    wl = workloads.get("c4")
+    params = list(wl.params)
+    if perturb and rank == 1:                         # rank 1 believes one matrix is 64 rows taller
+        p = params[10]
+        params[10] = (p[0], p[1], p[2] + 64, p[3], p[4], p[5])
+    pr = mf.mfsdp_plan(params, wl.world, mf.POLICY_COST_AWARE, wl.metric, rank)
+    try:
+        ops, h = mdist.validated_reduce_schedule(params, wl.world, pr.owner)
+        mine = [(o.seq, o.role, o.numel, o.owner_elem_off, o.flag) for o in ops if o.owner == rank]
+        out.put((rank, "ok", h, len(ops), mine, [pr.desc[i].elem_off for i in range(pr.desc._n)
+                                                 if pr.desc[i].role == mf.ROLE_MATRIX]))
+    except mdist.ScheduleMismatch as e:
+        out.put((rank, "mismatch", sorted(set(e.hashes)), str(e), None, None))
+    dist.destroy_process_group()
+
+
+def _run_sched(perturb):
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000 + (7 if perturb else 0)
+    procs = [ctx.Process(target=_sched_worker, args=(r, 2, port, q, perturb)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=150) for _ in range(2))
+    for p in procs:
+        p.join(30)
+        assert p.exitcode == 0
+    return res
+
+
+@pytest.mark.timeout(180)
+def test_two_ranks_derive_the_same_reduction_schedule():
+    a, b = _run_sched(False)
+    assert a[1] == b[1] == "ok" and a[2] == b[2] and a[3] == b[3] == 32 * 8        # 7 matrices + 1 tail per block
+    for res in (a, b):                               # the segments a rank receives are its own descriptor table's
+        flags = [m for m in res[4] if m[4] >= 0]
+        assert sorted(f[4] for f in flags) == list(range(len(res[5])))
+        for seq, role, numel, off, flag in flags:
+            assert res[5][flag] == off
+
+
+@pytest.mark.timeout(180)
+def test_schedule_mismatch_is_an_explicit_error_on_every_rank():
+    a, b = _run_sched(True)
+    assert a[1] == b[1] == "mismatch" and a[2] == b[2] and len(a[2]) == 2
+    assert "ranks [0]" in a[3] and "ranks [1]" in a[3]
