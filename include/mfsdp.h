@@ -272,7 +272,9 @@ int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void
  * mfsdp_signal_ready(ready, i, epoch, producer_stream) AFTER the work that fills matrix i's gradient, on the stream
  * that does that work.  The producer's work must not depend on SM resources that the waiting kernel occupies: enqueue
  * the producer BEFORE this call (a kernel already running keeps its SMs), or use copy engines.  A wait longer than
- * ~10 s of SM clocks traps (MFSDP_ECUDA on the next call) instead of hanging the device.  Newton-Schulz and the update
+ * ~10 s of SM clocks traps (MFSDP_ECUDA on the next call) instead of hanging the device.  The launch tables of a new
+ * (table, workspace) are built -- synchronously -- before the first kernel of the call is enqueued, so the call never
+ * blocks the host behind its own waiting kernel.  Newton-Schulz and the update
  * start when the whole momentum pass is done (stream order).  Results are bit-identical to mfsdp_muon_step. */
 int mfsdp_muon_step_gated(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
                           void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,

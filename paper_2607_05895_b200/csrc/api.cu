@@ -335,8 +335,11 @@ int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void*
   if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
   if (!W || !G || !M || !aligned(W, 128) || !aligned(G, 128) || !aligned(M, 128)) return MFSDP_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  // Build every launch table of this call BEFORE the first kernel is enqueued: table building allocates and copies
+  // synchronously, which must not happen behind a gated momentum kernel that waits for flags the host raises later.
+  const bool fuse = hp->precision == MFSDP_NS_BF16 && ns_tc_can_fuse_update(*pl);
   if ((rc = launch_momentum(*pl, G, M, *hp, st, ready, epoch))) return rc;
-  if (hp->precision == MFSDP_NS_BF16 && ns_tc_can_fuse_update(*pl))     // the update runs in the last APPLY epilogue
+  if (fuse)                                                             // the update runs in the last APPLY epilogue
     return launch_ns_tc(*pl, *hp, st, W, (hp->flags & MFSDP_STEP_KEEP_O) != 0);
   if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
   return launch_update(*pl, W, *hp, st);
