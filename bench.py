@@ -14,7 +14,12 @@ collective: "the optimizer step contains no matrix all-gather, broad
 
 `value` = algorithmic NS flops of all ranks / max-over-ranks device time (TFLOP/s, symmetric-aware count
 F_alg = K [m(m+1)n + m^2(m+1) + 2 m^2 n]); `ms_per_step` is the step latency, the other half of BASELINE's metric.
-Prints ONE JSON line on rank 0.
+Prints ONE JSON line on rank 0.  At N = 1 the line also carries `other_configs`: BASELINE.json configs 1-4 and the
+paper's own setting on config 5, measured after the headline's timed region in the same process.
+
+`--gpus N` with N > 1 and no WORLD_SIZE in the environment: this process spawns the N ranks itself (one per GPU, the
+same environment torch.distributed.run would set) and forwards rank 0's line; under torch.distributed.run it is one
+of the ranks.
 """
 import argparse
 import json
@@ -43,6 +48,7 @@ def parse_args():
                     help="the paper's own Muon hyper-parameters (PAPER.md:121): momentum 0.5, 2 NS steps, lr 1e-3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
     return ap.parse_args()
 
 
@@ -71,19 +77,27 @@ def apply_setting(wl, args):
 
 
 def ncu_traffic(workload):
-    """DRAM bytes of one k_ns_tc launch (dram__bytes_read.sum + dram__bytes_write.sum of an `ncu --set full` capture of
-    this same command), copied by hand into profiles/ncu_traffic.csv: lines `workload,kernel,bytes`.  None if absent."""
+    """(bytes, commit) of one Newton-Schulz launch: dram__bytes_read.sum + dram__bytes_write.sum of an `ncu --set full`
+    capture of this same command, kept in profiles/ncu_traffic.csv as `workload,kernel,bytes,commit` -- `commit` is the
+    git commit the capture was taken at (stated again in the profiles README of that round), printed beside the number
+    so that a stale capture is visible.  (None, None) if absent."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     if not os.path.exists(path):
-        return None
+        return None, None
     for line in open(path):
         f = [x.strip() for x in line.split(",")]
         if len(f) >= 3 and f[0] == workload and f[1] == "k_ns_tc":
             try:
-                return float(f[2])
+                return float(f[2]), (f[3] if len(f) > 3 else None)
             except ValueError:
-                return None
-    return None
+                return None, None
+    return None, None
+
+
+def min_hbm_bytes(rows, cols, K):
+    """minimal HBM bytes of the Newton-Schulz chain of one matrix, K (3 m n + 4 m^2) * 2."""
+    m, n = min(rows, cols), max(rows, cols)
+    return K * (3 * m * n + 4 * m * m) * 2
 
 
 def peaks():
@@ -157,23 +171,35 @@ def plan_for(wl, rank_override=None):
     return oplan.plan(wl.params, wl.world, wl.policy, wl.metric, r)
 
 
-def oracle_sample(wl, desc, budget_flops=2.5e12):
-    """A bounded sample of the resident set for the fp64 oracle: resident matrices, cheapest NS cost first, until
-    ~budget_flops dense fp64 flops (about 10-30 s of dgemm on the host cores); at least one matrix."""
+ORACLE_BUDGET_FLOPS = 3.6e12      # dense fp64 flops per sample: about 12 s of dgemm on 16 host cores
+
+
+def oracle_sample(wl, desc, budget_flops=ORACLE_BUDGET_FLOPS):
+    """Per-shape sample for the fp64 oracle: ONE resident matrix per distinct shape, cheapest shape
+    first, each run for as many whole Newton-Schulz iterations k <= K as the remaining budget affords (at least the
+    cheapest shape in full).  A shape whose single iteration does not fit is reported as not sampled.  The figure is a
+    RATE (flops executed / seconds), so no extrapolation is involved.  Returns [(desc, k)], [skipped shapes]."""
     import workloads
     K = wl.muon["ns_steps"]
-    mats = [d for d in desc if d["role"] == workloads.ROLE_MATRIX]
-    sample, acc = [], 0.0
-    for d in sorted(mats, key=lambda d: ns_flops(d["rows"], d["cols"], K)[1]):
-        f = ns_flops(d["rows"], d["cols"], K)[1]
-        if sample and acc + f > budget_flops:
-            break
-        sample.append(d); acc += f
-    return sample
+    first = {}
+    for d in desc:
+        if d["role"] == workloads.ROLE_MATRIX:
+            first.setdefault((d["rows"], d["cols"]), d)
+    sample, skipped, left = [], [], float(budget_flops)
+    for (r, c), d in sorted(first.items(), key=lambda kv: ns_flops(kv[0][0], kv[0][1], 1)[1]):
+        per_iter = ns_flops(r, c, 1)[1]
+        k = int(min(K, left // per_iter)) if sample else K
+        if k >= 1:
+            sample.append((d, k))
+            left -= k * per_iter
+        else:
+            skipped.append((r, c))
+    return sample, skipped
 
 
 def time_oracle(wl, sample, steps=1):
-    """Runs oracle.muon.muon_step as it stands on each sampled matrix; returns (seconds per pass, F_alg, cores)."""
+    """Runs oracle.muon.muon_step as it stands on each sampled matrix (with its iteration count); returns
+    (seconds per pass, algorithmic flops executed, cores)."""
     import numpy as np
     import torch
     import workloads
@@ -182,18 +208,18 @@ def time_oracle(wl, sample, steps=1):
     hp = wl.muon
     tdt = workloads.TORCH_DTYPE[wl.dtype]
     inputs = []
-    for d in sample:
+    for d, k in sample:
         W = torch.from_numpy(workloads.weight(wl, d["param_id"], d["rows"], d["cols"])).to(tdt).to(torch.float64).numpy()
         G = torch.from_numpy(workloads.gradient(wl, d["param_id"], d["rows"], d["cols"], 0)).to(tdt).to(
             torch.float64).numpy()
-        inputs.append((W, G, np.zeros_like(W)))
-    f_alg = sum(ns_flops(d["rows"], d["cols"], K)[0] for d in sample)
+        inputs.append((W, G, np.zeros_like(W), k))
+    f_alg = sum(ns_flops(d["rows"], d["cols"], k)[0] for d, k in sample)
     times = []
     for _ in range(steps):
         t0 = time.perf_counter()
-        for W, G, M in inputs:
+        for W, G, M, k in inputs:
             omuon.muon_step(W, G, M, lr=hp["lr"], weight_decay=hp["weight_decay"], momentum=hp["momentum"],
-                            nesterov=bool(hp["nesterov"]), ns_steps=K, coeffs=(hp["a"], hp["b"], hp["c"]),
+                            nesterov=bool(hp["nesterov"]), ns_steps=k, coeffs=(hp["a"], hp["b"], hp["c"]),
                             eps=hp["eps"], scale_mode=hp["scale_mode"])
         times.append(time.perf_counter() - t0)
     try:
@@ -204,32 +230,50 @@ def time_oracle(wl, sample, steps=1):
     return times, f_alg, cores
 
 
-def sample_text(sample):
-    shapes = {}
-    for d in sample:
-        shapes[(d["rows"], d["cols"])] = shapes.get((d["rows"], d["cols"]), 0) + 1
-    return "cheapest resident matrices: " + ", ".join("%d x %dx%d" % (n, r, c) for (r, c), n in shapes.items())
+def sample_text(wl, sample, skipped):
+    K = wl.muon["ns_steps"]
+    txt = "per-shape sampled, one matrix per distinct resident shape: " + ", ".join(
+        "%dx%d (%d of %d NS iterations)" % (d["rows"], d["cols"], k, K) for d, k in sample)
+    if skipped:
+        txt += "; not affordable within %.1e fp64 flops: " % ORACLE_BUDGET_FLOPS + ", ".join("%dx%d" % s for s in skipped)
+    return txt
+
+
+def workload_config(wl, descs, plan_rank):
+    """The `config` object of the JSON line -- the same on both arms (the planners agree bit for bit)."""
+    import workloads
+    K = wl.muon["ns_steps"]
+    mats = [d for d in descs if d["role"] == workloads.ROLE_MATRIX]
+    tails = [d for d in descs if d["role"] == workloads.ROLE_TAIL]
+    n_el = workloads.flat_elems(descs)[0]
+    wbytes = 2 if wl.dtype == workloads.BF16 else 4
+    return dict(workload=wl.name, plan_rank=plan_rank, matrices=len(mats), tails=len(tails), matrix_elems=int(n_el),
+                ns_steps=K, l2="inputs larger than L2" if n_el * wbytes > 256e6 else
+                "working set may fit L2 (not flushed)",
+                ns_flops_alg=sum(ns_flops(d["rows"], d["cols"], K)[0] for d in mats),
+                ns_flops_dense=sum(ns_flops(d["rows"], d["cols"], K)[1] for d in mats))
 
 
 def run_reference(args):
-    """--impl reference: the fp64 oracle, as it stands, on the host cores; each step a bounded sample."""
+    """--impl reference: the fp64 oracle, as it stands, on the host cores; each step the same bounded per-shape sample
+    the cpu_baseline leg of our arm uses."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import workloads
     wl = apply_setting(workloads.get(args.config), args)
     pl = plan_for(wl)
-    sample = oracle_sample(wl, pl["desc"], budget_flops=1.0e12)
+    sample, skipped = oracle_sample(wl, pl["desc"])
     for _ in range(max(0, min(args.warmup, 1))):
         time_oracle(wl, sample, 1)
     times, f_alg, cores = time_oracle(wl, sample, max(1, args.steps))
     t = sum(times) / len(times)
     val = f_alg / t / 1e12
+    txt = sample_text(wl, sample, skipped)
     line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=t * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
-                dtype="f64", data="synthetic (seeded, workloads/)",
-                config=dict(workload=wl.name, sample=sample_text(sample), ns_steps=wl.muon["ns_steps"]),
-                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle", sample=sample_text(sample)),
+                dtype="f64", data="synthetic (seeded, workloads/)", config=workload_config(wl, pl["desc"], pl["rank"]),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle", sample=txt),
                 e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line))
 
@@ -274,6 +318,132 @@ def ev_time(torch, stream, fn, reps):
     return e0.elapsed_time(e1) / reps
 
 
+class Resident:
+    """One resident set on the current device: plan, seeded inputs in pinned host memory and in HBM, workspace."""
+
+    def __init__(self, mf, wl, plan_rank, pin=True):
+        import torch
+        import workloads
+        self.mf, self.wl, self.plan_rank = mf, wl, plan_rank
+        pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, plan_rank)
+        self.desc = pr.desc
+        self.descs = [self.desc[i] for i in range(self.desc._n)]
+        self.ddicts = [d.as_dict() for d in self.descs]
+        self.mats = [d for d in self.descs if d.role == mf.ROLE_MATRIX]
+        self.tails = [d for d in self.descs if d.role == mf.ROLE_TAIL]
+        self.K = wl.muon["ns_steps"]
+        self.hp = mf.MuonHParams(precision=wl.precision, **wl.muon)
+        self.n_mat_el, self.n_tail_el = mf.mfsdp_flat_elems(self.desc)
+        self.wbytes = 2 if wl.dtype == mf.BF16 else 4
+        self.hW = workloads.fill_flat(wl, self.descs, workloads.KIND_W, pin=pin)
+        self.hG = workloads.fill_flat(wl, self.descs, workloads.KIND_G, step=0, pin=pin)
+        self.W, self.G = self.hW.cuda(), self.hG.cuda()
+        self.M = torch.zeros(self.n_mat_el, dtype=torch.float32, device="cuda")
+        self.P = workloads.fill_flat(wl, self.descs, workloads.KIND_W, role=mf.ROLE_TAIL).cuda()
+        self.Gt = workloads.fill_flat(wl, self.descs, workloads.KIND_G, role=mf.ROLE_TAIL).cuda()
+        self.m1 = torch.zeros(self.n_tail_el, dtype=torch.float32, device="cuda")
+        self.v1 = torch.zeros(self.n_tail_el, dtype=torch.float32, device="cuda")
+        ws_bytes = mf.mfsdp_workspace_bytes(self.desc, wl.precision)
+        raw = torch.empty(ws_bytes + 1024, dtype=torch.uint8, device="cuda")
+        off = (-raw.data_ptr()) % 1024
+        self.ws = raw[off:off + ws_bytes]
+        self._raw = raw
+        self.stream = torch.cuda.current_stream()
+        self.t = 0
+        self.f_alg = sum(ns_flops(d.rows, d.cols, self.K)[0] for d in self.mats)
+        self.f_dense = sum(ns_flops(d.rows, d.cols, self.K)[1] for d in self.mats)
+
+    def set_hparams(self, muon, adamw):
+        import copy
+        self.wl = copy.deepcopy(self.wl)              # the caller's workload object keeps its own setting
+        self.wl.muon.update(muon)
+        self.wl.adamw.update(adamw)
+        self.K = self.wl.muon["ns_steps"]
+        self.hp = self.mf.MuonHParams(precision=self.wl.precision, **self.wl.muon)
+        self.f_alg = sum(ns_flops(d.rows, d.cols, self.K)[0] for d in self.mats)
+        self.f_dense = sum(ns_flops(d.rows, d.cols, self.K)[1] for d in self.mats)
+
+    def step(self):
+        """One pass of the whole hot path: mfsdp_muon_step on every owned matrix + mfsdp_adamw_tail_step on the tails."""
+        mf = self.mf
+        self.t += 1
+        mf.mfsdp_muon_step(self.desc, self.W, self.G, self.M, self.ws, self.hp, self.stream)
+        if self.tails:
+            mf.mfsdp_adamw_tail_step(self.desc, self.P, self.Gt, self.m1, self.v1,
+                                     mf.AdamWHParams(step=self.t, **self.wl.adamw), self.stream)
+
+    def time_steps(self, torch, steps, barrier):
+        n0 = self.mf.mfsdp_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.stream)
+        for _ in range(steps):
+            self.step()
+        e1.record(self.stream)
+        barrier()
+        return e0.elapsed_time(e1) / steps, self.mf.mfsdp_launch_count() - n0
+
+    def time_passes(self, torch, reps):
+        """Device time of each pass on its own (CUDA events on the launching stream).  The Newton-Schulz pass is the
+        dominant kernel; inside mfsdp_muon_step its last epilogue also applies the weight update when that is fused."""
+        mf, st = self.mf, self.stream
+        t = dict(mom=ev_time(torch, st, lambda: mf.mfsdp_muon_momentum_pass(self.desc, self.G, self.M, self.ws, self.hp, st), reps),
+                 ns=ev_time(torch, st, lambda: mf.mfsdp_muon_ns_pass(self.desc, self.ws, self.hp, st), reps),
+                 upd=ev_time(torch, st, lambda: mf.mfsdp_muon_update_pass(self.desc, self.W, self.ws, self.hp, st), reps),
+                 adam=ev_time(torch, st, lambda: mf.mfsdp_adamw_tail_step(
+                     self.desc, self.P, self.Gt, self.m1, self.v1, mf.AdamWHParams(step=self.t + 1, **self.wl.adamw), st),
+                     reps) if self.tails else 0.0)
+        return t
+
+    def byte_counts(self):
+        b_mom = sum(elementwise_bytes(d.rows, d.cols, self.wbytes)["mom"] for d in self.mats)
+        b_upd = sum(elementwise_bytes(d.rows, d.cols, self.wbytes)["upd"] for d in self.mats)
+        b_adam = sum(d.rows * d.cols for d in self.tails) * (3 * self.wbytes + 16)
+        return b_mom, b_upd, b_adam
+
+
+def passes_record(res, t, pk):
+    b_mom, b_upd, b_adam = res.byte_counts()
+    gbs = lambda b, ms: b / (ms * 1e-3) / 1e9 if ms else 0.0
+    return dict(momentum=dict(ms=t["mom"], gbs=gbs(b_mom, t["mom"]), frac_hbm=gbs(b_mom, t["mom"]) / pk["hbm"]),
+                update=dict(ms=t["upd"], gbs=gbs(b_upd, t["upd"]), frac_hbm=gbs(b_upd, t["upd"]) / pk["hbm"],
+                            note="separate pass; mfsdp_muon_step applies the update in the last NS epilogue when "
+                                 "the weights are bf16 and every cols % 8 == 0"),
+                adamw=dict(ms=t["adam"], gbs=gbs(b_adam, t["adam"])), ns=dict(ms=t["ns"]))
+
+
+def measure_other_config(torch, mf, name, pk, local, paper=False, reuse=None):
+    """One record of `other_configs`: the same step on another BASELINE.json config (or the paper's own setting on the
+    headline's resident set), timed long enough to be meaningful (>= 0.3 s or 200 steps), clocks sampled alongside."""
+    import workloads
+    if reuse is None:
+        wl = workloads.get(name)
+        res = Resident(mf, wl, choose_plan_rank(rank_order_by_load(mf, wl), wl.rank, 0, 1), pin=False)
+    else:
+        res = reuse
+    if paper:      # PAPER.md:121
+        res.set_hparams(dict(momentum=0.5, ns_steps=2, lr=1e-3, weight_decay=1e-2), dict(beta2=0.999))
+    for _ in range(3):
+        res.step()
+    torch.cuda.synchronize()
+    ms0, _ = res.time_steps(torch, 3, torch.cuda.synchronize)
+    steps = int(max(5, min(200, 0.3e3 / max(ms0, 1e-3))))
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms, launches = res.time_steps(torch, steps, torch.cuda.synchronize)
+    t = res.time_passes(torch, max(3, min(steps, 50)))
+    clocks = sampler.stop()
+    capped = "sw_power_cap" in clocks.get("reasons", [])
+    peak = pk["tc_sustained"] if capped else pk["tc_burst"]
+    ns_tf = res.f_alg / (t["ns"] * 1e-3) / 1e12
+    rec = dict(workload=res.wl.name + ("+paper_setting(mu0.5,K2)" if paper else ""), ms_per_step=ms, steps=steps,
+               ns_ms=t["ns"], ns_tflops_alg=ns_tf, ns_frac=ns_tf / peak,
+               ns_frac_of="sustained bf16 peak (sw_power_cap sampled)" if capped else "burst bf16 peak",
+               precision="bf16" if res.wl.precision == mf.NS_BF16 else "f32 (FFMA correctness mode)",
+               momentum_gbs=passes_record(res, t, pk)["momentum"]["gbs"], update_gbs=passes_record(res, t, pk)["update"]["gbs"],
+               launches_per_step=launches / steps, clocks=dict(sm_mhz=clocks.get("sm_mhz"), reasons=clocks.get("reasons")))
+    return rec
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -293,38 +463,8 @@ def run_ours(args):
     wl = apply_setting(workloads.get(args.config), args)
     order = rank_order_by_load(mf, wl)
     plan_rank = choose_plan_rank(order, wl.rank, rank, world)
-    pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, plan_rank)
-    desc = pr.desc
-    descs = [desc[i] for i in range(desc._n)]
-    mats = [d for d in descs if d.role == mf.ROLE_MATRIX]
-    tails = [d for d in descs if d.role == mf.ROLE_TAIL]
-    K = wl.muon["ns_steps"]
-    hp = mf.MuonHParams(precision=wl.precision, **wl.muon)
-    n_mat_el, n_tail_el = mf.mfsdp_flat_elems(desc)
-    tdt = workloads.TORCH_DTYPE[wl.dtype]
-    wbytes = 2 if wl.dtype == mf.BF16 else 4
-
-    # seeded inputs, generated on the host, resident in pinned memory (e2e leg) and copied to HBM (device leg)
-    hW = workloads.fill_flat(wl, descs, workloads.KIND_W, pin=True)
-    hG = workloads.fill_flat(wl, descs, workloads.KIND_G, step=0, pin=True)
-    hM = torch.zeros(max(n_mat_el, 1), dtype=torch.float32, pin_memory=True)[:n_mat_el]
-    W, G, M = hW.cuda(), hG.cuda(), torch.zeros(n_mat_el, dtype=torch.float32, device="cuda")
-    P = workloads.fill_flat(wl, descs, workloads.KIND_W, role=mf.ROLE_TAIL).cuda()
-    Gt = workloads.fill_flat(wl, descs, workloads.KIND_G, role=mf.ROLE_TAIL).cuda()
-    m1 = torch.zeros(n_tail_el, dtype=torch.float32, device="cuda")
-    v1 = torch.zeros(n_tail_el, dtype=torch.float32, device="cuda")
-    ws_bytes = mf.mfsdp_workspace_bytes(desc, wl.precision)
-    raw = torch.empty(ws_bytes + 1024, dtype=torch.uint8, device="cuda")
-    off = (-raw.data_ptr()) % 1024
-    ws = raw[off:off + ws_bytes]
-    stream = torch.cuda.current_stream()
-    tstep = [0]
-
-    def step():
-        tstep[0] += 1
-        mf.mfsdp_muon_step(desc, W, G, M, ws, hp, stream)
-        if tails:
-            mf.mfsdp_adamw_tail_step(desc, P, Gt, m1, v1, mf.AdamWHParams(step=tstep[0], **wl.adamw), stream)
+    res = Resident(mf, wl, plan_rank)
+    stream = res.stream
 
     def barrier():
         if world > 1:
@@ -332,52 +472,40 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     for _ in range(max(args.warmup, 3)):
-        step()
+        res.step()
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    n0 = mf.mfsdp_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        step()
-    e1.record(stream)
-    barrier()
-    launches = mf.mfsdp_launch_count() - n0
-    ms = e0.elapsed_time(e1) / args.steps
-
+    ms, launches = res.time_steps(torch, args.steps, barrier)
     # per-pass device times inside the same clock-sampled window (dominant kernel: the Newton-Schulz pass)
-    reps = max(3, min(args.steps, 10))
-    t_mom = ev_time(torch, stream, lambda: mf.mfsdp_muon_momentum_pass(desc, G, M, ws, hp, stream), reps)
-    t_ns = ev_time(torch, stream, lambda: mf.mfsdp_muon_ns_pass(desc, ws, hp, stream), reps)
-    t_upd = ev_time(torch, stream, lambda: mf.mfsdp_muon_update_pass(desc, W, ws, hp, stream), reps)
-    t_adam = ev_time(torch, stream, lambda: mf.mfsdp_adamw_tail_step(
-        desc, P, Gt, m1, v1, mf.AdamWHParams(step=tstep[0] + 1, **wl.adamw), stream), reps) if tails else 0.0
+    t = res.time_passes(torch, max(3, min(args.steps, 10)))
     clocks = sampler.stop()
 
     # e2e: the same step through the HOST-buffer C-ABI entry point (pinned host W, G, M up; W, M back), every step
     ms_e2e = 0.0
     if not args.no_e2e:
-        dW, dG, dM = torch.empty_like(W), torch.empty_like(G), torch.empty_like(M)
-        hM.zero_()
+        hM = torch.zeros(max(res.n_mat_el, 1), dtype=torch.float32, pin_memory=True)[:res.n_mat_el]
+        dW, dG, dM = torch.empty_like(res.W), torch.empty_like(res.G), torch.empty_like(res.M)
         n_e2e = max(2, min(args.steps, 3))
-        mf.mfsdp_muon_step_host(desc, hW, hG, hM, dW, dG, dM, 1, ws, hp, stream)
+        mf.mfsdp_muon_step_host(res.desc, res.hW, res.hG, hM, dW, dG, dM, 1, res.ws, res.hp, stream)
         barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0 = time.perf_counter()
         e0.record(stream)
         for _ in range(n_e2e):
-            mf.mfsdp_muon_step_host(desc, hW, hG, hM, dW, dG, dM, 1, ws, hp, stream)
+            mf.mfsdp_muon_step_host(res.desc, res.hW, res.hG, hM, dW, dG, dM, 1, res.ws, res.hp, stream)
         e1.record(stream)
         barrier()
         ms_e2e = max(e0.elapsed_time(e1), (time.perf_counter() - t0) * 1e3) / n_e2e
-        del dW, dG, dM
-    f_alg = sum(ns_flops(d.rows, d.cols, K)[0] for d in mats)
-    f_dense = sum(ns_flops(d.rows, d.cols, K)[1] for d in mats)
-    b_mom = sum(elementwise_bytes(d.rows, d.cols, wbytes)["mom"] for d in mats)
-    b_upd = sum(elementwise_bytes(d.rows, d.cols, wbytes)["upd"] for d in mats)
-    b_adam = sum(d.rows * d.cols for d in tails) * (3 * wbytes + 16)
+        del dW, dG, dM, hM
 
-    ms_all, ms_e2e_all, f_all, launches_all = reduce_over_ranks(ms, ms_e2e, f_alg, launches, world, "cuda")
+    ms_all, ms_e2e_all, f_all, launches_all = reduce_over_ranks(ms, ms_e2e, res.f_alg, launches, world, "cuda")
+    per_rank = [ms]
+    if world > 1:
+        every = [torch.zeros(2, dtype=torch.float64, device="cuda") for _ in range(world)]
+        dist.all_gather(every, torch.tensor([ms, float(plan_rank)], dtype=torch.float64, device="cuda"))
+        per_rank = [float(x[0].item()) for x in every]
+        ranks_run = [int(x[1].item()) for x in every]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -385,44 +513,88 @@ def run_ours(args):
 
     pk = peaks()
     value = f_all / (ms_all * 1e-3) / 1e12
-    ns_tflops = f_alg / (t_ns * 1e-3) / 1e12
+    ns_tflops = res.f_alg / (t["ns"] * 1e-3) / 1e12
+    cfg = workload_config(wl, res.ddicts, plan_rank)
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=ms_all, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16" if
-                wl.precision == mf.NS_BF16 else "f32", data="synthetic (seeded, workloads/)",
-                config=dict(workload=wl.name, plan_rank=plan_rank, matrices=len(mats), tails=len(tails),
-                            matrix_elems=int(n_mat_el), ns_steps=K, l2="inputs larger than L2" if
-                            n_mat_el * wbytes > 256e6 else "working set may fit L2 (not flushed)",
-                            ns_flops_alg=f_alg, ns_flops_dense=f_dense),
+                wl.precision == mf.NS_BF16 else "f32", data="synthetic (seeded, workloads/)", config=cfg,
                 gpu_launches=launches_all, clocks=clocks)
+    traffic, traffic_commit = ncu_traffic(wl.name)
+    min_bytes = sum(min_hbm_bytes(d.rows, d.cols, res.K) for d in res.mats)
     line["roofline"] = dict(bound="tensor", kernel="k_ns_tc (one launch per tile class walks all iterations and phases)",
                             achieved=ns_tflops, peak=pk["tc_sustained"], unit="TFLOP/s",
-                            frac=ns_tflops / pk["tc_sustained"], traffic=ncu_traffic(wl.name),
+                            frac=ns_tflops / pk["tc_sustained"], traffic=traffic, traffic_commit=traffic_commit,
+                            traffic_ratio=(traffic / min_bytes) if traffic else None, min_hbm_bytes=min_bytes,
                             peak_source=pk["src"] + ", sustained bf16", frac_of_burst=ns_tflops / pk["tc_burst"],
-                            dense_equiv_tflops=f_dense / (t_ns * 1e-3) / 1e12, ms=t_ns)
-    line["passes"] = dict(
-        momentum=dict(ms=t_mom, gbs=b_mom / (t_mom * 1e-3) / 1e9, frac_hbm=b_mom / (t_mom * 1e-3) / 1e9 / pk["hbm"]),
-        update=dict(ms=t_upd, gbs=b_upd / (t_upd * 1e-3) / 1e9, frac_hbm=b_upd / (t_upd * 1e-3) / 1e9 / pk["hbm"]),
-        adamw=dict(ms=t_adam, gbs=(b_adam / (t_adam * 1e-3) / 1e9) if t_adam else 0.0), ns=dict(ms=t_ns))
+                            dense_equiv_tflops=res.f_dense / (t["ns"] * 1e-3) / 1e12, ms=t["ns"])
+    line["passes"] = passes_record(res, t, pk)
+    if world > 1:
+        pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, 0)
+        planned = [pr.rank_load[r] for r in ranks_run]
+        line["per_rank"] = dict(plan_ranks=ranks_run, ms=per_rank,
+                                imbalance_measured=max(per_rank) * len(per_rank) / sum(per_rank),
+                                imbalance_planned=max(planned) * len(planned) / max(1, sum(planned)))
     if not args.no_e2e:
-        h2d = n_mat_el * (2 * wbytes + 4)
-        d2h = n_mat_el * (wbytes + 4)
+        h2d = res.n_mat_el * (2 * res.wbytes + 4)
+        d2h = res.n_mat_el * (res.wbytes + 4)
         line["e2e"] = dict(value=f_all / (ms_e2e_all * 1e-3) / 1e12, unit=UNIT, ms_per_step=ms_e2e_all,
                            h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                            api="mfsdp_muon_step_host (pinned host W, G, M)")
+    if world == 1 and not args.no_other_configs and args.config == "c5" and not args.paper_setting:
+        others = []
+        try:
+            others.append(measure_other_config(torch, mf, "c5", pk, local, paper=True, reuse=res))
+        except Exception as e:      # a failed side measurement must not lose the headline
+            others.append(dict(workload="c5+paper_setting", error=repr(e)))
+        del res
+        torch.cuda.empty_cache()
+        for name in ("c1", "c2", "c3", "c4"):
+            try:
+                others.append(measure_other_config(torch, mf, name, pk, local))
+            except Exception as e:
+                others.append(dict(workload=name, error=repr(e)))
+            torch.cuda.empty_cache()
+        line["other_configs"] = others
     if not args.no_cpu_baseline and world == 1:
-        sample = oracle_sample(wl, [d.as_dict() | dict(role=d.role) for d in descs])
+        desc_d = plan_for(wl, plan_rank)["desc"]
+        sample, skipped = oracle_sample(wl, desc_d)
         times, fa, cores = time_oracle(wl, sample, 1)
         line["cpu_baseline"] = dict(value=fa / times[0] / 1e12, unit=UNIT, cores=cores, kind="oracle",
-                                    sample=sample_text(sample), seconds=times[0])
+                                    sample=sample_text(wl, sample, skipped), seconds=times[0])
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without torch.distributed.run: start the N ranks here (one process per GPU, NCCL
+    only for the report), forward rank 0's JSON line.  The path has no data-path collective."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = []
+    for r in range(args.gpus):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(args.gpus), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env,
+                                      stdout=subprocess.PIPE if r == 0 else subprocess.DEVNULL, text=True))
+    out, _ = procs[0].communicate()
+    rc = procs[0].returncode
+    for p_ in procs[1:]:
+        rc = rc or p_.wait()
+    sys.stdout.write(out)
+    sys.stdout.flush()
+    if rc:
+        raise SystemExit(rc)
 
 
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     else:
         run_ours(args)
 
