@@ -183,7 +183,9 @@ int mfsdp_score_plan(const mfsdp_param_t* params, size_t n_params, int world_siz
 /* Owner-segment gradient-reduction schedule ("each rank contributes its local full-gradient buffer, but
  * the reduced result is written only to the nonempty owner segment"; "deterministic native send/recv
  * schedules ... Cross-rank validation checks that every rank derives the same deterministic schedule and segment sizes
- * before communication begins").  HOST, integers.  DESIGN.md reading F1: one reduce-to-owner per role (on one NVSwitch
+ * before communication begins").  The same records, in forward block order (reverse_blocks = 0), are the
+ * materialisation schedule: the owner of a role sends its segment to the W - 1 ranks that need the full parameter.
+ * HOST, integers.  DESIGN.md reading F1: one reduce-to-owner per role (on one NVSwitch
  * domain: ncclReduce with root = owner, or grouped send/recv), blocks in reverse model order when reverse_blocks != 0
  * (backward produces the last block first), roles of a block in parameter order.  Every rank calls this with the same
  * (params, world_size, owner) and compares *hash_out (FNV-1a 64 over the records) with its peers before it communicates;
@@ -281,6 +283,22 @@ int mfsdp_muon_step_gated(const mfsdp_desc_t* desc, size_t n_desc, void* W, cons
                           const uint32_t* ready, uint32_t epoch, void* cuda_stream);
 /* Stream-ordered 32-bit write ready[index] = epoch (cuStreamWriteValue32: no kernel, no SM). */
 int mfsdp_signal_ready(uint32_t* ready, size_t index, uint32_t epoch, void* cuda_stream);
+
+/* mfsdp_muon_step that also writes every updated matrix into a second destination: the single-GPU half of the owner
+ * fan-out ("ranks with nonempty segments send only those segments to the ranks that need the full parameter
+ * for the current FSDP unit; in the common matrix case this is an owner fanout").  The weight-update
+ * epilogue stores each 16-byte vector of the new W twice: into the owner's shard W and into fanout[i], the full-
+ * parameter buffer of matrix i (rows x cols, row-major, 16-byte aligned, dtype of W).  The destination is an ordinary
+ * device address as far as the kernels are concerned: a local buffer (what the tests use), peer memory mapped over
+ * NVLink, or an NVSwitch multicast address, in which case the one store reaches every peer and no separate collective
+ * follows the step.  (Mapping such memory is the caller's business; nothing here was measured on more than one GPU.)
+ *   fanout   HOST in.  one DEVICE pointer per MATRIX descriptor, in table order; NULL entries = no copy for that matrix.
+ * The transfer order for non-multicast fan-out is the forward-order schedule of mfsdp_reduce_schedule
+ * (reverse_blocks = 0); its per-block cost estimate is C_B^owner of mfsdp_score_plan.  Not CUDA-graph capturable (the
+ * destination table is copied from the host array on every call).  Bit-identical W to mfsdp_muon_step. */
+int mfsdp_muon_step_fanout(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
+                           void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,
+                           void* const* fanout, void* cuda_stream);
 
 /* Individual passes of the step, exposed so tests can check each kernel against the oracle and bench.py can time
  * them.  Same arguments and errors as mfsdp_muon_step.

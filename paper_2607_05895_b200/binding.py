@@ -90,7 +90,7 @@ class PlanResult:
     policy_used: int = -1
 
 
-_SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_reduce_schedule", "mfsdp_muon_step_gated",
+_SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_reduce_schedule", "mfsdp_muon_step_gated", "mfsdp_muon_step_fanout",
             "mfsdp_signal_ready", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
@@ -137,6 +137,7 @@ def load():
     lib.mfsdp_muon_step.argtypes = [pD, sz, vp, vp, vp, vp, sz, pMH, vp]
     lib.mfsdp_muon_step_gated.argtypes = [pD, sz, vp, vp, vp, vp, sz, pMH, vp, C.c_uint32, vp]
     lib.mfsdp_signal_ready.argtypes = [vp, sz, C.c_uint32, vp]
+    lib.mfsdp_muon_step_fanout.argtypes = [pD, sz, vp, vp, vp, vp, sz, pMH, C.POINTER(C.c_void_p), vp]
     lib.mfsdp_muon_momentum_pass.argtypes = [pD, sz, vp, vp, vp, sz, pMH, vp]
     lib.mfsdp_muon_ns_pass.argtypes = [pD, sz, vp, sz, pMH, vp]
     lib.mfsdp_muon_update_pass.argtypes = [pD, sz, vp, vp, sz, pMH, vp]
@@ -361,6 +362,16 @@ def mfsdp_muon_step_gated(desc, W, G, M, workspace, hp, ready, epoch, stream=Non
     arr, n = _dn(desc)
     _check(load().mfsdp_muon_step_gated(arr, n, _ptr(W), _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
                                         C.byref(hp), _ptr(ready), int(epoch), _stream(stream)), "mfsdp_muon_step_gated")
+
+
+def mfsdp_muon_step_fanout(desc, W, G, M, workspace, hp, fanout, stream=None):
+    """fanout: one entry per matrix descriptor -- a CUDA tensor (or int address) that receives the updated matrix, or
+    None."""
+    arr, n = _dn(desc)
+    ptrs = (C.c_void_p * max(1, len(fanout)))(*[None if t is None else (t if isinstance(t, int) else t.data_ptr())
+                                                for t in fanout])
+    _check(load().mfsdp_muon_step_fanout(arr, n, _ptr(W), _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
+                                         C.byref(hp), ptrs, _stream(stream)), "mfsdp_muon_step_fanout")
 
 
 def mfsdp_signal_ready(ready, index, epoch, stream=None):

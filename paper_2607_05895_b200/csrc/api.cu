@@ -33,7 +33,7 @@ uint32_t g_trace_cap = 0;
 void free_plan(Plan* pl) {
   if (!pl) return;
   cudaFree(pl->d_mats); cudaFree(pl->d_tails); cudaFree(pl->d_chunk_begin); cudaFree(pl->d_tail_chunk_begin);
-  cudaFree(pl->d_chunk_mat); cudaFree(pl->d_chunk_tail);
+  cudaFree(pl->d_chunk_mat); cudaFree(pl->d_chunk_tail); cudaFree(pl->d_fan);
   destroy_ns_tc(pl->tc);
   delete pl;
 }
@@ -176,7 +176,8 @@ int get_plan(const mfsdp_desc_t* desc, size_t n_desc, int precision, void* works
       (rc = upload(&pl->d_tails, lay.tails.data(), lay.tails.size())) ||
       (rc = upload(&pl->d_chunk_begin, cb.data(), cb.size())) ||
       (rc = upload(&pl->d_tail_chunk_begin, tcb.data(), tcb.size())) ||
-      (rc = upload(&pl->d_chunk_mat, cm.data(), cm.size())) || (rc = upload(&pl->d_chunk_tail, ct.data(), ct.size()))) {
+      (rc = upload(&pl->d_chunk_mat, cm.data(), cm.size())) || (rc = upload(&pl->d_chunk_tail, ct.data(), ct.size())) ||
+      (rc = upload(&pl->d_fan, static_cast<const uint64_t*>(nullptr), lay.mats.size()))) {
     free_plan(pl);
     return rc;
   }
@@ -294,8 +295,15 @@ extern "C" int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, v
 namespace {
 int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M, void* workspace,
                    size_t ws_bytes, const mfsdp_muon_hparams_t* hp, const uint32_t* ready, uint32_t epoch,
-                   void* cuda_stream);
+                   void* cuda_stream, void* const* fanout = nullptr);
 }  // namespace
+
+extern "C" int mfsdp_muon_step_fanout(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
+                                      void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,
+                                      void* const* fanout, void* cuda_stream) {
+  if (!fanout) return MFSDP_EINVAL;
+  return muon_step_impl(desc, n_desc, W, G, M, workspace, ws_bytes, hp, nullptr, 0u, cuda_stream, fanout);
+}
 
 extern "C" int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
                                void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
@@ -328,7 +336,7 @@ extern "C" int mfsdp_signal_ready(uint32_t* ready, size_t index, uint32_t epoch,
 namespace {
 int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M, void* workspace,
                    size_t ws_bytes, const mfsdp_muon_hparams_t* hp, const uint32_t* ready, uint32_t epoch,
-                   void* cuda_stream) {
+                   void* cuda_stream, void* const* fanout) {
   Plan* pl = nullptr;
   int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
   if (rc) return rc;
@@ -338,11 +346,24 @@ int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void*
   // Build every launch table of this call BEFORE the first kernel is enqueued: table building allocates and copies
   // synchronously, which must not happen behind a gated momentum kernel that waits for flags the host raises later.
   const bool fuse = hp->precision == MFSDP_NS_BF16 && ns_tc_can_fuse_update(*pl);
+  const uint64_t* fan = nullptr;
+  if (fanout) {                            // destination table -> device, in stream order (the host array is staged by
+    size_t k = 0;                          // the runtime before cudaMemcpyAsync returns: it may be a temporary)
+    std::vector<uint64_t> tbl(pl->lay.mats.size());
+    for (size_t i = 0; i < n_desc; ++i)
+      if (desc[i].role == MFSDP_ROLE_MATRIX) {
+        if (fanout[k] && !aligned(fanout[k], 16)) return MFSDP_EINVAL;
+        tbl[k] = reinterpret_cast<uint64_t>(fanout[k]); ++k;
+      }
+    const cudaError_t e = cudaMemcpyAsync(pl->d_fan, tbl.data(), tbl.size() * sizeof(uint64_t), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    fan = pl->d_fan;
+  }
   if ((rc = launch_momentum(*pl, G, M, *hp, st, ready, epoch))) return rc;
   if (fuse)                                                             // the update runs in the last APPLY epilogue
-    return launch_ns_tc(*pl, *hp, st, W, (hp->flags & MFSDP_STEP_KEEP_O) != 0);
+    return launch_ns_tc(*pl, *hp, st, W, (hp->flags & MFSDP_STEP_KEEP_O) != 0, fan);
   if ((rc = ns_dispatch(*pl, *hp, st))) return rc;
-  return launch_update(*pl, W, *hp, st);
+  return launch_update(*pl, W, *hp, st, fan);
 }
 }  // namespace
 

@@ -233,12 +233,14 @@ template <typename WT, typename OT>
 __global__ void __launch_bounds__(kEwThreads) k_update(const MatLayout* __restrict__ mats,
                                                        const uint32_t* __restrict__ chunk_mat, uint32_t n_chunks,
                                                        WT* __restrict__ W, const uint8_t* __restrict__ ws, int o_buf,
-                                                       double lr, float decay, int scale_mode) {
+                                                       double lr, float decay, int scale_mode,
+                                                       const uint64_t* __restrict__ fan) {
   for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
     const uint32_t mi = chunk_mat[c];
     const MatLayout L = mats[mi];
     const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
     WT* w = W + L.elem_off;
+    WT* f = fan ? reinterpret_cast<WT*>(fan[mi]) : nullptr;    // fan-out copy of the updated matrix (rows x cols), or none
     const OT* o = reinterpret_cast<const OT*>(ws + (o_buf ? L.x_off[1] : L.x_off[0]));
     const float coef = (float)(lr * mats[mi].scale[scale_mode]);   // lr s, rounded once
     const bool vec = (L.cols % 8u) == 0u;
@@ -258,6 +260,7 @@ __global__ void __launch_bounds__(kEwThreads) k_update(const MatLayout* __restri
 #pragma unroll
           for (int i = 0; i < 8; ++i) wv[v].v[i] = fmaf(-coef, ov[v].v[i], decay * wv[v].v[i]);
           store8(w + e0, wv[v]);
+          if (f) store8(f + e0, wv[v]);
         }
       }
     } else {
@@ -270,12 +273,15 @@ __global__ void __launch_bounds__(kEwThreads) k_update(const MatLayout* __restri
 #pragma unroll
           for (int i = 0; i < 8; ++i) wv.v[i] = fmaf(-coef, ov.v[i], decay * wv.v[i]);
           store8(w + e0, wv);
+          if (f) store8(f + e0, wv);
         } else {
           const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
           for (uint64_t e = e0; e < e1; ++e) {
             const uint64_t r = e / L.cols, col = e - r * L.cols;
             const float ov = load1(o + r * L.pitch_x + col);
-            store1(w + e, fmaf(-coef, ov, decay * load1(w + e)));
+            const float wn = fmaf(-coef, ov, decay * load1(w + e));
+            store1(w + e, wn);
+            if (f) store1(f + e, wn);
           }
         }
       }
@@ -380,7 +386,7 @@ int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hpa
   return check_last_launch();
 }
 
-int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaStream_t st) {
+int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaStream_t st, const uint64_t* fan) {
   const WsLayout& lay = pl.lay;
   const uint32_t n_mat = (uint32_t)lay.mats.size();
   if (n_mat == 0) return MFSDP_OK;
@@ -391,7 +397,7 @@ int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaS
   const bool wbf = lay.mat_dtype == MFSDP_BF16, obf = pl.precision == MFSDP_NS_BF16;
 #define UPD(WT, OT)                                                                                      \
   k_update<WT, OT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                 \
-                                                static_cast<WT*>(W), ws, o_buf, hp.lr, decay, hp.scale_mode)
+                                                static_cast<WT*>(W), ws, o_buf, hp.lr, decay, hp.scale_mode, fan)
   if (wbf && obf) UPD(__nv_bfloat16, __nv_bfloat16);
   else if (wbf) UPD(__nv_bfloat16, float);
   else if (obf) UPD(float, __nv_bfloat16);

@@ -67,6 +67,7 @@ struct Plan {
   uint32_t* d_tail_chunk_begin = nullptr;  // [n_tail + 1]
   uint32_t* d_chunk_mat = nullptr;         // [n_chunks] chunk -> matrix index
   uint32_t* d_chunk_tail = nullptr;        // [n_tail_chunks] chunk -> tail index
+  uint64_t* d_fan = nullptr;               // [n_mat] fan-out destination address per matrix (mfsdp_muon_step_fanout)
   NsTcPlan* tc = nullptr;
 };
 
@@ -76,11 +77,13 @@ int get_plan(const mfsdp_desc_t* desc, size_t n_desc, int precision, void* works
 // ---- kernels (host launchers); all return an MFSDP_* code ------------------------------------------------------
 int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hparams_t& hp, cudaStream_t st,
                     const uint32_t* ready = nullptr, uint32_t epoch = 0);   // ready != nullptr: gated per matrix
-int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaStream_t st);
+int launch_update(const Plan& pl, void* W, const mfsdp_muon_hparams_t& hp, cudaStream_t st,
+                  const uint64_t* fan = nullptr);   // fan != nullptr: device table of fan-out destinations (0 = none)
 int launch_adamw(const Plan& pl, void* P, const void* G, void* m, void* v, const mfsdp_adamw_hparams_t& hp,
                  cudaStream_t st);
 int launch_ns_fp32(const Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st);
-int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void* W = nullptr, bool keep_o = true);
+int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void* W = nullptr, bool keep_o = true,
+                 const uint64_t* fan = nullptr);
 bool ns_tc_can_fuse_update(Plan& pl);   // bf16 weights, every cols % 8 == 0: the update runs in the last APPLY epilogue
 void destroy_ns_tc(NsTcPlan* p);
 int ns_class(uint32_t rows, uint32_t cols);   // 0 whole-matrix kernel, 1 single-CTA tiles, 2 CTA-pair tiles

@@ -56,8 +56,8 @@ __device__ __forceinline__ uint32_t pack_bf16f(float lo, float hi) {
 
 // W <- fl(1 - lr wd) W - fl(lr s) O for this thread's 64 consecutive elements of one W row (bf16, 16-byte aligned),
 // O as stored (bf16 pairs in pk); columns at or beyond `n_valid` are left alone.  Same arithmetic as k_update.
-__device__ __forceinline__ void update_row64(__nv_bfloat16* wrow, uint32_t n_valid, const uint32_t (&pk)[32], float coef,
-                                             float decay) {
+__device__ __forceinline__ void update_row64(__nv_bfloat16* wrow, __nv_bfloat16* fan_row, uint32_t n_valid,
+                                             const uint32_t (&pk)[32], float coef, float decay) {
   uint4 wv[8];
 #pragma unroll
   for (int j = 0; j < 8; ++j)
@@ -74,6 +74,7 @@ __device__ __forceinline__ void update_row64(__nv_bfloat16* wrow, uint32_t n_val
         nw[i] = pack_bf16f(fmaf(-coef, o0, decay * w0), fmaf(-coef, o1, decay * w1));
       }
       *reinterpret_cast<uint4*>(wrow + 8 * j) = make_uint4(nw[0], nw[1], nw[2], nw[3]);
+      if (fan_row) *reinterpret_cast<uint4*>(fan_row + 8 * j) = make_uint4(nw[0], nw[1], nw[2], nw[3]);
     }
   }
 }
@@ -160,11 +161,12 @@ __global__ void __launch_bounds__(kThreadsF, 2) k_ns_fused(const FusedParams p) 
 
     // last iteration: the APPLY epilogue also updates W (this thread's rows of it) from the O values it holds
     float coef = 0.f;
-    __nv_bfloat16* wmat = nullptr;
+    __nv_bfloat16 *wmat = nullptr, *fmat = nullptr;          // the matrix in W, and its optional fan-out copy
     if (p.ua.W != nullptr) {
       const TcUpd* u = p.ua.upd + fm.mat;
       coef = (float)(p.ua.lr * u->scale[p.ua.scale_mode]);
       wmat = reinterpret_cast<__nv_bfloat16*>(p.ua.W) + u->elem_off;
+      if (p.ua.fan) fmat = reinterpret_cast<__nv_bfloat16*>(p.ua.fan[fm.mat]);
     }
 
     for (uint32_t it = 0; it < p.ns_steps; ++it) {
@@ -265,7 +267,8 @@ __global__ void __launch_bounds__(kThreadsF, 2) k_ns_fused(const FusedParams p) 
                 pk[j] = pack_bf16f(beta * __uint_as_float(v[2 * j]), beta * __uint_as_float(v[2 * j + 1]));
               st_row(x0 + cc * panel_bytes + r * 128u, sw, pk);
               if (upd && r < fm.rows && 64u * cc < fm.cols)
-                update_row64(wmat + (size_t)r * fm.cols + 64u * cc, fm.cols - 64u * cc, pk, coef, p.ua.decay);
+                update_row64(wmat + (size_t)r * fm.cols + 64u * cc, fmat ? fmat + (size_t)r * fm.cols + 64u * cc : nullptr,
+                             fm.cols - 64u * cc, pk, coef, p.ua.decay);
             }
           } else {
             for (uint32_t rb = 0; rb < n_rb; ++rb)
@@ -276,7 +279,9 @@ __global__ void __launch_bounds__(kThreadsF, 2) k_ns_fused(const FusedParams p) 
                   pk[j] = pack_bf16f(beta * __uint_as_float(v[2 * j]), beta * __uint_as_float(v[2 * j + 1]));
                 st_row(x0 + cc * panel_bytes + (rb * 128u + r) * 128u, sw, pk);
                 if (upd && rb * 128u + r < fm.rows && 64u * cc < fm.cols)
-                  update_row64(wmat + (size_t)(rb * 128u + r) * fm.cols + 64u * cc, fm.cols - 64u * cc, pk, coef, p.ua.decay);
+                  update_row64(wmat + (size_t)(rb * 128u + r) * fm.cols + 64u * cc,
+                               fmat ? fmat + (size_t)(rb * 128u + r) * fm.cols + 64u * cc : nullptr, fm.cols - 64u * cc, pk,
+                               coef, p.ua.decay);
               }
           }
           ptx::fence_async_smem();                           // generic-proxy writes -> the next UMMAs / the TMA store

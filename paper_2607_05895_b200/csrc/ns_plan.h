@@ -47,6 +47,7 @@ struct UpdArgs {                 // W == nullptr: no fused update (the pass only
   float decay;
   int scale_mode;
   uint32_t keep_o;               // also store O (tests, callers that consume the orthogonalised update)
+  const uint64_t* fan;           // optional: per matrix the address of a fan-out copy of the updated W (0 = none)
 };
 
 enum { kCounterWords = 4 };         // [0], [1] tile counters of the CTA-pair / single-CTA class, [2], [3] fused classes

@@ -471,10 +471,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
       const bool upd = p.ua.W != nullptr && t.phase == PH_APPLY && w.it + 1 == p.ns_steps;   // warp-uniform
       float coef = 0.f;
       uint64_t w_elem = 0;
+      __nv_bfloat16* fan_row = nullptr;                          // this thread's row of the fan-out copy of W, at t.n0
       if (upd) {
         const TcUpd* u = p.ua.upd + t.mat;
         coef = (float)(p.ua.lr * u->scale[p.ua.scale_mode]);           // lr s, rounded once (as k_update does)
         w_elem = u->elem_off;
+        const uint64_t fb = p.ua.fan ? p.ua.fan[t.mat] : 0ull;
+        if (fb) fan_row = reinterpret_cast<__nv_bfloat16*>(fb) + (size_t)r * c.out_cols + t.n0;
       }
       const uint32_t n_acc = t.nw > kBN ? 2u : 1u;
       const uint32_t acc0 = n_acc == 2 ? 0u : acc_next;
@@ -588,6 +591,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
                     nw[i] = pack_bf16(fmaf(-coef, o0, p.ua.decay * w0), fmaf(-coef, o1, p.ua.decay * w1));
                   }
                   *reinterpret_cast<uint4*>(wrow + 8 * j) = make_uint4(nw[0], nw[1], nw[2], nw[3]);
+                  if (fan_row) *reinterpret_cast<uint4*>(fan_row + 64 * cc + 8 * j) = make_uint4(nw[0], nw[1], nw[2], nw[3]);
                 }
               }
             }
@@ -913,7 +917,7 @@ bool ns_tc_can_fuse_update(Plan& pl) {
 
 // W != nullptr (and ns_tc_can_fuse_update): the last APPLY epilogue also applies the weight update; O is then stored
 // only when keep_o is set.
-int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void* W, bool keep_o) {
+int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void* W, bool keep_o, const uint64_t* fan) {
   if (pl.lay.mats.empty()) return MFSDP_OK;
   {
     std::lock_guard<std::mutex> lock(plan_mutex());     // two threads stepping the same table build it once
@@ -936,6 +940,7 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void
   p.ua.decay = (float)(1.0 - hp.lr * hp.weight_decay);
   p.ua.scale_mode = hp.scale_mode;
   p.ua.keep_o = keep_o ? 1u : 0u;
+  p.ua.fan = p.ua.W ? fan : nullptr;
   p.ns_steps = (uint32_t)hp.ns_steps;
   p.done = tc.d_counters + kCounterWords;
   {

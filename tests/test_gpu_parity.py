@@ -478,6 +478,37 @@ def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
             assert torch.equal(x, y)
 
 
+@pytest.mark.parametrize("wname", ["medium", "small", "fused", "c3"])
+def test_fanout_copy_of_the_updated_weights(wname):
+    """SURVEY 8(f) f2, single-GPU half: mfsdp_muon_step_fanout writes every updated matrix into its fan-out destination
+    from the same registers that update the owner's shard -- in the Newton-Schulz epilogue where the update is fused
+    (medium, c3, the whole-matrix class of `fused`), in k_update otherwise (small: odd column counts).  Every second
+    matrix gets no destination.  W is bit-identical to the plain step; destinations equal their W segment; skipped
+    destinations and the guard bands around each destination stay untouched."""
+    wl = workloads.get(wname)
+    a = gh.Session(wl)
+    a.load_grads(0)
+    a.muon_step()
+    b = gh.Session(wl)
+    b.load_grads(0)
+    guard = 64
+    bufs, fan = [], []
+    for i, d in enumerate(b.mats):
+        t = torch.full((d.rows * d.cols + 2 * guard,), -7.0, dtype=b.W.dtype, device="cuda")
+        bufs.append(t)
+        fan.append(None if i % 2 else t[guard:guard + d.rows * d.cols])
+    mf.mfsdp_muon_step_fanout(b.desc, b.W, b.G, b.M, b.ws, b.hp, fan)
+    torch.cuda.synchronize()
+    assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M)
+    for i, d in enumerate(b.mats):
+        n = d.rows * d.cols
+        assert bool((bufs[i][:guard] == -7.0).all()) and bool((bufs[i][guard + n:] == -7.0).all())
+        if i % 2:
+            assert bool((bufs[i] == -7.0).all())
+        else:
+            assert torch.equal(bufs[i][guard:guard + n], b.W[d.elem_off:d.elem_off + n])
+
+
 def test_host_buffer_entry_point():
     wl = workloads.small_ragged()
     a = gh.Session(wl)
