@@ -342,7 +342,7 @@ int mfsdp_debug_ws_offsets(const mfsdp_desc_t* desc, size_t n_desc, int precisio
 int mfsdp_release_plans(void);
 
 /* Which Newton-Schulz kernel class a rows x cols matrix runs in under MFSDP_NS_BF16 with the current knob values (HOST):
- * 0 = whole-matrix kernel (X, A, P stay on chip: the A / P workspace buffers of mfsdp_debug_ws_offsets are NOT written),
+ * 0 = a whole-matrix kernel (A and P stay on chip: the A / P workspace buffers of mfsdp_debug_ws_offsets are NOT written),
  * 1 = single-CTA tiles, 2 = CTA-pair tiles.  Negative code on rows == 0 or cols == 0. */
 int mfsdp_ns_class(uint32_t rows, uint32_t cols);
 
@@ -364,9 +364,12 @@ int mfsdp_ns_class(uint32_t rows, uint32_t cols);
  *   MFSDP_TUNE_FUSED_BELOW_D matrices with min(rows, cols) < value whose padded X fits 128 KB of shared memory run in
  *                           the whole-matrix kernel (one CTA keeps X, A and P on chip for all K iterations); 1 switches
  *                           that kernel off.  129
+ *   MFSDP_TUNE_FUSED2_BELOW_D matrices with 128 < min(rows, cols) < value (<= 257) and max(rows, cols) <= 512 run in
+ *                           the second whole-matrix kernel (one CTA keeps A and P on chip for all K iterations and
+ *                           streams X through shared memory); 1 switches that kernel off.  257
  * Returns MFSDP_EINVAL for an unknown knob or value < 1; mfsdp_get_tune returns the value or a negative code. */
 enum { MFSDP_TUNE_PAIR_MIN_D = 0, MFSDP_TUNE_SYM_BAND = 1, MFSDP_TUNE_SYM_BAND2 = 2, MFSDP_TUNE_RECT_GROUP = 3,
-       MFSDP_TUNE_WIDE_MIN_KB = 4, MFSDP_TUNE_FUSED_BELOW_D = 5, MFSDP_TUNE_COUNT_ = 6 };
+       MFSDP_TUNE_WIDE_MIN_KB = 4, MFSDP_TUNE_FUSED_BELOW_D = 5, MFSDP_TUNE_FUSED2_BELOW_D = 6, MFSDP_TUNE_COUNT_ = 7 };
 int mfsdp_tune(int knob, int value);
 int mfsdp_get_tune(int knob);
 

@@ -220,7 +220,7 @@ def mfsdp_launch_count():
     return int(load().mfsdp_launch_count())
 
 
-TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D = 0, 1, 2, 3, 4, 5
+TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D, TUNE_FUSED2_BELOW_D = 0, 1, 2, 3, 4, 5, 6
 
 
 def mfsdp_ns_class(rows, cols):

@@ -25,7 +25,7 @@ std::vector<std::vector<uint8_t>> g_plan_keys;
 constexpr size_t kMaxPlans = 1024;   // cached launch tables; beyond it get_plan fails loudly (MFSDP_ECACHE)
 
 // Scheduling knobs (mfsdp_tune): defaults only -- no environment variables, no other hidden state.
-std::atomic<int> g_tune[MFSDP_TUNE_COUNT_] = {{1024}, {16}, {8}, {4}, {8}, {129}};
+std::atomic<int> g_tune[MFSDP_TUNE_COUNT_] = {{1024}, {16}, {8}, {4}, {8}, {129}, {257}};
 
 unsigned long long* g_trace = nullptr;
 uint32_t g_trace_cap = 0;

@@ -50,23 +50,25 @@ struct UpdArgs {                 // W == nullptr: no fused update (the pass only
   const uint64_t* fan;           // optional: per matrix the address of a fan-out copy of the updated W (0 = none)
 };
 
-enum { kCounterWords = 4 };         // [0], [1] tile counters of the CTA-pair / single-CTA class, [2], [3] fused classes
+enum { kCounterWords = 5 };         // [0], [1] tile counters of the single-CTA / CTA-pair class, [2], [3], [4] fused classes
 
 struct NsTcPlan {
   CUtensorMap* d_tmaps = nullptr;   // TM_COUNT per matrix
   TcMat* d_mats = nullptr;
   TcTile* d_tiles[2] = {nullptr, nullptr};   // [kCG - 1]: the tiles of ONE iteration, GRAM then POLY then APPLY
   uint32_t n_tiles[2] = {0, 0};
-  FusedMat* d_fused[2] = {nullptr, nullptr}; // whole-matrix class: [0] padded X <= 64 KB (2 CTAs / SM), [1] <= 128 KB
-  uint32_t n_fused[2] = {0, 0};
+  // whole-matrix classes: [0] d <= 128, padded X <= 64 KB (2 CTAs / SM), [1] d <= 128, X <= 128 KB (ns_fused.cu);
+  // [2] 128 < d <= 256, A / P on chip, X streamed (ns_fused2.cu)
+  FusedMat* d_fused[3] = {nullptr, nullptr, nullptr};
+  uint32_t n_fused[3] = {0, 0, 0};
   TcUpd* d_upd = nullptr;
   bool upd_ok = false;              // bf16 weights and every cols % 8 == 0: the update can be fused into the epilogues
   uint32_t* d_counters = nullptr;   // kCounterWords work counters then [n_mat] completion reports; zeroed per pass
   uint32_t n_mat = 0;
   int sms = 148;
   int max_pairs = 74;               // co-resident CTA pairs
-  cudaStream_t side[3] = {nullptr, nullptr, nullptr};   // forked streams: the classes touch disjoint matrices
-  cudaEvent_t fork = nullptr, join[3] = {nullptr, nullptr, nullptr};
+  cudaStream_t side[4] = {nullptr, nullptr, nullptr, nullptr};   // forked streams: the classes touch disjoint matrices
+  cudaEvent_t fork = nullptr, join[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 // ns_fused.cu
@@ -74,6 +76,11 @@ int fused_setup();                                        // kernel attributes (
 int launch_ns_fused(const NsTcPlan& tc, int cls, uint8_t* ws, const float* inv_norm, const mfsdp_muon_hparams_t& hp,
                     const UpdArgs& ua, cudaStream_t st);
 bool fused_eligible(uint32_t rows, uint32_t cols, uint32_t below_d, FusedMat* out, int* cls);
+// ns_fused2.cu
+int fused2_setup();
+int launch_ns_fused2(const NsTcPlan& tc, const float* inv_norm, const mfsdp_muon_hparams_t& hp, const UpdArgs& ua,
+                     cudaStream_t st);
+bool fused2_eligible(uint32_t rows, uint32_t cols, uint32_t below_d, FusedMat* out);
 
 
 }  // namespace mfsdp

@@ -801,13 +801,15 @@ int build_tc_plan(Plan& pl) {
   const uint32_t fused_below_d = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_FUSED_BELOW_D));
   // class 0 = whole-matrix kernel (ns_fused.cu: small d, X resident in shared memory), 1 = single-CTA tiles, 2 = CTA pairs
   std::vector<uint32_t> cls(lay.mats.size());
-  std::vector<FusedMat> fused[2];
+  const uint32_t fused2_below_d = (uint32_t)std::max(1, tune_value(MFSDP_TUNE_FUSED2_BELOW_D));
+  std::vector<FusedMat> fused[3];
   for (uint32_t i : order) {                      // cost-sorted: the fused CTAs claim the expensive matrices first
     const MatLayout& L = lay.mats[i];
     FusedMat f;
     int fc = 0;
     cls[i] = (uint32_t)ns_class(L.rows, L.cols);
-    if (cls[i] == 0 && fused_eligible(L.rows, L.cols, fused_below_d, &f, &fc)) {
+    if (cls[i] == 0) {
+      if (!fused_eligible(L.rows, L.cols, fused_below_d, &f, &fc)) { fused2_eligible(L.rows, L.cols, fused2_below_d, &f); fc = 2; }
       f.mat = i;
       fused[fc].push_back(f);
     }
@@ -851,18 +853,18 @@ int build_tc_plan(Plan& pl) {
     }
     if ((rc = dev_upload(&tc->d_upd, upd))) return rc;
   }
-  for (int g = 0; g < 2; ++g) {
+  for (int g = 0; g < 3; ++g) {
     tc->n_fused[g] = (uint32_t)fused[g].size();
     if ((rc = dev_upload(&tc->d_fused[g], fused[g]))) return rc;
   }
-  if ((rc = fused_setup())) return rc;
+  if ((rc = fused_setup()) || (rc = fused2_setup())) return rc;
   tc->n_mat = (uint32_t)lay.mats.size();
   cudaDeviceGetAttribute(&tc->sms, cudaDevAttrMultiProcessorCount, pl.device);
   cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&tc->d_counters), (kCounterWords + (size_t)tc->n_mat) * sizeof(uint32_t));
   if (e != cudaSuccess) return cuda_fail(e);
   // the classes touch disjoint matrices: each runs on its own forked stream, joined before the pass returns
   if ((e = cudaEventCreateWithFlags(&tc->fork, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
-  for (int k = 0; k < 3; ++k) {
+  for (int k = 0; k < 4; ++k) {
     if ((e = cudaStreamCreateWithFlags(&tc->side[k], cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e);
     if ((e = cudaEventCreateWithFlags(&tc->join[k], cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
   }
@@ -894,15 +896,17 @@ int ns_class(uint32_t rows, uint32_t cols) {
   FusedMat f;
   int fc = 0;
   if (fused_eligible(rows, cols, (uint32_t)std::max(1, tune_value(MFSDP_TUNE_FUSED_BELOW_D)), &f, &fc)) return 0;
+  if (fused2_eligible(rows, cols, (uint32_t)std::max(1, tune_value(MFSDP_TUNE_FUSED2_BELOW_D)), &f)) return 0;
   return std::min(rows, cols) >= (uint32_t)std::max(1, tune_value(MFSDP_TUNE_PAIR_MIN_D)) ? 2 : 1;
 }
 
 void destroy_ns_tc(NsTcPlan* p) {
   if (!p) return;
   cudaFree(p->d_tmaps); cudaFree(p->d_mats); cudaFree(p->d_counters); cudaFree(p->d_upd);
-  for (int g = 0; g < 2; ++g) { cudaFree(p->d_tiles[g]); cudaFree(p->d_fused[g]); }
+  for (int g = 0; g < 2; ++g) cudaFree(p->d_tiles[g]);
+  for (int g = 0; g < 3; ++g) cudaFree(p->d_fused[g]);
   if (p->fork) cudaEventDestroy(p->fork);
-  for (int k = 0; k < 3; ++k) {
+  for (int k = 0; k < 4; ++k) {
     if (p->join[k]) cudaEventDestroy(p->join[k]);
     if (p->side[k]) cudaStreamDestroy(p->side[k]);
   }
@@ -952,13 +956,13 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void
   // and joined back.  The whole-matrix kernels go first: their CTAs leave the SMs after a few tens of microseconds and
   // the persistent tile kernels pick the SMs up as they become free (tiles are claimed dynamically, so CTAs that
   // start late simply claim later tiles).
-  struct Job { int kind; uint64_t work; };       // kind 0, 1 = fused class; 2 = single-CTA tiles; 3 = CTA-pair tiles
-  Job jobs[4];
+  struct Job { int kind; uint64_t work; };       // kind 0, 1, 2 = fused class; 3 = single-CTA tiles; 4 = CTA-pair tiles
+  Job jobs[5];
   int n_jobs = 0;
-  for (int c = 1; c >= 0; --c)
-    if (tc.n_fused[c]) jobs[n_jobs++] = Job{c, (uint64_t)tc.n_fused[c]};
+  for (int c = 2; c >= 0; --c)
+    if (tc.n_fused[c]) jobs[n_jobs++] = Job{c, (uint64_t)tc.n_fused[c] * (c == 2 ? 16u : 1u)};
   for (int g = 1; g >= 0; --g)
-    if (tc.n_tiles[g]) jobs[n_jobs++] = Job{2 + g, (uint64_t)tc.n_tiles[g] * p.ns_steps * 64};
+    if (tc.n_tiles[g]) jobs[n_jobs++] = Job{3 + g, (uint64_t)tc.n_tiles[g] * p.ns_steps * 64};
   if (n_jobs == 0) return MFSDP_OK;
   int main_job = 0;
   for (int j = 1; j < n_jobs; ++j)
@@ -975,8 +979,10 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void
     int rc = MFSDP_OK;
     if (jobs[j].kind < 2) {
       rc = launch_ns_fused(tc, jobs[j].kind, p.ws, p.inv_norm, hp, p.ua, js);
+    } else if (jobs[j].kind == 2) {
+      rc = launch_ns_fused2(tc, p.inv_norm, hp, p.ua, js);
     } else {
-      const int g = jobs[j].kind - 2;
+      const int g = jobs[j].kind - 3;
       p.tiles = tc.d_tiles[g];
       p.n_iter_tiles = tc.n_tiles[g];
       p.counter = tc.d_counters + g;

@@ -246,9 +246,9 @@ def test_step_entry_points_reject_bad_arguments_without_a_gpu():
 def test_tune_knobs_roundtrip_and_reject_bad_values():
     """mfsdp_tune / mfsdp_get_tune are host-only: defaults, round trip, error codes (no device needed)."""
     knobs = [mf.TUNE_PAIR_MIN_D, mf.TUNE_SYM_BAND, mf.TUNE_SYM_BAND2, mf.TUNE_RECT_GROUP, mf.TUNE_WIDE_MIN_KB,
-             mf.TUNE_FUSED_BELOW_D]
+             mf.TUNE_FUSED_BELOW_D, mf.TUNE_FUSED2_BELOW_D]
     old = [mf.mfsdp_get_tune(k) for k in knobs]
-    assert old == [1024, 16, 8, 4, 8, 129]         # the header's defaults; no environment variable can change them
+    assert old == [1024, 16, 8, 4, 8, 129, 257]         # the header's defaults; no environment variable can change them
     try:
         for k in knobs:
             mf.mfsdp_tune(k, 3)

@@ -30,13 +30,17 @@ def pair_min_d():
 
 @pytest.fixture
 def fused_below_d():
-    """Sets MFSDP_TUNE_FUSED_BELOW_D for one test (1 = whole-matrix kernel off) and restores the default."""
-    old = mf.mfsdp_get_tune(mf.TUNE_FUSED_BELOW_D)
+    """Sets MFSDP_TUNE_FUSED_BELOW_D / MFSDP_TUNE_FUSED2_BELOW_D for one test (1 = that whole-matrix kernel off) and
+    restores the defaults."""
+    old = mf.mfsdp_get_tune(mf.TUNE_FUSED_BELOW_D), mf.mfsdp_get_tune(mf.TUNE_FUSED2_BELOW_D)
 
-    def set_(v):
+    def set_(v, v2=None):
         mf.mfsdp_tune(mf.TUNE_FUSED_BELOW_D, v)
+        if v2 is not None:
+            mf.mfsdp_tune(mf.TUNE_FUSED2_BELOW_D, v2)
     yield set_
-    mf.mfsdp_tune(mf.TUNE_FUSED_BELOW_D, old)
+    mf.mfsdp_tune(mf.TUNE_FUSED_BELOW_D, old[0])
+    mf.mfsdp_tune(mf.TUNE_FUSED2_BELOW_D, old[1])
 
 
 def _o_bits(sess):
@@ -205,13 +209,14 @@ def test_edge_shapes(pair_min_d, precision, min_d):
         gh.check_matrix_against_oracle(sess, i, W_old[i], M_old[i])
 
 
-@pytest.mark.parametrize("below_d", [129, 65, 1])
-@pytest.mark.parametrize("wname", ["fused", "small", "edge"])
-def test_whole_matrix_class_bf16(fused_below_d, wname, below_d):
-    """The whole-matrix kernel (one CTA keeps X, A, P on chip for all K iterations) on every shape it accepts -- both
-    size classes, tall / wide, ragged d and n, K = 5 and the odd / even buffer choice of K = 2 -- against the oracle;
-    and the same sets with the class narrowed (d < 65) and switched off (everything on the tile kernel)."""
-    fused_below_d(below_d)
+@pytest.mark.parametrize("below_d,below_d2", [(129, 257), (65, 193), (1, 1)])
+@pytest.mark.parametrize("wname", ["fused", "fused2", "small", "medium", "edge"])
+def test_whole_matrix_class_bf16(fused_below_d, wname, below_d, below_d2):
+    """The whole-matrix kernels (one CTA per matrix for all K iterations: d <= 128 with X, A, P on chip; 128 < d <= 256
+    with A, P on chip and X streamed) on every shape they accept -- all size classes, tall / wide, ragged d and n,
+    K = 5 and the odd / even buffer choice of K = 2 -- against the oracle; and the same sets with the classes narrowed
+    (d < 65, d < 193) and switched off (everything on the tile kernel)."""
+    fused_below_d(below_d, below_d2)
     wl = workloads.get(wname)
     for K in (5, 2):
         sess, errs = _full_step_check(wl, precision=mf.NS_BF16, hp_over=dict(ns_steps=K))
@@ -251,7 +256,7 @@ def test_scale_invariance_power_of_two():
                 assert torch.equal(a, b)
 
 
-@pytest.mark.parametrize("wname,min_d", [("medium", 1), ("medium", 100000), ("c2", 0), ("c3", 0)])
+@pytest.mark.parametrize("wname,min_d", [("medium", 1), ("medium", 100000), ("c2", 0), ("c3", 0), ("fused2", 0)])
 def test_dependency_protocol_poison_stress(pair_min_d, wname, min_d):
     """The inter-CTA protocol of the tile kernel (epilogue: TMA stores performed -> fence.proxy.async.global ->
     red.release.gpu on the matrix' counter; scheduler: ld.acquire.gpu >= need -> publish; consumers: fence.proxy.async
@@ -406,7 +411,7 @@ def test_paper_setting_parity():
                 assert ulps.max() <= 1 and (ulps > 0).mean() <= 2e-3
 
 
-@pytest.mark.parametrize("wname", ["small", "medium", "fused", "c3"])
+@pytest.mark.parametrize("wname", ["small", "medium", "fused", "fused2", "c3"])
 def test_separate_passes_equal_fused_step(wname):
     """mfsdp_muon_step == momentum pass + NS pass + update pass, bit for bit -- also where the step applies the weight
     update inside the last Newton-Schulz epilogue (bf16 weights, every cols % 8 == 0: medium, c3) instead of running
@@ -478,7 +483,7 @@ def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
             assert torch.equal(x, y)
 
 
-@pytest.mark.parametrize("wname", ["medium", "small", "fused", "c3"])
+@pytest.mark.parametrize("wname", ["medium", "small", "fused", "fused2", "c3"])
 def test_fanout_copy_of_the_updated_weights(wname):
     """SURVEY 8(f) f2, single-GPU half: mfsdp_muon_step_fanout writes every updated matrix into its fan-out destination
     from the same registers that update the owner's shard -- in the Newton-Schulz epilogue where the update is fused

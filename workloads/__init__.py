@@ -135,6 +135,20 @@ def fused_shapes(seed=19, dtype=BF16, precision=NS_BF16):
     return Workload("fused_shapes", params, seed=seed, precision=precision, dtype=dtype, row_lognormal=True)
 
 
+def fused2_shapes(seed=23, dtype=BF16, precision=NS_BF16):
+    """Shapes of the second whole-matrix Newton-Schulz class (128 < min(rows, cols) <= 256, max <= 512; A and P on
+    chip, X streamed): the largest (256 x 512, 512 x 256), d = 192 (half-empty second row block), d and n that are
+    not multiples of 16 / 64 / 128, tall and wide twins, one APPLY chunk and several, and neighbours just outside the
+    class (256 x 520, 129 x 1024); every column count a multiple of 8, so that the weight update runs inside the
+    kernels' last epilogue."""
+    shapes = [(256, 512), (512, 256), (192, 384), (384, 192), (256, 256), (200, 504), (504, 200), (136, 136),
+              (255, 264), (264, 256), (129, 1024), (440, 144), (256, 520), (130, 136), (248, 392)]
+    params = [(i // 4, 2, r, c, dtype, 0) for i, (r, c) in enumerate(shapes)]
+    params += [(1, 1, 77, 1, dtype, 0)]
+    params.sort(key=lambda p: p[0])
+    return Workload("fused2_shapes", params, seed=seed, precision=precision, dtype=dtype, row_lognormal=True)
+
+
 def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
     """The paper's convergence model puts the 50,257 x 768 embedding and the untied LM head on Muon:
     a very tall matrix with an odd row count (GRAM k loop of 786 blocks) next to one ordinary matrix."""
@@ -143,7 +157,7 @@ def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
 
 
 CONFIGS = {"c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
-           "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes, "fused": fused_shapes,
+           "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes, "fused": fused_shapes, "fused2": fused2_shapes,
            "vocab": vocab_embedding}
 
 
