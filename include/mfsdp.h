@@ -314,9 +314,14 @@ int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, void* W, voi
 
 /* The same step with HOST buffers (pinned for overlap; pageable works, serialised by the driver): copies G (and W, M
  * when `upload_state` != 0) to the caller's device staging buffers dW/dG/dM (128-byte aligned), runs the step on
- * `cuda_stream`, copies W and M back and synchronises the stream before returning.  Two internal copy streams carry
- * the upload of W and the download of M underneath the Newton-Schulz pass; everything is ordered after the work
- * already queued on `cuda_stream`.  Used for the end-to-end measurement. */
+ * `cuda_stream`, copies W and M back and synchronises the stream before returning.  The resident set is cut into up
+ * to 8 groups of consecutive matrices which are pipelined over two internal copy streams and the caller's stream: the
+ * upload of group g + 1, the step of group g and the download of group g - 1 overlap (PCIe is full duplex; inside a
+ * group W rides in under Newton-Schulz and M goes out right after the momentum pass).  That needs one workspace slice
+ * per group: pass a workspace of mfsdp_host_workspace_bytes (a few KB more than mfsdp_workspace_bytes); with a smaller
+ * one the call still works, as a single group.  Everything is ordered after the work already queued on
+ * `cuda_stream`.  Results are bit-identical to mfsdp_muon_step.  Used for the end-to-end measurement. */
+int mfsdp_host_workspace_bytes(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t* bytes);
 int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, const void* hG, void* hM,
                          void* dW, void* dG, void* dM, int upload_state,
                          void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);

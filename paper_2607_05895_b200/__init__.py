@@ -12,7 +12,7 @@ from .binding import (  # noqa: F401
     MfsdpError, Param, Desc, MuonHParams, AdamWHParams, PlanResult,
     lib_path, load, exported_symbols,
     mfsdp_plan, mfsdp_plan_ex, mfsdp_score_plan, mfsdp_reduce_schedule, mfsdp_muon_step_gated, mfsdp_signal_ready, mfsdp_muon_step_fanout,
-    ReduceOp, Caps, RankScore, BlockScore, mfsdp_validate_desc, mfsdp_flat_elems, mfsdp_workspace_bytes, mfsdp_workspace_view,
+    ReduceOp, Caps, RankScore, BlockScore, mfsdp_validate_desc, mfsdp_flat_elems, mfsdp_workspace_bytes, mfsdp_host_workspace_bytes, mfsdp_workspace_view,
     mfsdp_debug_ws_offsets, mfsdp_muon_step, mfsdp_muon_momentum_pass, mfsdp_muon_ns_pass, mfsdp_muon_update_pass,
     mfsdp_muon_step_host, mfsdp_adamw_tail_step, mfsdp_strerror, mfsdp_version, mfsdp_launch_count,
     mfsdp_tune, mfsdp_get_tune, mfsdp_debug_trace, TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D, TUNE_FUSED2_BELOW_D, mfsdp_release_plans, mfsdp_ns_class,

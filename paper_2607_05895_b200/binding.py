@@ -93,7 +93,7 @@ class PlanResult:
 _SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_reduce_schedule", "mfsdp_muon_step_gated", "mfsdp_muon_step_fanout",
             "mfsdp_signal_ready", "mfsdp_validate_desc", "mfsdp_flat_elems", "mfsdp_workspace_bytes",
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
-            "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
+            "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_host_workspace_bytes", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
             "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
             "mfsdp_release_plans", "mfsdp_ns_class"]
 _lib = None
@@ -131,6 +131,7 @@ def load():
     lib.mfsdp_validate_desc.argtypes = [pD, sz]
     lib.mfsdp_flat_elems.argtypes = [pD, sz, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     lib.mfsdp_workspace_bytes.argtypes = [pD, sz, i32, psz]
+    lib.mfsdp_host_workspace_bytes.argtypes = [pD, sz, i32, psz]
     lib.mfsdp_workspace_view.argtypes = [pD, sz, i32, i32, sz, psz, psz, psz]
     lib.mfsdp_debug_ws_offsets.argtypes = [pD, sz, i32, sz, psz]
     pMH, pAH = C.POINTER(MuonHParams), C.POINTER(AdamWHParams)
@@ -331,6 +332,13 @@ def mfsdp_workspace_bytes(desc, precision=NS_BF16):
     arr, n = _dn(desc)
     out = C.c_size_t(0)
     _check(load().mfsdp_workspace_bytes(arr, n, precision, C.byref(out)), "mfsdp_workspace_bytes")
+    return out.value
+
+
+def mfsdp_host_workspace_bytes(desc, precision=NS_BF16):
+    arr, n = _dn(desc)
+    out = C.c_size_t(0)
+    _check(load().mfsdp_host_workspace_bytes(arr, n, precision, C.byref(out)), "mfsdp_host_workspace_bytes")
     return out.value
 
 

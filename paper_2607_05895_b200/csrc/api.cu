@@ -369,11 +369,16 @@ int muon_step_impl(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void*
 
 namespace mfsdp {
 namespace {
-// Copy engines of mfsdp_muon_step_host: one stream per direction next to the caller's compute stream, so that the
-// uploads of W and the download of M run under the Newton-Schulz pass (PCIe is full duplex).
+// mfsdp_muon_step_host: the resident set is cut into up to kHostGroups groups of consecutive matrices of about equal
+// bytes, and the groups are pipelined over three streams: uploads (G, M, then W of group g) on `in`, the step of group
+// g on the caller's stream as soon as its G and M have landed (the weight update, which is the only consumer of W,
+// waits for W), downloads (M after the momentum pass, W after the update) on `out`.  PCIe is full duplex, so in steady
+// state the upload of group g + 1, the compute of group g and the download of group g - 1 overlap.
+constexpr int kHostGroups = 8;
 struct HostPipe {
   cudaStream_t in = nullptr, out = nullptr;
-  cudaEvent_t start = nullptr, gm_in = nullptr, w_in = nullptr, mom = nullptr, m_out = nullptr;
+  cudaEvent_t start = nullptr, fin = nullptr;
+  cudaEvent_t gm_in[kHostGroups], w_in[kHostGroups], mom[kHostGroups], done[kHostGroups];
   int device = -1;
 };
 std::map<int, HostPipe> g_pipes;         // one per device, created on first use (guarded by g_host_mu)
@@ -387,7 +392,8 @@ int host_pipe(HostPipe** out) {
     if ((e = cudaStreamCreateWithFlags(&p.in, cudaStreamNonBlocking)) != cudaSuccess ||
         (e = cudaStreamCreateWithFlags(&p.out, cudaStreamNonBlocking)) != cudaSuccess)
       return cuda_fail(e);
-    cudaEvent_t* evs[5] = {&p.start, &p.gm_in, &p.w_in, &p.mom, &p.m_out};
+    std::vector<cudaEvent_t*> evs = {&p.start, &p.fin};
+    for (int g = 0; g < kHostGroups; ++g) { evs.push_back(&p.gm_in[g]); evs.push_back(&p.w_in[g]); evs.push_back(&p.mom[g]); evs.push_back(&p.done[g]); }
     for (cudaEvent_t* ev : evs)
       if ((e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e);
     p.device = dev;
@@ -396,23 +402,94 @@ int host_pipe(HostPipe** out) {
   *out = &g_pipe;
   return MFSDP_OK;
 }
+
+struct HostGroup {
+  std::vector<mfsdp_desc_t> desc;   // the group's matrix descriptors (original element offsets)
+  uint64_t e0 = 0, e1 = 0;          // element range [e0, e1) of the rank-flat buffers this group covers
+  size_t ws_off = 0, ws_bytes = 0;  // its slice of the workspace
+};
+
+// Groups of consecutive matrix descriptors with about equal element counts; *total_ws = workspace they need together.
+int host_groups(const mfsdp_desc_t* desc, size_t n_desc, int precision, std::vector<HostGroup>& groups, size_t* total_ws) {
+  groups.clear();
+  std::vector<const mfsdp_desc_t*> mats;
+  uint64_t total = 0;
+  for (size_t i = 0; i < n_desc; ++i)
+    if (desc[i].role == MFSDP_ROLE_MATRIX) { mats.push_back(&desc[i]); total += (uint64_t)desc[i].rows * desc[i].cols; }
+  uint64_t flat = 0;
+  int rc = mfsdp_flat_elems(desc, n_desc, &flat, nullptr);
+  if (rc) return rc;
+  const int want = (int)std::min<size_t>(kHostGroups, mats.size());
+  uint64_t acc = 0;
+  for (size_t i = 0; i < mats.size(); ++i) {
+    if (groups.empty() || (acc * (uint64_t)want >= total * groups.size() && (int)groups.size() < want)) {
+      groups.emplace_back();
+      groups.back().e0 = mats[i]->elem_off;
+    }
+    groups.back().desc.push_back(*mats[i]);
+    acc += (uint64_t)mats[i]->rows * mats[i]->cols;
+  }
+  size_t off = 0;
+  for (size_t g = 0; g < groups.size(); ++g) {
+    groups[g].e1 = g + 1 < groups.size() ? groups[g + 1].e0 : flat;
+    WsLayout lay;
+    if ((rc = build_ws_layout(groups[g].desc.data(), groups[g].desc.size(), precision, lay))) return rc;
+    groups[g].ws_off = off;
+    groups[g].ws_bytes = (size_t)align_up_u64(lay.total_bytes, kBufAlign);
+    off += groups[g].ws_bytes;
+  }
+  if (total_ws) *total_ws = off;
+  return MFSDP_OK;
+}
 }  // namespace
 }  // namespace mfsdp
+
+extern "C" int mfsdp_host_workspace_bytes(const mfsdp_desc_t* desc, size_t n_desc, int precision, size_t* bytes) {
+  if (!bytes || (n_desc && !desc)) return MFSDP_EINVAL;
+  std::vector<HostGroup> groups;
+  size_t grouped = 0, plain = 0;
+  int rc = host_groups(desc, n_desc, precision, groups, &grouped);
+  if (rc) return rc;
+  if ((rc = mfsdp_workspace_bytes(desc, n_desc, precision, &plain))) return rc;
+  *bytes = std::max(grouped, plain);
+  return MFSDP_OK;
+}
 
 extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, const void* hG, void* hM,
                                     void* dW, void* dG, void* dM, int upload_state, void* workspace,
                                     size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream) {
-  Plan* pl = nullptr;
-  int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &pl);
+  Plan* full = nullptr;
+  int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &full);
   if (rc) return rc;
-  if (!pl || pl->lay.mats.empty()) return MFSDP_OK;
+  if (!full || full->lay.mats.empty()) return MFSDP_OK;
   if (!hW || !hG || !hM || !dW || !dG || !dM) return MFSDP_EINVAL;
   if (!aligned(dW, 128) || !aligned(dG, 128) || !aligned(dM, 128)) return MFSDP_EINVAL;
-  uint64_t elems = 0;
-  if ((rc = mfsdp_flat_elems(desc, n_desc, &elems, nullptr))) return rc;
-  const size_t es = pl->lay.mat_dtype == MFSDP_BF16 ? 2 : 4;
+  const size_t es = full->lay.mat_dtype == MFSDP_BF16 ? 2 : 4;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   std::lock_guard<std::mutex> lock(g_host_mu);
+
+  // groups and their plans (launch tables are built here, before anything is enqueued)
+  std::vector<HostGroup> groups;
+  size_t need = 0;
+  if ((rc = host_groups(desc, n_desc, hp->precision, groups, &need))) return rc;
+  std::vector<Plan*> plans;
+  if (need <= ws_bytes && groups.size() > 1) {
+    for (HostGroup& g : groups) {
+      Plan* pl = nullptr;
+      if ((rc = get_plan(g.desc.data(), g.desc.size(), hp->precision, static_cast<uint8_t*>(workspace) + g.ws_off, true, &pl)))
+        return rc;
+      plans.push_back(pl);
+    }
+  } else {                                   // workspace sized for the plain step only: one group, the whole table
+    uint64_t flat = 0;
+    if ((rc = mfsdp_flat_elems(desc, n_desc, &flat, nullptr))) return rc;
+    groups.assign(1, HostGroup());
+    groups[0].e0 = 0; groups[0].e1 = flat;
+    plans.assign(1, full);
+  }
+  if (hp->precision == MFSDP_NS_BF16)
+    for (Plan* pl : plans) ns_tc_can_fuse_update(*pl);     // builds the tensor-core tables now
+
   HostPipe* hpipe = nullptr;
   if ((rc = host_pipe(&hpipe))) return rc;
   HostPipe& q = *hpipe;
@@ -421,27 +498,40 @@ extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, voi
   // three streams before returning, so that the caller may free or reuse them.
   auto bail = [&](int code) { cudaStreamSynchronize(q.in); cudaStreamSynchronize(q.out); cudaStreamSynchronize(st); return code; };
 #define MFSDP_TRY(call) do { if ((e = (call)) != cudaSuccess) return bail(cuda_fail(e)); } while (0)
-  // in:  G, M (needed by the momentum pass), then W (needed only by the update pass: rides under Newton-Schulz)
+  uint8_t *hWb = static_cast<uint8_t*>(hW), *hMb = static_cast<uint8_t*>(hM), *dWb = static_cast<uint8_t*>(dW),
+          *dGb = static_cast<uint8_t*>(dG), *dMb = static_cast<uint8_t*>(dM);
+  const uint8_t* hGb = static_cast<const uint8_t*>(hG);
   MFSDP_TRY(cudaEventRecord(q.start, st));
   MFSDP_TRY(cudaStreamWaitEvent(q.in, q.start, 0));
-  MFSDP_TRY(cudaMemcpyAsync(dG, hG, elems * es, cudaMemcpyHostToDevice, q.in));
-  if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dM, hM, elems * 4, cudaMemcpyHostToDevice, q.in));
-  MFSDP_TRY(cudaEventRecord(q.gm_in, q.in));
-  if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dW, hW, elems * es, cudaMemcpyHostToDevice, q.in));
-  MFSDP_TRY(cudaEventRecord(q.w_in, q.in));
-  // compute on the caller's stream
-  MFSDP_TRY(cudaStreamWaitEvent(st, q.gm_in, 0));
-  if ((rc = launch_momentum(*pl, dG, dM, *hp, st))) return bail(rc);
-  MFSDP_TRY(cudaEventRecord(q.mom, st));
-  // out: M is final after the momentum pass: its download rides under Newton-Schulz too
-  MFSDP_TRY(cudaStreamWaitEvent(q.out, q.mom, 0));
-  MFSDP_TRY(cudaMemcpyAsync(hM, dM, elems * 4, cudaMemcpyDeviceToHost, q.out));
-  MFSDP_TRY(cudaEventRecord(q.m_out, q.out));
-  if ((rc = ns_dispatch(*pl, *hp, st))) return bail(rc);
-  MFSDP_TRY(cudaStreamWaitEvent(st, q.w_in, 0));
-  if ((rc = launch_update(*pl, dW, *hp, st))) return bail(rc);
-  MFSDP_TRY(cudaMemcpyAsync(hW, dW, elems * es, cudaMemcpyDeviceToHost, st));
-  MFSDP_TRY(cudaStreamWaitEvent(st, q.m_out, 0));
+  MFSDP_TRY(cudaStreamWaitEvent(q.out, q.start, 0));
+  const size_t ng = groups.size();
+  for (size_t g = 0; g < ng; ++g) {          // in: G, M of the group (momentum pass), then W (update pass only)
+    const uint64_t e0 = groups[g].e0, n = groups[g].e1 - groups[g].e0;
+    MFSDP_TRY(cudaMemcpyAsync(dGb + e0 * es, hGb + e0 * es, n * es, cudaMemcpyHostToDevice, q.in));
+    if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dMb + e0 * 4, hMb + e0 * 4, n * 4, cudaMemcpyHostToDevice, q.in));
+    MFSDP_TRY(cudaEventRecord(q.gm_in[g], q.in));
+    if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dWb + e0 * es, hWb + e0 * es, n * es, cudaMemcpyHostToDevice, q.in));
+    MFSDP_TRY(cudaEventRecord(q.w_in[g], q.in));
+  }
+  for (size_t g = 0; g < ng; ++g) {
+    const uint64_t e0 = groups[g].e0, n = groups[g].e1 - groups[g].e0;
+    Plan& pl = *plans[g];
+    // compute on the caller's stream
+    MFSDP_TRY(cudaStreamWaitEvent(st, q.gm_in[g], 0));
+    if ((rc = launch_momentum(pl, dG, dM, *hp, st))) return bail(rc);
+    MFSDP_TRY(cudaEventRecord(q.mom[g], st));
+    if ((rc = ns_dispatch(pl, *hp, st))) return bail(rc);
+    MFSDP_TRY(cudaStreamWaitEvent(st, q.w_in[g], 0));
+    if ((rc = launch_update(pl, dW, *hp, st))) return bail(rc);
+    MFSDP_TRY(cudaEventRecord(q.done[g], st));
+    // out: M is final after the momentum pass, W after the update
+    MFSDP_TRY(cudaStreamWaitEvent(q.out, q.mom[g], 0));
+    MFSDP_TRY(cudaMemcpyAsync(hMb + e0 * 4, dMb + e0 * 4, n * 4, cudaMemcpyDeviceToHost, q.out));
+    MFSDP_TRY(cudaStreamWaitEvent(q.out, q.done[g], 0));
+    MFSDP_TRY(cudaMemcpyAsync(hWb + e0 * es, dWb + e0 * es, n * es, cudaMemcpyDeviceToHost, q.out));
+  }
+  MFSDP_TRY(cudaEventRecord(q.fin, q.out));
+  MFSDP_TRY(cudaStreamWaitEvent(st, q.fin, 0));
   MFSDP_TRY(cudaStreamSynchronize(st));
 #undef MFSDP_TRY
   return MFSDP_OK;

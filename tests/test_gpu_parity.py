@@ -514,16 +514,25 @@ def test_fanout_copy_of_the_updated_weights(wname):
             assert torch.equal(bufs[i][guard:guard + n], b.W[d.elem_off:d.elem_off + n])
 
 
-def test_host_buffer_entry_point():
-    wl = workloads.small_ragged()
+@pytest.mark.parametrize("wname", ["small", "medium", "fused2"])
+@pytest.mark.parametrize("grouped", [False, True])
+def test_host_buffer_entry_point(wname, grouped):
+    """mfsdp_muon_step_host (pinned host W, G, M in; W, M out) == mfsdp_muon_step, bit for bit: with a workspace of
+    mfsdp_workspace_bytes (one group) and with one of mfsdp_host_workspace_bytes (the resident set pipelined in up to 8
+    groups: upload of group g + 1, step of group g, download of group g - 1 overlap), two consecutive steps."""
+    wl = workloads.get(wname)
     a = gh.Session(wl)
-    a.load_grads(0)
-    hW, hG = a.hW.clone().pin_memory(), a.hG.clone().pin_memory()
+    hW = a.hW.clone().pin_memory()
     hM = torch.zeros(a.n_mat_el, dtype=torch.float32).pin_memory()
-    dW, dG, dM = torch.empty_like(a.W), torch.empty_like(a.G), torch.empty_like(a.M)
-    mf.mfsdp_muon_step_host(a.desc, hW, hG, hM, dW, dG, dM, 1, a.ws, a.hp)
-    a.muon_step()
-    assert torch.equal(hW, a.W.cpu()) and torch.equal(hM, a.M.cpu())
+    dW, dG, dM = torch.empty_like(a.W), torch.empty_like(a.W), torch.empty_like(a.M)
+    ws = gh.aligned_bytes(mf.mfsdp_host_workspace_bytes(a.desc, a.precision)) if grouped else a.ws
+    assert ws.numel() >= a.ws.numel()
+    for step in range(2):
+        a.load_grads(step)
+        hG = a.hG.clone().pin_memory()
+        mf.mfsdp_muon_step_host(a.desc, hW, hG, hM, dW, dG, dM, 1, ws, a.hp)
+        a.muon_step()
+        assert torch.equal(hW, a.W.cpu()) and torch.equal(hM, a.M.cpu())
 
 
 def test_launch_counter_counts_kernels():
