@@ -60,6 +60,15 @@ __device__ __forceinline__ F8 load8_ro(const __nv_bfloat16* p) {
   }
   return r;
 }
+__device__ __forceinline__ void store8_cs(__nv_bfloat16* p, const F8& x) {
+  uint32_t w[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const __nv_bfloat162 h = __floats2bfloat162_rn(x.v[2 * i], x.v[2 * i + 1]);   // RNE
+    w[i] = *reinterpret_cast<const uint32_t*>(&h);
+  }
+  __stcs(reinterpret_cast<uint4*>(p), make_uint4(w[0], w[1], w[2], w[3]));
+}
 // L2-only loads (gated pass: the gradient is written by another agent -- copy engine, peer GPU -- while this kernel runs)
 __device__ __forceinline__ F8 load8_cg(const float* p) {
   F8 r;
@@ -86,6 +95,18 @@ __device__ __forceinline__ float load1_cg(const __nv_bfloat16* p) {
 __device__ __forceinline__ void store8(float* p, const F8& x) {
   *reinterpret_cast<float4*>(p) = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]);
   *reinterpret_cast<float4*>(p + 4) = make_float4(x.v[4], x.v[5], x.v[6], x.v[7]);
+}
+// streaming (evict-first) forms for data that is touched exactly once per pass
+__device__ __forceinline__ F8 load8_cs(const float* p) {
+  F8 r;
+  const float4 a = __ldcs(reinterpret_cast<const float4*>(p));
+  const float4 b = __ldcs(reinterpret_cast<const float4*>(p + 4));
+  r.v[0] = a.x; r.v[1] = a.y; r.v[2] = a.z; r.v[3] = a.w; r.v[4] = b.x; r.v[5] = b.y; r.v[6] = b.z; r.v[7] = b.w;
+  return r;
+}
+__device__ __forceinline__ void store8_cs(float* p, const F8& x) {
+  __stcs(reinterpret_cast<float4*>(p), make_float4(x.v[0], x.v[1], x.v[2], x.v[3]));
+  __stcs(reinterpret_cast<float4*>(p + 4), make_float4(x.v[4], x.v[5], x.v[6], x.v[7]));
 }
 __device__ __forceinline__ void store8(__nv_bfloat16* p, const F8& x) {
   uint32_t w[4];
@@ -157,7 +178,7 @@ __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __rest
         for (int v = 0; v < kBatch; ++v) {
           const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
           gv[v] = kGated ? load8_cg(g + e0) : load8_ro(g + e0);
-          mv[v] = load8(m + e0);
+          mv[v] = load8_cs(m + e0);
         }
 #pragma unroll
         for (int v = 0; v < kBatch; ++v) {
@@ -170,8 +191,8 @@ __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __rest
             uv.v[i] = nesterov ? fmaf(mu, mv[v].v[i], gs) : mv[v].v[i];  // U = (1-mu) G + mu M   |   U = M
             acc = fma((double)uv.v[i], (double)uv.v[i], acc);
           }
-          store8(m + e0, mv[v]);
-          store8(x + e0, uv);
+          store8_cs(m + e0, mv[v]);        // M is touched once per step: evict-first
+          store8(x + e0, uv);              // X~ is the next kernel's input: keep it in L2 (small sets fit)
         }
       }
     } else {                                   // ragged chunk or odd pitch: same element -> thread mapping, guarded
