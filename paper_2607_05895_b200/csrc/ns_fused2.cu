@@ -4,8 +4,9 @@
 // too large to stay (256 x 512 bf16 = 256 KB) and streams through a 2 x 32 KB TMA ring from the L2-resident ping-pong
 // buffers: once for GRAM, once for APPLY per iteration, while X_new goes out through TMA stores.  Compared with the
 // tile kernel (ns_tc.cu) on such matrices: no gpu-scope dependency counters, no tile feed, A and P never round-trip
-// through global memory, and X is read twice per iteration instead of once per output tile -- the single-CTA tiles
-// there are bound by the L2 -> SM path (48 KB per 64-k block per 128 x 256 tile against ~48 B/clk/SM).
+// through global memory, and X is read twice per iteration instead of once per output tile.  (The single-CTA tiles
+// there are bound by the instruction issue of their producer and UMMA threads -- ~650 and ~520 cycles per 64-k block
+// for 6 TMA loads and 4 UMMAs of 128 cycles -- and by one exposed load latency per tile: DESIGN.md section 9.)
 //
 // Per iteration (same arithmetic and rounding points as ns_tc.cu; Y = X for wide, X^T for tall matrices):
 //   GRAM   A = alpha Y Y^T     two row blocks of 128, accumulators 2 x 256 TMEM columns; k streams in 64-blocks
