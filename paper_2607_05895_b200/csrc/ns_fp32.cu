@@ -8,9 +8,9 @@
 namespace mfsdp {
 namespace {
 
-constexpr int kT = 64;    // output tile
 constexpr int kK = 32;    // k slab
-constexpr int kPer = kT * kK / 256;   // slab elements per thread and operand
+// Output tile kT x kT per CTA of 256 threads (thread = kT/16 x kT/16 outputs): 64 for throughput, 32 when the whole
+// set has so few 64-tiles that most SMs would idle (BASELINE config 1: 2 matrices, 16-64 tiles per phase).
 
 enum { PH_GRAM = 0, PH_POLY = 1, PH_APPLY = 2 };
 
@@ -22,7 +22,10 @@ struct NsArgs {
   float a, b, c;
 };
 
+template <int kT>
 __global__ void __launch_bounds__(256) k_ns_fp32(NsArgs g) {
+  constexpr int kPer = kT * kK / 256;   // slab elements per thread and operand
+  constexpr int kR = kT / 16;           // outputs per thread and dimension
   const MatLayout L = g.mats[blockIdx.y];
   const uint32_t d = L.d, n = L.n_long;
   const uint32_t Mo = d, No = (g.phase == PH_APPLY) ? n : d, Kd = (g.phase == PH_GRAM) ? n : d;
@@ -71,7 +74,7 @@ __global__ void __launch_bounds__(256) k_ns_fp32(NsArgs g) {
       sB[bk][bm] = rb[r];
     }
   };
-  float acc[4][4] = {};
+  float acc[kR][kR] = {};
   fetch(0);
   for (uint32_t k0 = 0; k0 < Kd; k0 += kK) {
     stash();
@@ -79,23 +82,23 @@ __global__ void __launch_bounds__(256) k_ns_fp32(NsArgs g) {
     if (k0 + kK < Kd) fetch(k0 + kK);        // next slab in flight (registers) while this one is multiplied
 #pragma unroll
     for (int kk = 0; kk < kK; ++kk) {
-      float av[4], bv[4];
+      float av[kR], bv[kR];
 #pragma unroll
-      for (int r = 0; r < 4; ++r) { av[r] = sA[kk][ty * 4 + r]; bv[r] = sB[kk][tx * 4 + r]; }
+      for (int r = 0; r < kR; ++r) { av[r] = sA[kk][ty * kR + r]; bv[r] = sB[kk][tx * kR + r]; }
 #pragma unroll
-      for (int r = 0; r < 4; ++r)
+      for (int r = 0; r < kR; ++r)
 #pragma unroll
-        for (int s = 0; s < 4; ++s) acc[r][s] = fmaf(av[r], bv[s], acc[r][s]);
+        for (int s = 0; s < kR; ++s) acc[r][s] = fmaf(av[r], bv[s], acc[r][s]);
     }
     __syncthreads();
   }
   const float inv = g.first ? g.inv_norm[blockIdx.y] : 1.f;
   const float alpha = (g.phase == PH_GRAM) ? inv * inv : (g.phase == PH_APPLY ? inv : 1.f);
 #pragma unroll
-  for (int r = 0; r < 4; ++r)
+  for (int r = 0; r < kR; ++r)
 #pragma unroll
-    for (int s = 0; s < 4; ++s) {
-      const uint32_t i = i0 + ty * 4 + r, j = j0 + tx * 4 + s;
+    for (int s = 0; s < kR; ++s) {
+      const uint32_t i = i0 + ty * kR + r, j = j0 + tx * kR + s;
       if (i >= Mo || j >= No) continue;
       float out;
       if (g.phase == PH_POLY) out = fmaf(g.c, acc[r][s], fmaf(g.b, A[i * sc_i + j], (i == j) ? g.a : 0.f));
@@ -110,11 +113,22 @@ int launch_ns_fp32(const Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t 
   const WsLayout& lay = pl.lay;
   const uint32_t n_mat = (uint32_t)lay.mats.size();
   if (n_mat == 0) return MFSDP_OK;
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   uint32_t max_gram = 1, max_apply = 1;
-  for (const MatLayout& L : lay.mats) {
-    const uint32_t td = (L.d + kT - 1) / kT, tn = (L.n_long + kT - 1) / kT;
-    max_gram = td * td > max_gram ? td * td : max_gram;
-    max_apply = td * tn > max_apply ? td * tn : max_apply;
+  uint64_t total_apply = 0;
+  int kT = 64;
+  for (int pass = 0; pass < 2; ++pass) {
+    max_gram = max_apply = 1; total_apply = 0;
+    for (const MatLayout& L : lay.mats) {
+      const uint32_t td = (L.d + kT - 1) / kT, tn = (L.n_long + kT - 1) / kT;
+      max_gram = td * td > max_gram ? td * td : max_gram;
+      max_apply = td * tn > max_apply ? td * tn : max_apply;
+      total_apply += (uint64_t)td * tn;
+    }
+    if (kT == 32 || total_apply >= 2ull * (uint64_t)sms) break;    // enough 64-tiles to fill the SMs
+    kT = 32;
   }
   NsArgs g;
   g.mats = pl.d_mats;
@@ -127,7 +141,7 @@ int launch_ns_fp32(const Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t 
     for (int ph = 0; ph < 3; ++ph) {
       g.phase = ph;
       const dim3 grid(ph == PH_APPLY ? max_apply : max_gram, n_mat);
-      k_ns_fp32<<<grid, 256, 0, st>>>(g);
+      if (kT == 64) k_ns_fp32<64><<<grid, 256, 0, st>>>(g); else k_ns_fp32<32><<<grid, 256, 0, st>>>(g);
       count_launch();
       const int rc = check_last_launch();
       if (rc) return rc;

@@ -161,6 +161,14 @@ def test_small_ragged_fp32_mode(dtype):
     _full_step_check(wl)
 
 
+def test_medium_ragged_fp32_mode():
+    """fp32 mode on a set with enough 64 x 64 tiles to fill the SMs (the 64-tile instantiation of k_ns_fp32; the tiny
+    sets above run the 32-tile one)."""
+    wl = workloads.medium_ragged(precision=mf.NS_FP32)
+    _, errs = _full_step_check(wl)
+    assert max(errs) <= 1e-4
+
+
 # ---- a3: Newton-Schulz, bf16 tensor-core mode --------------------------------------------------------------------------------
 def test_c1_bf16_mode_full_step():
     wl = workloads.get("c1")
