@@ -442,7 +442,7 @@ def test_separate_passes_equal_fused_step(wname):
                 assert torch.equal(x, y)
 
 
-@pytest.mark.parametrize("wname", ["medium", "small"])
+@pytest.mark.parametrize("wname", ["medium", "small", "c1"])
 @pytest.mark.parametrize("consumer_first", [True, False])
 def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
     """SURVEY 8(f) f1 in the form one GPU can test: the gradients of the resident matrices arrive in 3 waves (here:
@@ -491,7 +491,7 @@ def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
             assert torch.equal(x, y)
 
 
-@pytest.mark.parametrize("wname", ["medium", "small", "fused", "fused2", "c3"])
+@pytest.mark.parametrize("wname", ["medium", "small", "fused", "fused2", "c3", "c1"])
 def test_fanout_copy_of_the_updated_weights(wname):
     """SURVEY 8(f) f2, single-GPU half: mfsdp_muon_step_fanout writes every updated matrix into its fan-out destination
     from the same registers that update the owner's shard -- in the Newton-Schulz epilogue where the update is fused
@@ -535,12 +535,50 @@ def test_host_buffer_entry_point(wname, grouped):
     dW, dG, dM = torch.empty_like(a.W), torch.empty_like(a.W), torch.empty_like(a.M)
     ws = gh.aligned_bytes(mf.mfsdp_host_workspace_bytes(a.desc, a.precision)) if grouped else a.ws
     assert ws.numel() >= a.ws.numel()
-    for step in range(2):
+    for step in range(3):
         a.load_grads(step)
         hG = a.hG.clone().pin_memory()
-        mf.mfsdp_muon_step_host(a.desc, hW, hG, hM, dW, dG, dM, 1, ws, a.hp)
+        # third step: upload_state = 0 -- W and M are taken from the device staging buffers the previous call left
+        mf.mfsdp_muon_step_host(a.desc, hW, hG, hM, dW, dG, dM, 1 if step < 2 else 0, ws, a.hp)
         a.muon_step()
         assert torch.equal(hW, a.W.cpu()) and torch.equal(hM, a.M.cpu())
+
+
+def test_plan_cache_never_evicts_and_release_plans():
+    """The launch-table cache: a cached plan is never freed behind the caller's back -- after 1024 distinct
+    (table, workspace, precision) keys the next new key fails with MFSDP_ECACHE, known keys keep working, and
+    mfsdp_release_plans() empties the cache; results after a release are bit-identical."""
+    mf.mfsdp_release_plans()
+    wl = workloads.get("small")
+    a = gh.Session(wl)
+    a.load_grads(0)
+    a.muon_step()
+    ref = a.W.clone()
+    hp = mf.AdamWHParams(step=1, **wl.adamw)
+    bufs = [torch.zeros(4096, dtype=torch.bfloat16, device="cuda") for _ in range(2)]
+    mv = [torch.zeros(4096, dtype=torch.float32, device="cuda") for _ in range(2)]
+    full_at = None
+    for i in range(1100):                                     # tail-only tables of different lengths: tiny plans
+        desc = mf.make_desc_array([dict(role=mf.ROLE_TAIL, param_id=0, block_id=0, rows=8 + i, cols=1, dtype=mf.BF16,
+                                        flags=0, elem_off=0)])
+        try:
+            mf.mfsdp_adamw_tail_step(desc, bufs[0], bufs[1], mv[0], mv[1], hp)
+        except mf.MfsdpError as e:
+            assert e.code == mf.ECACHE and "mfsdp_release_plans" in str(e)
+            full_at = i
+            break
+    assert full_at is not None and 1000 <= full_at <= 1024
+    b = gh.Session(wl)                                        # a NEW key (new workspace) cannot be planned now ...
+    b.load_grads(0)
+    with pytest.raises(mf.MfsdpError) as e:
+        b.muon_step()
+    assert e.value.code == mf.ECACHE
+    a.W.copy_(a.hW.cuda()); a.M.zero_()
+    a.muon_step()                                             # ... a cached one still runs
+    assert torch.equal(a.W, ref)
+    mf.mfsdp_release_plans()
+    b.muon_step()
+    assert torch.equal(b.W, ref)
 
 
 def test_launch_counter_counts_kernels():
