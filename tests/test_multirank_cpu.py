@@ -116,3 +116,61 @@ def test_schedule_mismatch_is_an_explicit_error_on_every_rank():
     a, b = _run_sched(True)
     assert a[1] == b[1] == "mismatch" and a[2] == b[2] and len(a[2]) == 2
     assert "ranks [0]" in a[3] and "ranks [1]" in a[3]
+
+
+# ---- the exchange steps themselves on CPU (gloo): reduce-to-owner and owner fan-out -------------------------
+def _exchange_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import paper_2607_05895_b200 as mf
+    from paper_2607_05895_b200 import dist as mdist
+    import workloads
+    wl = workloads.get("small")                       # 9 matrices + 3 tails in 3 blocks, planned over 2 ranks
+    pr = mf.mfsdp_plan(wl.params, world, mf.POLICY_ROLE_GREEDY, mf.METRIC_NUMEL, rank)
+    ops, _ = mdist.validated_reduce_schedule(wl.params, world, pr.owner)
+    fwd, _ = mdist.validated_reduce_schedule(wl.params, world, pr.owner, reverse_blocks=False)
+    n_mat, n_tail = mf.mfsdp_flat_elems(pr.desc)
+    # every rank's full local gradient of role r: seeded by (rank, role), fp32 on CPU
+    grads = {op.role: torch.Generator().manual_seed(1000 * rank + op.role) for op in ops}
+    grads = {op.role: torch.randn(op.numel, generator=grads[op.role]) for op in ops}
+    sent = {r: g.clone() for r, g in grads.items()}
+    G, Gt = torch.zeros(max(n_mat, 1)), torch.zeros(max(n_tail, 1))
+    mdist.reduce_gradients_to_owners(ops, rank, lambda r: grads[r], G, Gt)
+    # expected: sum over ranks of the seeded gradients, only in the segments this rank owns
+    ok = True
+    for op in ops:
+        want = sum(torch.randn(op.numel, generator=torch.Generator().manual_seed(1000 * q + op.role)) for q in range(world))
+        flat = G if op.kind == mf.ROLE_MATRIX else Gt
+        if op.owner == rank:
+            ok &= bool(torch.allclose(flat[op.owner_elem_off:op.owner_elem_off + op.numel], want, rtol=0, atol=1e-6))
+    owned = sum(op.numel for op in ops if op.owner == rank)
+    nonzero = int((G != 0).sum() + (Gt != 0).sum())
+    # fan-out: owners publish "updated weights" = their reduced gradient segments; every rank ends with all of them
+    full = {op.role: torch.zeros(op.numel) for op in fwd}
+    mdist.fanout_parameters(fwd, rank, G, Gt, lambda r: full[r])
+    fan_ok = True
+    for op in fwd:
+        want = sum(torch.randn(op.numel, generator=torch.Generator().manual_seed(1000 * q + op.role)) for q in range(world))
+        fan_ok &= bool(torch.allclose(full[op.role], want, rtol=0, atol=1e-6))
+    out.put((rank, ok, owned, nonzero, fan_ok, [op.role for op in ops][:3], [op.role for op in fwd][:3]))
+    dist.destroy_process_group()
+
+
+@pytest.mark.timeout(180)
+def test_reduce_to_owner_and_fanout_over_gloo():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_exchange_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=150) for _ in range(2))
+    for p in procs:
+        p.join(30)
+        assert p.exitcode == 0
+    for rank, ok, owned, nonzero, fan_ok, first_rev, first_fwd in res:
+        assert ok, "rank %d: an owned segment is not the sum of the ranks' gradients" % rank
+        assert fan_ok, "rank %d: a materialised parameter differs from its owner's segment" % rank
+        assert nonzero <= owned and nonzero >= owned - 8      # nothing lands outside owned segments (exact zeros are rare)
+    assert res[0][5] == res[1][5] and res[0][6] == res[1][6] and res[0][5] != res[0][6]   # same order on both ranks
