@@ -440,7 +440,9 @@ def measure_other_config(torch, mf, name, pk, local, paper=False, reuse=None):
                ns_frac_of="sustained bf16 peak (sw_power_cap sampled)" if capped else "burst bf16 peak",
                precision="bf16" if res.wl.precision == mf.NS_BF16 else "f32 (FFMA correctness mode)",
                momentum_gbs=passes_record(res, t, pk)["momentum"]["gbs"], update_gbs=passes_record(res, t, pk)["update"]["gbs"],
-               launches_per_step=launches / steps, clocks=dict(sm_mhz=clocks.get("sm_mhz"), reasons=clocks.get("reasons")))
+               launches_per_step=launches / steps, clocks=dict(sm_mhz=clocks.get("sm_mhz"), reasons=clocks.get("reasons")),
+               l2="inputs larger than L2" if res.n_mat_el * res.wbytes > 256e6 else
+               "working set may fit L2 (not flushed): steady-state optimizer-step latency of a set this small")
     return rec
 
 
