@@ -29,6 +29,11 @@
 // counter in list order, waits until the tile's inputs (every tile of the same matrix in the preceding phases) have
 // been reported complete through a per-matrix counter, and publishes the index to the other roles through a
 // shared-memory ring.
+//
+// On the last iteration the APPLY epilogue can also apply the weight update W <- W (1 - lr wd) - lr s O from the O tile
+// it holds (UpdArgs; bf16 weights, every cols % 8 == 0) and copy the new W to a fan-out destination; O is then stored
+// only on request.  Small matrices do not come here at all: d <= 128 runs in ns_fused.cu, 128 < d <= 256 (n <= 512) in
+// ns_fused2.cu (one CTA per matrix for all iterations); the classes of one pass run concurrently on forked streams.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
