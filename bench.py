@@ -42,7 +42,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--config", default="c5", choices=["c1", "c2", "c3", "c4", "c5", "paper16l"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--paper-setting", action="store_true",
                     help="the paper's own Muon hyper-parameters (PAPER.md:121): momentum 0.5, 2 NS steps, lr 1e-3")
@@ -555,9 +555,9 @@ def run_ours(args):
             others.append(dict(workload="c5+paper_setting", error=repr(e)))
         del res
         torch.cuda.empty_cache()
-        for name in ("c1", "c2", "c3", "c4"):
-            try:
-                others.append(measure_other_config(torch, mf, name, pk, local))
+        for name in ("c1", "c2", "c3", "c4", "paper16l"):
+            try:      # paper16l: the paper's own Table 1 / 3 workload (one rank's share) with the paper's own setting
+                others.append(measure_other_config(torch, mf, name, pk, local, paper=(name == "paper16l")))
             except Exception as e:
                 others.append(dict(workload=name, error=repr(e)))
             torch.cuda.empty_cache()

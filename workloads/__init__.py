@@ -93,6 +93,18 @@ def c5_llama70b():
                     metric=METRIC_NS_FLOPS, rank=-1)
 
 
+def paper_qwen16l():
+    """The paper's own latency workload as far as its text fixes it ("bf16 Qwen-style decoder-transformer
+    shapes (hidden 4096, intermediate 16384, 32 heads ...)", 16 layers over shard span 8; Table 1 / 3: "16L / 3.2B",
+    MatrixFSDP optimizer step 87 ms on 8 x A100).  3.2 B / 16 layers = 201 M parameters per layer fits six matrices per
+    layer -- q, k, v, o 4096 x 4096, up 16384 x 4096, down 4096 x 16384 (SURVEY.md section 6 inference; the paper lists
+    no per-layer shapes, no embedding size) -- plus two RMSNorm vectors.  Planner as the paper describes it: ROLE-GREEDY
+    on owner-resident numel, 8 ranks, heaviest rank.  Run with the paper's Muon setting (mu 0.5, K 2)."""
+    mats = [(4096, 4096)] * 4 + [(16384, 4096), (4096, 16384)]
+    return Workload("paper_qwen16l_3.2b_heaviestof8", _layers(16, mats, [4096, 4096], BF16), seed=5, world=8,
+                    metric=METRIC_NUMEL, rank=-1)
+
+
 def small_ragged(seed=7, dtype=BF16, precision=NS_BF16):
     """Parity-test set the oracle finishes in seconds: several tiles, ragged tails, wide / tall / square, odd pitches."""
     shapes = [(320, 200), (200, 320), (130, 130), (64, 520), (520, 64), (384, 384), (72, 1000), (257, 129), (8, 24)]
@@ -156,7 +168,7 @@ def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
     return Workload("vocab_embedding", params, seed=seed, precision=precision, dtype=dtype)
 
 
-CONFIGS = {"c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
+CONFIGS = {"paper16l": paper_qwen16l, "c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
            "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes, "fused": fused_shapes, "fused2": fused2_shapes,
            "vocab": vocab_embedding}
 
