@@ -336,6 +336,65 @@ int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, cons
 int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, const void* G, void* m, void* v,
                           const mfsdp_adamw_hparams_t* hp, void* cuda_stream);
 
+/* ---- owner-local Shampoo on the same descriptors (DEVICE work, HOST call) ---------------------------------------
+ * "The owner-placement runtime is optimizer-agnostic: each 2D matrix is whole on its owner, so any
+ * single-device matrix optimizer runs there with no gather and no distributed variant.  We verify this by swapping
+ * owner-Muon for Shampoo (full L/R preconditioners with inverse fourth root) ... float32".  The
+ * paper prints neither formulas nor hyper-parameters; what is computed is Algorithm 1 of Gupta et al. (2018) for
+ * matrices under the readings S1-S6 of DESIGN.md section 4.  For every MATRIX descriptor (tails are ignored):
+ *   S1  L <- beta2 L + w G G^T ;  R <- beta2 R + w G^T G ;  w = 1 if beta2 == 1 (running sum) else 1 - beta2
+ *   S2  ridge relative to the mean eigenvalue: S~ = S + rho I, rho = eps tr S / d ;  tr S <= 0 -> the preconditioner is I
+ *   S7  float32 floor of the ridge: rho = max(eps tr S / d, eps_floor ||S||_F).  The statistic carries rounding noise of
+ *       about 2^-22 ||S||_F in this arithmetic; a ridge below it leaves S~ indefinite (rank-deficient statistics: every
+ *       wide or tall matrix) and no float32 iteration can then return S~^{-1/4}.  eps_floor = 2^-20 keeps the condition
+ *       number below 2^20; 0 = the plain S2 (a root that meets a NaN falls back to (tr S / d + rho)^{-1/4} I, flagged)
+ *   S3  P_L = L~^{-1/4}, P_R = R~^{-1/4}
+ *   S4  D = P_L G P_R ;  W <- W (1 - lr weight_decay) - lr D
+ *   S5  the roots are recomputed at steps with (step - 1) % root_every == 0, from statistics that include G_step;
+ *       other steps reuse the stored roots
+ *   S6  the roots are computed by the coupled Newton iteration  M_0 = z S~, X_0 = z^{1/4} I, z = 5 / (2 (||S||_F + rho)),
+ *       T = (5 I - M) / 4, X <- X T, M <- T^4 M  until max |M - I| < root_tol, the error stops falling (fp32-class
+ *       noise floor) or max_root_iters is reached; X -> S~^{-1/4}.
+ * Arithmetic: every matrix product runs on the bf16 tensor cores with fp32 values carried as three bf16 terms
+ * (24 significand bits, fp32 exponent range) and fp32 accumulation -- fp32-class, not bit-identical to an fp32 FFMA loop.
+ * L and R are fp32; P_L, P_R are kept as three bf16 planes (their sum is the fp32 value).
+ *   W, G        DEVICE.  rank-flat matrix parameters (in/out) / gradients (in), 16-byte aligned; dtype of the descriptors.
+ *   state       DEVICE in/out.  mfsdp_shampoo_state_bytes, 1024-byte aligned, caller-owned, ZEROED before the first
+ *                               step (L_0 = R_0 = 0); layout per matrix: mfsdp_shampoo_view.
+ *   workspace   DEVICE scratch. 1024-byte aligned; at least min_bytes of mfsdp_shampoo_workspace_bytes.  The roots of the
+ *                               resident set are computed in groups of as many (L, R) problems as fit behind the fixed part:
+ *                               full_bytes processes them all at once (fewest launches), min_bytes one at a time.
+ *   hp          HOST in.
+ * Enqueues on cuda_stream and does not synchronise (the number of launches is fixed: converged problems are skipped
+ * on the device).  Launch tables are cached per (table, W, G, state, workspace, ws_bytes, flags); at most 64 keys
+ * (MFSDP_ECACHE beyond; mfsdp_release_plans frees them).  Errors as mfsdp_muon_step. */
+enum { MFSDP_SHAMPOO_KEEP_D = 1u };      /* flags bit0: also leave D = P_L G P_R (fp32) in the workspace              */
+typedef struct {
+  double  lr;              /* eta                                                                                  */
+  double  weight_decay;    /* lambda (decoupled)                                                                   */
+  double  beta2;           /* in (0, 1]; 1 = running sum (Gupta et al.), < 1 = moving average (Anil et al.)        */
+  double  eps;             /* relative ridge, >= 0 (1e-6)                                                          */
+  double  eps_floor;       /* S7, >= 0 (2^-20)                                                                     */
+  double  root_tol;        /* 0 -> 1e-6                                                                            */
+  int64_t step;            /* 1-based                                                                              */
+  int32_t root_every;      /* >= 1                                                                                 */
+  int32_t max_root_iters;  /* 0 -> 40                                                                              */
+  uint32_t flags;          /* MFSDP_SHAMPOO_*                                                                      */
+  uint32_t reserved;       /* 0                                                                                    */
+} mfsdp_shampoo_hparams_t;
+int mfsdp_shampoo_state_bytes(const mfsdp_desc_t* desc, size_t n_desc, size_t* bytes);
+int mfsdp_shampoo_workspace_bytes(const mfsdp_desc_t* desc, size_t n_desc, uint32_t flags, size_t* min_bytes,
+                                  size_t* full_bytes);
+int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* state, size_t state_bytes,
+                       void* workspace, size_t ws_bytes, const mfsdp_shampoo_hparams_t* hp, void* cuda_stream);
+/* Layout of the `index`-th matrix (HOST; tests and callers that checkpoint the state):
+ * out[0..3] = byte offsets in `state` of L (rows x out[4] floats), R (cols x out[5] floats), P_L (3 planes of
+ * rows x out[4] bf16, out[6] elements apart), P_R (3 planes of cols x out[5] bf16, out[7] elements apart);
+ * out[8] = byte offset in the workspace of D (rows x out[5] floats; MFSDP_SHAMPOO_KEEP_D only);
+ * out[9] = byte offset in the workspace of the root control records of this matrix (L then R), out[10] bytes each:
+ *   { double tr, fro2; float rho, z, x0, last_err; uint32 err_bits, iters, done (1 converged / stopped, 2 NaN), identity }. */
+int mfsdp_shampoo_view(const mfsdp_desc_t* desc, size_t n_desc, uint32_t flags, size_t index, size_t out[12]);
+
 /* Debug / test aid (HOST): byte offsets inside the workspace of the `index`-th matrix' NS buffers:
  * out[0], out[1] = X ping-pong buffers (X~ = cast(U) is written to out[0]; rows x cols like the parameter),
  * out[2] = A (d x d, d = min(rows, cols)), out[3] = P = aI + bA + cA^2 (d x d),

@@ -16,5 +16,6 @@ from .binding import (  # noqa: F401
     mfsdp_debug_ws_offsets, mfsdp_muon_step, mfsdp_muon_momentum_pass, mfsdp_muon_ns_pass, mfsdp_muon_update_pass,
     mfsdp_muon_step_host, mfsdp_adamw_tail_step, mfsdp_strerror, mfsdp_version, mfsdp_launch_count,
     mfsdp_tune, mfsdp_get_tune, mfsdp_debug_trace, TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D, TUNE_FUSED2_BELOW_D, mfsdp_release_plans, mfsdp_ns_class,
-    make_desc_array,
+    make_desc_array, SHAMPOO_KEEP_D, ShampooHParams, mfsdp_shampoo_state_bytes, mfsdp_shampoo_workspace_bytes,
+    mfsdp_shampoo_view, mfsdp_shampoo_step,
 )

@@ -12,6 +12,7 @@ METRIC_NUMEL, METRIC_NS_FLOPS = 0, 1
 SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE = 0, 1, 2
 NS_BF16, NS_FP32 = 0, 1
 STEP_KEEP_O = 1
+SHAMPOO_KEEP_D = 1
 OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE = 0, -1, -2, -3, -4, -5, -6
 
 
@@ -48,6 +49,16 @@ class AdamWHParams(C.Structure):     # mfsdp_adamw_hparams_t
 
     def __init__(self, lr=1e-3, beta1=0.9, beta2=0.95, eps=1e-8, weight_decay=0.01, step=1):
         super().__init__(lr, beta1, beta2, eps, weight_decay, step)
+
+
+class ShampooHParams(C.Structure):   # mfsdp_shampoo_hparams_t
+    _fields_ = [("lr", C.c_double), ("weight_decay", C.c_double), ("beta2", C.c_double), ("eps", C.c_double),
+                ("eps_floor", C.c_double), ("root_tol", C.c_double), ("step", C.c_int64), ("root_every", C.c_int32),
+                ("max_root_iters", C.c_int32), ("flags", C.c_uint32), ("reserved", C.c_uint32)]
+
+    def __init__(self, lr=1e-3, weight_decay=0.0, beta2=1.0, eps=1e-6, eps_floor=2.0 ** -20, root_tol=0.0, step=1,
+                 root_every=1, max_root_iters=0, flags=0):
+        super().__init__(lr, weight_decay, beta2, eps, eps_floor, root_tol, step, root_every, max_root_iters, flags, 0)
 
 
 class Caps(C.Structure):             # mfsdp_caps_t
@@ -95,7 +106,8 @@ _SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_reduce_sch
             "mfsdp_workspace_view", "mfsdp_muon_step", "mfsdp_muon_momentum_pass", "mfsdp_muon_ns_pass",
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_host_workspace_bytes", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
             "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
-            "mfsdp_release_plans", "mfsdp_ns_class"]
+            "mfsdp_release_plans", "mfsdp_ns_class", "mfsdp_shampoo_state_bytes", "mfsdp_shampoo_workspace_bytes",
+            "mfsdp_shampoo_step", "mfsdp_shampoo_view"]
 _lib = None
 
 
@@ -152,6 +164,10 @@ def load():
     lib.mfsdp_get_tune.argtypes = [i32]
     lib.mfsdp_debug_trace.argtypes = [vp, sz]
     lib.mfsdp_ns_class.argtypes = [C.c_uint32, C.c_uint32]
+    lib.mfsdp_shampoo_state_bytes.argtypes = [pD, sz, psz]
+    lib.mfsdp_shampoo_workspace_bytes.argtypes = [pD, sz, C.c_uint32, psz, psz]
+    lib.mfsdp_shampoo_view.argtypes = [pD, sz, C.c_uint32, sz, psz]
+    lib.mfsdp_shampoo_step.argtypes = [pD, sz, vp, vp, vp, sz, vp, sz, C.POINTER(ShampooHParams), vp]
     for name in _SYMBOLS:
         getattr(lib, name)          # AttributeError if the library does not export what the header declares
     _lib = lib
@@ -430,3 +446,31 @@ def mfsdp_adamw_tail_step(desc, P, G, m, v, hp, stream=None):
     arr, n = _dn(desc)
     _check(load().mfsdp_adamw_tail_step(arr, n, _ptr(P), _ptr(G), _ptr(m), _ptr(v), C.byref(hp), _stream(stream)),
            "mfsdp_adamw_tail_step")
+
+
+def mfsdp_shampoo_state_bytes(desc):
+    arr, n = _dn(desc)
+    out = C.c_size_t(0)
+    _check(load().mfsdp_shampoo_state_bytes(arr, n, C.byref(out)), "mfsdp_shampoo_state_bytes")
+    return out.value
+
+
+def mfsdp_shampoo_workspace_bytes(desc, flags=0):
+    """(min_bytes, full_bytes)"""
+    arr, n = _dn(desc)
+    lo, hi = C.c_size_t(0), C.c_size_t(0)
+    _check(load().mfsdp_shampoo_workspace_bytes(arr, n, flags, C.byref(lo), C.byref(hi)), "mfsdp_shampoo_workspace_bytes")
+    return lo.value, hi.value
+
+
+def mfsdp_shampoo_view(desc, flags, index):
+    arr, n = _dn(desc)
+    out = (C.c_size_t * 12)()
+    _check(load().mfsdp_shampoo_view(arr, n, flags, index, out), "mfsdp_shampoo_view")
+    return list(out)
+
+
+def mfsdp_shampoo_step(desc, W, G, state, workspace, hp, stream=None):
+    arr, n = _dn(desc)
+    _check(load().mfsdp_shampoo_step(arr, n, _ptr(W), _ptr(G), _ptr(state), _nbytes(state), _ptr(workspace),
+                                     _nbytes(workspace), C.byref(hp), _stream(stream)), "mfsdp_shampoo_step")

@@ -592,6 +592,8 @@ extern "C" int mfsdp_release_plans(void) {
     free_plan(pl);
   }
   if (have_dev) cudaSetDevice(dev);
+  release_shampoo_plans();
+  if (have_dev) cudaSetDevice(dev);
   g_plans.clear();
   g_plan_keys.clear();
   return MFSDP_OK;

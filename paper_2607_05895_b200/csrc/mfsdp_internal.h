@@ -86,6 +86,7 @@ int launch_ns_tc(Plan& pl, const mfsdp_muon_hparams_t& hp, cudaStream_t st, void
                  const uint64_t* fan = nullptr);
 bool ns_tc_can_fuse_update(Plan& pl);   // bf16 weights, every cols % 8 == 0: the update runs in the last APPLY epilogue
 void destroy_ns_tc(NsTcPlan* p);
+void release_shampoo_plans();          // shampoo.cu; caller holds plan_mutex()
 int ns_class(uint32_t rows, uint32_t cols);   // 0 whole-matrix kernel, 1 single-CTA tiles, 2 CTA-pair tiles
 
 // ---- bookkeeping ---------------------------------------------------------------------------------------------

@@ -1,0 +1,397 @@
+// Grouped fp32-class GEMM on the bf16 tensor cores (tcgen05), used by the owner-local Shampoo step (shampoo.cu).
+//
+// Shampoo's preconditioner statistics and inverse fourth roots need fp32-class arithmetic (PAPER.md:182 runs them in
+// "float32"); Blackwell has no fp32 tensor-core path and its FFMA pipes deliver ~1/30 of the bf16 tensor rate.  An
+// fp32 value v is therefore carried as THREE bf16 terms  v = b1 + b2 + b3  (b1 = rn(v), b2 = rn(v - b1),
+// b3 = rn(v - b1 - b2): 24 significand bits, fp32's exponent range, no scaling), stored as three row-major planes,
+// and a product of two such matrices is the sum of the six term products with i + j <= 2 (the three dropped ones are
+// below 2^-24 of the leading one), all accumulated into ONE fp32 TMEM accumulator:
+//     C = sum_{i + j <= 2} A_i B_j^T          6 UMMAs per 16-element k step for 6 operand tiles in shared memory.
+// bf16 inputs (a bf16 gradient) are exact single terms: 1 or 3 UMMAs per k step.
+//
+// Accumulation.  The tensor core adds into its fp32 accumulator with truncation, one truncating add per UMMA k step:
+// a chain of K / 16 (x 6) adds shrinks every sum by ~ (adds / 2) 2^-24 -- measured 1.8e-6 at K = 904 with one term,
+// 5e-5 at K = 4096 with six: not fp32-class.  So the TMEM accumulator only ever holds the partial sum of ONE chunk of
+// k (kKC blocks of 64), the five small term products are issued first (their truncation is relative to sums 2^-8
+// smaller) and the four leading-term k steps last; the epilogue warps fold each chunk into registers with
+// round-to-nearest fp32 adds (128 accumulator registers per thread = the thread's row of the 128 x 128 tile) while the
+// UMMAs of the next chunks run into the other three TMEM buffers.  Residual bias ~ 2 .. 8 x 2^-24 per chunk, unbiased
+// rounding across chunks.
+//
+// One launch works through the tiles of MANY independent problems (every L and every R of the resident set at
+// once): 128 x 128 output tiles, k blocks of 64, one CTA per SM, static round-robin over a host-built tile list
+// whose order keeps the tiles in flight a compact block of one output (operand panels shared through L2).
+// Warp 0 = TMA producer (3-D tensor maps: column, row, term plane; 128-byte swizzle; out-of-range elements read as
+// zero, so ragged edges need no special cases), warp 1 = TMEM owner + UMMA issuer, warps 2-5 = epilogue.  Four
+// chunk accumulators (4 x 128 TMEM columns) rotate, so the stores of one tile overlap the UMMAs of the next.
+// Operands may be K-major (row-major with k contiguous) or MN-major (row-major with the output index
+// contiguous: G^T G and P_L G read G in place, never transposed in memory).
+//
+// Epilogue (all optional, per problem): v = alpha acc + beta Cin;  fp32 store;  three-term split store;  the split of
+// T = (5 I - v) / 4 (the next coupled-Newton step matrix);  max |v - I| into an error word;  the weight update
+// W <- decay W - lr v.  Symmetric problems compute only the tiles on and above the block diagonal and store the
+// mirror image as well.
+#ifndef MFSDP_SGEMM3_CUH_
+#define MFSDP_SGEMM3_CUH_
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#include "ptx_sm100.cuh"
+
+namespace mfsdp {
+
+struct alignas(64) SgProb {
+  CUtensorMap ta, tb;               // operand storage: dims (cols, rows, planes)
+  uint32_t M, N, K;                 // output rows, columns; reduction length
+  uint32_t a_mn, b_mn;              // 1: operand stored [k][m] (MN-major) instead of [m][k]
+  uint32_t sym;                     // symmetric output: tiles with n0 >= m0 only, mirrored by the epilogue
+  uint32_t f32_pitch;               // row pitch of cin / out_f32 (elements; multiple of 64 so that 32-column chunks fit)
+  uint32_t sp_pitch;                // row pitch of the split planes (elements, multiple of 64)
+  uint64_t sp_plane;                // elements between the planes of out_split / t_split
+  const float* cin;                 // optional; may alias out_f32 (read before written by the same thread)
+  float* out_f32;                   // optional
+  __nv_bfloat16* out_split;         // optional: three planes
+  __nv_bfloat16* t_split;           // optional: split of (5 I - v) / 4
+  uint32_t* err;                    // optional: atomicMax of the bits of max |v - delta|
+  const uint32_t* done;             // optional: non-zero -> the problem is finished, its tiles are skipped
+  void* W;                          // optional: rank-flat weights of this matrix (pitch = N), updated in place
+  uint32_t w_bf16;                  // dtype of W
+  uint32_t pad;
+};
+struct SgTile { uint32_t prob, m0, n0; };
+struct SgParams {
+  const SgProb* probs;
+  const SgTile* tiles;
+  uint32_t n_tiles;
+  float alpha, beta;                // v = alpha acc + beta Cin
+  float decay, lr;                  // W <- decay W - lr v
+};
+
+constexpr uint32_t kSgThreads = 192;
+constexpr uint32_t kSgBox = 16384;  // one term of one operand of one stage: 128 rows x 64 k, or 2 x (64 k x 64 mn)
+template <int AT, int BT> struct SgCfg {
+  static constexpr uint32_t kStage = (AT + BT) * kSgBox;
+  static constexpr uint32_t kStages = (AT + BT) == 2 ? 6 : (AT + BT) == 4 ? 3 : 2;
+  static constexpr uint32_t kSmem = kStages * kStage + 256 + 1024;
+  // k blocks per TMEM chunk.  One: at most four truncating adds of leading-term products per partial sum.  (With one
+  // term per operand a block is 256 cycles of UMMA, less than the epilogue warps need to fold it -- 4 tcgen05.ld of 32
+  // columns + 128 adds -- so the statistics GEMM of a bf16 gradient runs fold-bound; it is a few percent of a step.)
+  static constexpr uint32_t kKC = 1;
+};
+constexpr uint32_t kSgAccs = 4;      // TMEM chunk accumulators of 128 columns
+
+namespace sg {
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const void* tmap, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+      "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
+      : "memory");
+}
+__device__ __forceinline__ void split3(float v, uint32_t& b1, uint32_t& b2, uint32_t& b3) {   // bf16 bit patterns
+  const __nv_bfloat16 h1 = __float2bfloat16_rn(v);
+  const float r1 = v - __bfloat162float(h1);                      // exact
+  const __nv_bfloat16 h2 = __float2bfloat16_rn(r1);
+  const float r2 = r1 - __bfloat162float(h2);                     // exact
+  const __nv_bfloat16 h3 = __float2bfloat16_rn(r2);
+  b1 = __bfloat16_as_ushort(h1); b2 = __bfloat16_as_ushort(h2); b3 = __bfloat16_as_ushort(h3);
+}
+// 8 consecutive values of one row -> the three planes (16 bytes each)
+__device__ __forceinline__ void store_split8(__nv_bfloat16* p0, uint64_t plane, const float* v) {
+  uint32_t w[3][4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    uint32_t a1, a2, a3, c1, c2, c3;
+    split3(v[2 * j], a1, a2, a3);
+    split3(v[2 * j + 1], c1, c2, c3);
+    w[0][j] = a1 | (c1 << 16); w[1][j] = a2 | (c2 << 16); w[2][j] = a3 | (c3 << 16);
+  }
+#pragma unroll
+  for (int t = 0; t < 3; ++t)
+    *reinterpret_cast<uint4*>(p0 + t * plane) = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+}
+__device__ __forceinline__ void store_split1(__nv_bfloat16* d, uint64_t plane, float v) {
+  uint32_t b1, b2, b3;
+  split3(v, b1, b2, b3);
+  d[0] = __ushort_as_bfloat16((unsigned short)b1);
+  d[plane] = __ushort_as_bfloat16((unsigned short)b2);
+  d[2 * plane] = __ushort_as_bfloat16((unsigned short)b3);
+}
+}  // namespace sg
+
+template <int AT, int BT>
+__global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
+  using Cfg = SgCfg<AT, BT>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  const uint32_t ring0 = ptx::smem_u32(smem);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::kStages * Cfg::kStage);
+  const uint32_t full0 = ptx::smem_u32(bars), empty0 = ptx::smem_u32(bars + Cfg::kStages);
+  const uint32_t tfull0 = ptx::smem_u32(bars + 2 * Cfg::kStages), tempty0 = ptx::smem_u32(bars + 2 * Cfg::kStages + kSgAccs);
+  uint32_t* tmem_holder = reinterpret_cast<uint32_t*>(bars + 2 * Cfg::kStages + 2 * kSgAccs);
+  const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (uint32_t s = 0; s < Cfg::kStages; ++s) { ptx::mbar_init(full0 + 8 * s, 1); ptx::mbar_init(empty0 + 8 * s, 1); }
+    for (uint32_t s = 0; s < kSgAccs; ++s) { ptx::mbar_init(tfull0 + 8 * s, 1); ptx::mbar_init(tempty0 + 8 * s, 4); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 1) ptx::tmem_alloc<512, 1>(ptx::smem_u32(tmem_holder));
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = *tmem_holder;
+
+  uint32_t stage = 0, ring_phase = 0;   // producer, issuer
+  uint32_t cc = 0;                      // k chunks this CTA has worked on: TMEM accumulator = cc % 4 (issuer, epilogue)
+
+  for (uint32_t ti = blockIdx.x; ti < p.n_tiles; ti += gridDim.x) {
+    const SgTile t = p.tiles[ti];
+    const SgProb* pr = p.probs + t.prob;
+    if (pr->done != nullptr && *pr->done != 0u) continue;       // stable during the launch: every role agrees
+    const uint32_t K = pr->K, nkb = (K + 63u) >> 6;
+    const uint32_t a_mn = pr->a_mn, b_mn = pr->b_mn;
+
+    if (warp == 0) {
+      // ===== TMA producer =====
+      for (uint32_t kb = 0; kb < nkb; ++kb) {
+        ptx::mbar_wait(empty0 + 8 * stage, ring_phase ^ 1u);
+        if (ptx::elect_one()) {
+          const uint32_t dst = ring0 + stage * Cfg::kStage, fb = full0 + 8 * stage;
+          ptx::mbar_arrive_expect_tx(fb, Cfg::kStage);
+#pragma unroll
+          for (int i = 0; i < AT; ++i) {
+            if (!a_mn) sg::tma_load_3d(dst + i * kSgBox, &pr->ta, (int)(64 * kb), (int)t.m0, i, fb);
+            else {
+              sg::tma_load_3d(dst + i * kSgBox, &pr->ta, (int)t.m0, (int)(64 * kb), i, fb);
+              sg::tma_load_3d(dst + i * kSgBox + 8192, &pr->ta, (int)t.m0 + 64, (int)(64 * kb), i, fb);
+            }
+          }
+#pragma unroll
+          for (int j = 0; j < BT; ++j) {
+            const uint32_t d = dst + (AT + j) * kSgBox;
+            if (!b_mn) sg::tma_load_3d(d, &pr->tb, (int)(64 * kb), (int)t.n0, j, fb);
+            else {
+              sg::tma_load_3d(d, &pr->tb, (int)t.n0, (int)(64 * kb), j, fb);
+              sg::tma_load_3d(d + 8192, &pr->tb, (int)t.n0 + 64, (int)(64 * kb), j, fb);
+            }
+          }
+        }
+        __syncwarp();
+        if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
+      }
+    } else if (warp == 1) {
+      // ===== UMMA issuer: loops run converged (warp-uniform descriptors), one elected lane issues =====
+      const uint32_t idesc = ptx::idesc_bf16_f32(128, 128, a_mn, b_mn);
+      const uint32_t a_step = a_mn ? (2048u >> 4) : (32u >> 4), b_step = b_mn ? (2048u >> 4) : (32u >> 4);
+      const uint32_t a_lbo = a_mn ? 8192u : 16u, b_lbo = b_mn ? 8192u : 16u;
+      for (uint32_t kb0 = 0; kb0 < nkb; kb0 += Cfg::kKC) {
+        const uint32_t buf = cc % kSgAccs, use = cc / kSgAccs;
+        ptx::mbar_wait(tempty0 + 8 * buf, (use & 1u) ^ 1u);       // the epilogue has folded this accumulator's last chunk
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + buf * 128u;
+        const uint32_t kb1 = min(nkb, kb0 + Cfg::kKC);
+        for (uint32_t kb = kb0; kb < kb1; ++kb) {
+          ptx::mbar_wait(full0 + 8 * stage, ring_phase);
+          ptx::tc_fence_after();
+          const uint32_t ksteps = min(4u, (K - 64u * kb + 15u) >> 4);
+          const uint32_t base = ring0 + stage * Cfg::kStage;
+          if (ptx::elect_one()) {
+            uint32_t fresh = kb == kb0 ? 0u : 1u;                  // the first UMMA of a chunk overwrites the accumulator
+            // the small term products first, the leading one last (see "Accumulation" above)
+#pragma unroll
+            for (int i = 0; i < AT; ++i)
+#pragma unroll
+              for (int j = 0; j < BT; ++j)
+                if (i + j <= 2 && i + j > 0) {
+                  const uint64_t ad0 = ptx::smem_desc_sw128(base + i * kSgBox, a_lbo, 1024);
+                  const uint64_t bd0 = ptx::smem_desc_sw128(base + (AT + j) * kSgBox, b_lbo, 1024);
+                  for (uint32_t ks = 0; ks < ksteps; ++ks) {
+                    ptx::umma_bf16(d_tmem, ad0 + (uint64_t)(ks * a_step), bd0 + (uint64_t)(ks * b_step), idesc, fresh);
+                    fresh = 1u;
+                  }
+                }
+            {
+              const uint64_t ad0 = ptx::smem_desc_sw128(base, a_lbo, 1024);
+              const uint64_t bd0 = ptx::smem_desc_sw128(base + AT * kSgBox, b_lbo, 1024);
+              for (uint32_t ks = 0; ks < ksteps; ++ks) {
+                ptx::umma_bf16(d_tmem, ad0 + (uint64_t)(ks * a_step), bd0 + (uint64_t)(ks * b_step), idesc, fresh);
+                fresh = 1u;
+              }
+            }
+            ptx::umma_commit(empty0 + 8 * stage);
+            if (kb + 1 == kb1) ptx::umma_commit(tfull0 + 8 * buf);
+          }
+          __syncwarp();
+          if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
+        }
+        ++cc;
+      }
+    } else {
+      // ===== epilogue: warp owns TMEM lanes 32 q .. + 31 = rows m0 + 32 q .. of the tile =====
+      const uint32_t q = warp & 3u;
+      const uint32_t M = pr->M, N = pr->N;
+      const uint32_t r = t.m0 + q * 32u + lane;
+      const bool row_ok = r < M;
+      // symmetric outputs: a tile above the block diagonal also stores its mirror image; a tile ON the diagonal stores
+      // its upper triangle (c >= r) and the mirror of the strict upper triangle, so that the result is bit-symmetric
+      // (with several terms the two triangles of a diagonal tile are summed in different orders)
+      const bool mirror = pr->sym != 0u && t.n0 >= t.m0;
+      const bool diag = pr->sym != 0u && t.n0 == t.m0;
+      // fold the k chunks into registers: this thread's row of the tile, round-to-nearest adds
+      float acc[128];
+      for (uint32_t kb0 = 0; kb0 < nkb; kb0 += Cfg::kKC) {
+        const uint32_t buf = cc % kSgAccs, use = cc / kSgAccs;
+        ptx::mbar_wait(tfull0 + 8 * buf, use & 1u);
+        ptx::tc_fence_after();
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+          uint32_t raw[32];
+          ptx::tmem_ld32(tmem_base + ((q * 32u) << 16) + buf * 128u + 32u * h, raw);
+          ptx::tmem_ld_wait();
+          if (kb0 == 0) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) acc[32 * h + j] = __uint_as_float(raw[j]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) acc[32 * h + j] += __uint_as_float(raw[j]);
+          }
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(tempty0 + 8 * buf);
+        ++cc;
+      }
+      uint32_t emax = 0u;                                         // bits of max |v - delta| (NaN sorts above everything)
+      if (t.m0 + q * 32u < M) {
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          const uint32_t c0 = t.n0 + 32u * ch;
+          if (c0 < N) {
+          float* v = acc + 32 * ch;                                 // compile-time offsets: stays in registers
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] *= p.alpha;
+          if (pr->cin != nullptr && row_ok) {
+            const float4* src = reinterpret_cast<const float4*>(pr->cin + (size_t)r * pr->f32_pitch + c0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const float4 c = src[j];
+              v[4 * j] = fmaf(p.beta, c.x, v[4 * j]); v[4 * j + 1] = fmaf(p.beta, c.y, v[4 * j + 1]);
+              v[4 * j + 2] = fmaf(p.beta, c.z, v[4 * j + 2]); v[4 * j + 3] = fmaf(p.beta, c.w, v[4 * j + 3]);
+            }
+          }
+          if (pr->err != nullptr && row_ok) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j)
+              if (c0 + j < N) emax = max(emax, __float_as_uint(fabsf(v[j] - (c0 + j == r ? 1.f : 0.f))));
+          }
+          if (pr->out_f32 != nullptr && row_ok) {
+            if (!diag) {
+              float4* dst = reinterpret_cast<float4*>(pr->out_f32 + (size_t)r * pr->f32_pitch + c0);
+#pragma unroll
+              for (int j = 0; j < 8; ++j) dst[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N && c0 + j >= r) pr->out_f32[(size_t)r * pr->f32_pitch + c0 + j] = v[j];
+            }
+            if (mirror) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N && (!diag || c0 + j > r)) pr->out_f32[(size_t)(c0 + j) * pr->f32_pitch + r] = v[j];
+            }
+          }
+          if (pr->out_split != nullptr && row_ok) {
+            __nv_bfloat16* dst = pr->out_split + (size_t)r * pr->sp_pitch + c0;
+            if (!diag) {
+#pragma unroll
+              for (int g = 0; g < 4; ++g) sg::store_split8(dst + 8 * g, pr->sp_plane, v + 8 * g);
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, pr->sp_plane, v[j]);
+            }
+            if (mirror) {
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N && (!diag || c0 + j > r))
+                  sg::store_split1(pr->out_split + (size_t)(c0 + j) * pr->sp_pitch + r, pr->sp_plane, v[j]);
+            }
+          }
+          if (pr->t_split != nullptr && row_ok) {                     // T = (5 I - v) / 4
+            __nv_bfloat16* dst = pr->t_split + (size_t)r * pr->sp_pitch + c0;
+            if (!diag) {
+#pragma unroll
+              for (int g = 0; g < 4; ++g) {
+                float tv[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) tv[j] = 0.25f * ((c0 + 8 * g + j == r ? 5.f : 0.f) - v[8 * g + j]);
+                sg::store_split8(dst + 8 * g, pr->sp_plane, tv);
+              }
+            } else {
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N && c0 + j >= r)
+                  sg::store_split1(dst + j, pr->sp_plane, 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]));
+            }
+            if (mirror) {                                             // strictly off the diagonal
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N && (!diag || c0 + j > r))
+                  sg::store_split1(pr->t_split + (size_t)(c0 + j) * pr->sp_pitch + r, pr->sp_plane, -0.25f * v[j]);
+            }
+          }
+          if (pr->W != nullptr && row_ok) {
+            // W <- decay W - lr v (rank-flat, pitch = N: no padding, element-wise predicates at the right edge)
+            if (pr->w_bf16) {
+              __nv_bfloat16* w = reinterpret_cast<__nv_bfloat16*>(pr->W) + (size_t)r * N + c0;
+              if ((N & 7u) == 0u && c0 + 32u <= N) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  uint4 x = reinterpret_cast<const uint4*>(w)[j];
+                  uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                  for (int i = 0; i < 4; ++i) {
+                    const float w0 = __uint_as_float(xs[i] << 16), w1 = __uint_as_float(xs[i] & 0xffff0000u);
+                    const __nv_bfloat162 h = __floats2bfloat162_rn(fmaf(-p.lr, v[8 * j + 2 * i], p.decay * w0),
+                                                                   fmaf(-p.lr, v[8 * j + 2 * i + 1], p.decay * w1));
+                    xs[i] = *reinterpret_cast<const uint32_t*>(&h);
+                  }
+                  reinterpret_cast<uint4*>(w)[j] = make_uint4(xs[0], xs[1], xs[2], xs[3]);
+                }
+              } else {
+#pragma unroll
+                for (int j = 0; j < 32; ++j)
+                  if (c0 + j < N) w[j] = __float2bfloat16_rn(fmaf(-p.lr, v[j], p.decay * __bfloat162float(w[j])));
+              }
+            } else {
+              float* w = reinterpret_cast<float*>(pr->W) + (size_t)r * N + c0;
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (c0 + j < N) w[j] = fmaf(-p.lr, v[j], p.decay * w[j]);
+            }
+          }
+          }
+        }
+      }
+      if (pr->err != nullptr) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) emax = max(emax, __shfl_xor_sync(0xffffffffu, emax, o));
+        if (lane == 0 && emax != 0u) atomicMax(pr->err, emax);
+      }
+    }
+  }
+
+  __syncwarp();
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc<512, 1>(tmem_base);
+  }
+}
+
+}  // namespace mfsdp
+
+#endif  // MFSDP_SGEMM3_CUH_

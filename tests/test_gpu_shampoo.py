@@ -1,0 +1,203 @@
+"""GPU parity of the owner-local Shampoo step (`-m gpu`): mfsdp_shampoo_step through
+the C ABI against oracle/shampoo.py (fp64, roots by eigendecomposition) on the same seeded inputs.
+
+Tolerances ("Shampoo tolerances").  Statistics: fp32 sums of exact bf16 products, folded in
+64-element k chunks with round-to-nearest adds: relF(L), relF(R) <= 1e-6 (measured 1e-7), bit-symmetric.  Roots: the
+arithmetic (three-term bf16 operands, fp32 accumulation and state) perturbs S~ = S + rho I by about u ||S||_F with
+u = 2^-22 per product; an eigenvalue at the ridge moves by the relative amount u ||S||_F / rho and lambda^{-1/4} by a
+quarter of that.  With rho >= eps_floor ||S||_F = 2^-20 ||S||_F (reading S7) that bounds the relative error of P in
+its largest (ridge) directions by 2^-22 / 2^-20 / 4 = 6e-2 per product; asserted: relF(P) <= 2e-2 (measured <= 8e-3
+where the ridge is at the floor, 1e-6 .. 1e-3 otherwise).  D = P_L G P_R sees those directions only through the part
+of G that lies in them: relF(D) <= 2e-3 with fresh roots (measured <= 4e-4), and with a 30 x larger ridge (eps = 1e-3)
+relF(P), relF(D) <= 2e-3 also for stale roots.  W is checked lock-step from the GPU's own D with the rule of reading
+U1, and against the oracle's W in norm.  Measured values are printed."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2607_05895_b200 as mf
+import workloads
+from oracle import shampoo as oshampoo
+
+import gpu_harness as gh
+from helpers import bf16_rne, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+
+class ShampooSession:
+    def __init__(self, wl, ws_mode="full", **hp):
+        pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, wl.rank)
+        self.wl = wl
+        self.desc = mf.make_desc_array(pr.desc)
+        self.descs = [self.desc[i] for i in range(self.desc._n)]
+        self.mats = [d for d in self.descs if d.role == mf.ROLE_MATRIX]
+        self.flags = mf.SHAMPOO_KEEP_D
+        self.hp_kw = dict(lr=1e-3, weight_decay=0.01, beta2=1.0, eps=1e-6, eps_floor=2.0 ** -20, root_every=1)
+        self.hp_kw.update(hp)
+        self.n_mat_el, _ = mf.mfsdp_flat_elems(self.desc)
+        self.state = gh.aligned_bytes(mf.mfsdp_shampoo_state_bytes(self.desc))
+        self.state.zero_()
+        lo, hi = mf.mfsdp_shampoo_workspace_bytes(self.desc, self.flags)
+        self.ws = gh.aligned_bytes(lo if ws_mode == "min" else hi)
+        self.hW = workloads.fill_flat(wl, self.descs, workloads.KIND_W)
+        self.W = self.hW.cuda()
+        self.G = None
+        self.hG = None
+        # oracle state
+        self.oL = [np.zeros((d.rows, d.rows)) for d in self.mats]
+        self.oR = [np.zeros((d.cols, d.cols)) for d in self.mats]
+        self.oPL = [None] * len(self.mats)
+        self.oPR = [None] * len(self.mats)
+
+    def seg64(self, flat, d):
+        n = d.rows * d.cols
+        return flat[d.elem_off:d.elem_off + n].reshape(d.rows, d.cols).to(torch.float64).cpu().numpy()
+
+    def step(self, t):
+        self.hG = workloads.fill_flat(self.wl, self.descs, workloads.KIND_G, step=t)
+        self.G = self.hG.cuda()
+        hp = mf.ShampooHParams(step=t, flags=self.flags, **self.hp_kw)
+        mf.mfsdp_shampoo_step(self.desc, self.W, self.G, self.state, self.ws, hp)
+        torch.cuda.synchronize()
+
+    # ---- read-back ----
+    def view(self, i):
+        return mf.mfsdp_shampoo_view(self.desc, self.flags, i)
+
+    def read_f32(self, buf, off, rows, cols, pitch):
+        return buf[off:off + rows * pitch * 4].view(torch.float32).reshape(rows, pitch)[:, :cols].to(torch.float64).cpu().numpy()
+
+    def read_split(self, buf, off, rows, cols, pitch, plane):
+        raw = buf[off:off + 3 * plane * 2].view(torch.bfloat16).reshape(3, rows, pitch)[:, :, :cols].to(torch.float64)
+        return raw.sum(dim=0).cpu().numpy()
+
+    def read_all(self, i):
+        d = self.mats[i]
+        v = self.view(i)
+        L = self.read_f32(self.state, v[0], d.rows, d.rows, v[4])
+        R = self.read_f32(self.state, v[1], d.cols, d.cols, v[5])
+        PL = self.read_split(self.state, v[2], d.rows, d.rows, v[4], v[6])
+        PR = self.read_split(self.state, v[3], d.cols, d.cols, v[5], v[7])
+        D = self.read_f32(self.ws, v[8], d.rows, d.cols, v[5])
+        ctl = []
+        for k in range(2):
+            raw = self.ws[v[9] + k * v[10]: v[9] + (k + 1) * v[10]].cpu().numpy().tobytes()
+            tr, fro2 = np.frombuffer(raw[:16], dtype=np.float64)
+            rho, z, x0, last = np.frombuffer(raw[16:32], dtype=np.float32)
+            err, iters, done, ident = np.frombuffer(raw[32:48], dtype=np.uint32)
+            ctl.append(dict(tr=tr, rho=rho, z=z, last_err=float(last), iters=int(iters), done=int(done), identity=int(ident)))
+        return L, R, PL, PR, D, ctl
+
+
+def _run_and_check(sess, steps, tol_p, tol_d, label):
+    worst = dict(L=0.0, R=0.0, PL=0.0, PR=0.0, D=0.0)
+    for t in range(1, steps + 1):
+        W_old = [sess.seg64(sess.W, d) for d in sess.mats]
+        sess.step(t)
+        kw = sess.hp_kw
+        for i, d in enumerate(sess.mats):
+            G = sess.seg64(sess.hG, d)
+            out = oshampoo.shampoo_step(W_old[i], G, sess.oL[i], sess.oR[i], sess.oPL[i], sess.oPR[i], t, lr=kw["lr"],
+                                        weight_decay=kw["weight_decay"], beta2=kw["beta2"], eps=kw["eps"],
+                                        root_every=kw["root_every"], eps_floor=kw["eps_floor"])
+            sess.oL[i], sess.oR[i], sess.oPL[i], sess.oPR[i] = out["L"], out["R"], out["P_L"], out["P_R"]
+            L, R, PL, PR, D, ctl = sess.read_all(i)
+            e = dict(L=rel_fro(L, out["L"]), R=rel_fro(R, out["R"]), PL=rel_fro(PL, out["P_L"]),
+                     PR=rel_fro(PR, out["P_R"]), D=rel_fro(D, out["D"]))
+            print("%s step %d mat %d %dx%d: relF L %.1e R %.1e P_L %.1e P_R %.1e D %.1e | iters %d/%d err %.1e/%.1e done %d/%d"
+                  % (label, t, i, d.rows, d.cols, e["L"], e["R"], e["PL"], e["PR"], e["D"], ctl[0]["iters"],
+                     ctl[1]["iters"], ctl[0]["last_err"], ctl[1]["last_err"], ctl[0]["done"], ctl[1]["done"]))
+            for k in worst:
+                worst[k] = max(worst[k], e[k])
+            assert np.array_equal(L, L.T) and np.array_equal(R, R.T), "statistics must be bit-symmetric"
+            assert e["L"] <= 1e-6 and e["R"] <= 1e-6, (label, t, i, e)
+            assert e["PL"] <= tol_p and e["PR"] <= tol_p, (label, t, i, e, ctl)
+            assert e["D"] <= tol_d, (label, t, i, e)
+            assert ctl[0]["done"] == 1 and ctl[1]["done"] == 1, ctl
+            # lock-step update from the GPU's own D (reading U1): W = rn(decay W_old - lr D)
+            decay = np.float32(1.0 - kw["lr"] * kw["weight_decay"])
+            want = decay.astype(np.float64) * W_old[i] - np.float64(np.float32(kw["lr"])) * D
+            got = sess.seg64(sess.W, d)
+            if d.dtype == mf.BF16:
+                delta = 4 * 2.0 ** -24 * (np.abs(W_old[i]) + np.abs(kw["lr"] * D))
+                lo, hi = bf16_rne(want - delta).astype(np.float64), bf16_rne(want + delta).astype(np.float64)
+                assert np.all((got >= lo) & (got <= hi)), (label, t, i)
+                assert np.mean(got != bf16_rne(want).astype(np.float64)) <= 1e-3
+            else:
+                assert rel_fro(got, want) <= 1e-6
+            # and against the oracle's W within what the D tolerance allows
+            store = 2.0 ** -9 if d.dtype == mf.BF16 else 2.0 ** -24
+            assert np.linalg.norm(got - out["W"]) <= (kw["lr"] * tol_d * np.linalg.norm(out["D"])
+                                                      + store * np.linalg.norm(out["W"])), (label, t, i)
+    print(label, "worst", {k: "%.1e" % v for k, v in worst.items()})
+    return worst
+
+
+def test_shampoo_small_ragged_three_steps():
+    sess = ShampooSession(workloads.small_ragged())
+    _run_and_check(sess, 3, 2e-2, 2e-3, "small")
+
+
+def test_shampoo_medium_ragged_moving_average_stale_roots():
+    sess = ShampooSession(workloads.medium_ragged(), beta2=0.99, root_every=2, eps=1e-3)
+    _run_and_check(sess, 3, 2e-3, 2e-3, "medium")
+
+
+def test_shampoo_fp32_storage():
+    sess = ShampooSession(workloads.c1_tiny())
+    _run_and_check(sess, 2, 2e-2, 2e-3, "c1")
+
+
+def test_shampoo_grouped_workspace_is_bit_identical():
+    a = ShampooSession(workloads.small_ragged(), ws_mode="full")
+    b = ShampooSession(workloads.small_ragged(), ws_mode="min")
+    assert b.ws.numel() < a.ws.numel()
+    for t in (1, 2):
+        a.step(t)
+        b.step(t)
+    assert torch.equal(a.W.view(torch.int16), b.W.view(torch.int16))
+    assert torch.equal(a.state, b.state)
+
+
+def test_shampoo_zero_gradient_only_decays():
+    sess = ShampooSession(workloads.small_ragged(), weight_decay=0.1, lr=0.5)
+    W0 = sess.W.clone()
+    sess.hG = torch.zeros_like(sess.hW)
+    sess.G = sess.hG.cuda()
+    hp = mf.ShampooHParams(step=1, flags=sess.flags, **sess.hp_kw)
+    mf.mfsdp_shampoo_step(sess.desc, sess.W, sess.G, sess.state, sess.ws, hp)
+    torch.cuda.synchronize()
+    for i, d in enumerate(sess.mats):
+        L, R, PL, PR, D, ctl = sess.read_all(i)
+        assert ctl[0]["identity"] == 1 and ctl[1]["identity"] == 1
+        assert np.array_equal(PL, np.eye(d.rows)) and np.array_equal(PR, np.eye(d.cols))
+        assert not D.any()
+    want = bf16_rne(np.float32(0.95) * W0.float().cpu().numpy())
+    assert np.array_equal(sess.W.float().cpu().numpy(), want)
+
+
+def test_shampoo_run_to_run_determinism():
+    outs = []
+    for _ in range(2):
+        s = ShampooSession(workloads.medium_ragged(), eps=1e-4)
+        s.step(1)
+        s.step(2)
+        outs.append((s.W.clone(), s.state.clone()))
+    assert torch.equal(outs[0][0].view(torch.int16), outs[1][0].view(torch.int16))
+    assert torch.equal(outs[0][1], outs[1][1])
+
+
+def test_shampoo_argument_errors():
+    sess = ShampooSession(workloads.small_ragged())
+    sess.hG = workloads.fill_flat(sess.wl, sess.descs, workloads.KIND_G, step=1)
+    sess.G = sess.hG.cuda()
+    with pytest.raises(mf.MfsdpError) as e:
+        mf.mfsdp_shampoo_step(sess.desc, sess.W, sess.G, sess.state, sess.ws, mf.ShampooHParams(step=0))
+    assert e.value.code == mf.EINVAL
+    with pytest.raises(mf.MfsdpError) as e:
+        mf.mfsdp_shampoo_step(sess.desc, sess.W, sess.G, sess.state, sess.ws[:4096], mf.ShampooHParams(step=1))
+    assert e.value.code == mf.ECAP
+    with pytest.raises(mf.MfsdpError) as e:
+        mf.mfsdp_shampoo_step(sess.desc, sess.W, sess.G, sess.state[:1024], sess.ws, mf.ShampooHParams(step=1))
+    assert e.value.code == mf.ECAP

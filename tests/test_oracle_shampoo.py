@@ -171,3 +171,24 @@ def test_zero_gradient_only_decays():
     np.testing.assert_array_equal(out["D"], np.zeros((3, 4)))
     np.testing.assert_array_equal(out["P_L"], np.eye(3))
     np.testing.assert_allclose(out["W"], W0 * 0.99, rtol=1e-15)
+
+
+def test_ridge_floor_closed_form_and_switch():
+    # reading S7: rho = max(eps tr S / d, eps_floor ||S||_F).  S = diag(9, 16, 0): tr / d = 25 / 3, ||S||_F = sqrt(337)
+    S = np.diag([9.0, 16.0, 0.0])
+    eps, fl = 1e-3, 1e-2
+    rho_s2, rho_s7 = eps * 25 / 3, fl * np.sqrt(337.0)
+    assert rho_s7 > rho_s2
+    P = shampoo.inverse_root(S, eps, eps_floor=fl)
+    np.testing.assert_allclose(P, np.diag([(9 + rho_s7) ** -0.25, (16 + rho_s7) ** -0.25, rho_s7 ** -0.25]), rtol=1e-14)
+    # the floor is inactive when the S2 ridge is the larger one, and off by default
+    P2 = shampoo.inverse_root(S, eps, eps_floor=1e-6)
+    np.testing.assert_allclose(P2, np.diag([(9 + rho_s2) ** -0.25, (16 + rho_s2) ** -0.25, rho_s2 ** -0.25]), rtol=1e-14)
+    np.testing.assert_array_equal(shampoo.inverse_root(S, eps), P2)
+    # the step passes it to both roots
+    G = np.array([[2.0, 0, 0], [0, 3.0, 0]])
+    out = shampoo.shampoo_step(np.zeros((2, 3)), G, np.zeros((2, 2)), np.zeros((3, 3)), None, None, 1, eps=0.0,
+                               eps_floor=0.1)
+    rl = rr = 0.1 * np.sqrt(16.0 + 81.0)
+    np.testing.assert_allclose(out["D"][0, 0], 2 * (4 + rl) ** -0.25 * (4 + rr) ** -0.25, rtol=1e-14)
+    np.testing.assert_allclose(out["P_R"][2, 2], rr ** -0.25, rtol=1e-14)
