@@ -49,6 +49,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--shampoo", default=None, choices=["c1", "c2", "c3", "c4", "paper16l"],
+                    help="time only the owner-local Shampoo step (PAPER.md:182) on this config and print its record "
+                         "(the `other_configs` entry; used for profiling)")
     return ap.parse_args()
 
 
@@ -446,6 +449,74 @@ def measure_other_config(torch, mf, name, pk, local, paper=False, reuse=None):
     return rec
 
 
+def measure_shampoo(torch, mf, name, pk, local, ws_cap_bytes=64e9):
+    """One record of `other_configs` for the owner-local Shampoo step on a
+    BASELINE.json config: step 1 recomputes every inverse fourth root (root_every = 2), step 2 reuses them.  Flops are
+    counted from the iteration counts the device reports: fp32-class flops (symmetric products count once) and the
+    bf16 UMMA flops actually issued for them (x6 for three-term operands, x3 / x1 where the bf16 gradient is one term),
+    the latter against the bf16 tensor peak."""
+    import numpy as np
+    import workloads
+    wl = workloads.get(name)
+    pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, choose_plan_rank(rank_order_by_load(mf, wl), wl.rank, 0, 1))
+    desc = pr.desc
+    descs = [desc[i] for i in range(desc._n)]
+    mats = [d for d in descs if d.role == mf.ROLE_MATRIX]
+
+    def aligned(nbytes):
+        raw = torch.empty(nbytes + 1024, dtype=torch.uint8, device="cuda")
+        off = (-raw.data_ptr()) % 1024
+        out = raw[off:off + nbytes]
+        out._keep = raw
+        return out
+    state = aligned(mf.mfsdp_shampoo_state_bytes(desc))
+    state.zero_()
+    lo, hi = mf.mfsdp_shampoo_workspace_bytes(desc, 0)
+    ws = aligned(int(max(lo, min(hi, ws_cap_bytes))))
+    W = workloads.fill_flat(wl, descs, workloads.KIND_W).cuda()
+    gt = 1 if wl.dtype == mf.BF16 else 3
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(local)
+    sampler.start()
+    recs = []
+    for t in (1, 2):
+        G = workloads.fill_flat(wl, descs, workloads.KIND_G, step=t).cuda()
+        torch.cuda.synchronize()
+        n0 = mf.mfsdp_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        mf.mfsdp_shampoo_step(desc, W, G, state, ws, mf.ShampooHParams(step=t, root_every=2), stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        f32 = umma = 0.0
+        iters = []
+        for i, d in enumerate(mats):
+            v = mf.mfsdp_shampoo_view(desc, 0, i)
+            raw = ws[v[9]: v[9] + 2 * v[10]].cpu().numpy().tobytes()
+            for k, dd in enumerate((d.rows, d.cols)):
+                it = int(np.frombuffer(raw[k * v[10] + 36: k * v[10] + 40], dtype=np.uint32)[0])
+                iters.append(it)
+                if t == 1:
+                    f32 += it * 4.0 * dd ** 3                    # four symmetric d x d x d products per iteration
+                    umma += it * 4.0 * dd ** 3 * 6
+            stat = float(d.rows) * d.rows * d.cols + float(d.cols) * d.cols * d.rows
+            p1, p2 = 2.0 * d.rows * d.rows * d.cols, 2.0 * d.rows * d.cols * d.cols
+            f32 += stat + p1 + p2
+            umma += stat * gt * (gt + 1) / 2 + p1 * 3 * (1 if gt == 1 else 2) + p2 * 6
+        recs.append(dict(ms=ms, launches=mf.mfsdp_launch_count() - n0, f32_class_tflops=f32 / ms / 1e9,
+                         umma_bf16_tflops=umma / ms / 1e9, root_iters_max=max(iters), root_iters_mean=float(np.mean(iters))))
+    clocks = sampler.stop()
+    capped = "sw_power_cap" in clocks.get("reasons", [])
+    peak = pk["tc_sustained"] if capped else pk["tc_burst"]
+    return dict(workload=wl.name, optimizer="owner-local Shampoo (PAPER.md:182): full L / R, inverse fourth roots by coupled "
+                "Newton, fp32-class GEMMs as three-term bf16 on tcgen05", refresh_step=recs[0], stale_step=recs[1],
+                refresh_frac_of_bf16_peak=recs[0]["umma_bf16_tflops"] / peak,
+                frac_of="sustained bf16 peak (sw_power_cap sampled)" if capped else "burst bf16 peak",
+                state_gb=state.numel() / 1e9, workspace_gb=ws.numel() / 1e9, n_matrices=len(mats),
+                clocks=dict(sm_mhz=clocks.get("sm_mhz"), reasons=clocks.get("reasons")))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -462,6 +533,9 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     mf.load()
 
+    if args.shampoo:
+        print(json.dumps(measure_shampoo(torch, mf, args.shampoo, peaks(), local)))
+        return
     wl = apply_setting(workloads.get(args.config), args)
     order = rank_order_by_load(mf, wl)
     plan_rank = choose_plan_rank(order, wl.rank, rank, world)
@@ -560,6 +634,12 @@ def run_ours(args):
                 others.append(measure_other_config(torch, mf, name, pk, local, paper=(name == "paper16l")))
             except Exception as e:
                 others.append(dict(workload=name, error=repr(e)))
+            torch.cuda.empty_cache()
+        for name in ("c2", "c4"):
+            try:
+                others.append(measure_shampoo(torch, mf, name, pk, local))
+            except Exception as e:
+                others.append(dict(workload=name + "+shampoo", error=repr(e)))
             torch.cuda.empty_cache()
         line["other_configs"] = others
     if not args.no_cpu_baseline and world == 1:

@@ -43,7 +43,7 @@ def demangle(name):
 
 
 def main():
-    objs = sys.argv[1:] or [os.path.join(PKG, "build", f) for f in ("ns_tc.o", "ns_fused.o", "ns_fused2.o", "elementwise.o")]
+    objs = sys.argv[1:] or [os.path.join(PKG, "build", f) for f in ("ns_tc.o", "ns_fused.o", "ns_fused2.o", "shampoo.o", "elementwise.o")]
     for obj in objs:
         print("== %s (sm_100a)" % os.path.relpath(obj, os.path.dirname(PKG)))
         for fn, h in histogram(obj).items():

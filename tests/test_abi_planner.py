@@ -311,3 +311,51 @@ def test_gated_step_and_signal_reject_bad_arguments_without_a_gpu():
     assert lib.mfsdp_muon_step_gated(pr.desc, pr.desc._n, 1024, 1024, 1024, 1024, 1 << 30, ctypes.byref(hp), 1026, 1,
                                      None) == mf.EINVAL                      # misaligned flags
     assert lib.mfsdp_signal_ready(None, 0, 1, None) == mf.EINVAL
+
+
+def test_shampoo_layout_and_argument_checks_without_a_gpu():
+    """mfsdp_shampoo_state_bytes / _workspace_bytes / _view are host-only; the step checks its arguments before any
+    CUDA call and answers MFSDP_EARCH without a device (no CPU fallback)."""
+    assert ctypes.sizeof(mf.ShampooHParams) == 6 * 8 + 8 + 4 * 4
+    lib = mf.load()
+    wl = workloads.get("small")
+    pr = mf.mfsdp_plan(wl.params, 1)
+    n = pr.desc._n
+    mats = [pr.desc[j] for j in range(n) if pr.desc[j].role == mf.ROLE_MATRIX]
+    total = mf.mfsdp_shampoo_state_bytes(pr.desc)
+    spans = []
+    for i, d in enumerate(mats):
+        v = mf.mfsdp_shampoo_view(pr.desc, mf.SHAMPOO_KEEP_D, i)
+        pr_, pc_ = v[4], v[5]
+        assert pr_ >= d.rows and pc_ >= d.cols and pr_ % 64 == 0 and pc_ % 64 == 0
+        assert v[6] == d.rows * pr_ and v[7] == d.cols * pc_ and v[10] == 48
+        for off, nbytes in ((v[0], d.rows * pr_ * 4), (v[1], d.cols * pc_ * 4), (v[2], 3 * v[6] * 2), (v[3], 3 * v[7] * 2)):
+            assert off % 1024 == 0 and off + nbytes <= total
+            spans.append((off, off + nbytes))
+    spans.sort()
+    for (a0, a1), (b0, b1) in zip(spans, spans[1:]):
+        assert a1 <= b0, "state buffers overlap"
+    lo, hi = mf.mfsdp_shampoo_workspace_bytes(pr.desc, 0)
+    lo_d, hi_d = mf.mfsdp_shampoo_workspace_bytes(pr.desc, mf.SHAMPOO_KEEP_D)
+    dmax = max(max(d.rows, d.cols) for d in mats)
+    assert lo < hi and lo_d > lo and hi_d - hi == lo_d - lo
+    assert lo >= 7 * 3 * dmax * dmax * 2, "the smallest workspace holds the seven three-plane buffers of the largest root"
+    with pytest.raises(mf.MfsdpError):
+        mf.mfsdp_shampoo_view(pr.desc, 0, len(mats))
+    with pytest.raises(mf.MfsdpError):
+        mf.mfsdp_shampoo_workspace_bytes(pr.desc, 2)
+    # the step: argument checks first
+    ok = mf.ShampooHParams(step=1)
+    call = lambda hp, W=1024, G=1024, st=1024, ws=1024: lib.mfsdp_shampoo_step(pr.desc, n, W, G, st, 1 << 40, ws, 1 << 40,
+                                                                                 ctypes.byref(hp) if hp else None, None)
+    assert call(None) == mf.EINVAL
+    for bad in (dict(step=0), dict(root_every=0), dict(beta2=0.0), dict(beta2=1.5), dict(eps=-1.0), dict(eps_floor=-1.0),
+                dict(max_root_iters=-1), dict(flags=4)):
+        assert call(mf.ShampooHParams(**dict(dict(step=1), **bad))) == mf.EINVAL, bad
+    assert call(ok, W=None) == mf.EINVAL and call(ok, st=1000) == mf.EINVAL and call(ok, ws=1032) == mf.EINVAL
+    import torch
+    if not torch.cuda.is_available():
+        assert call(ok) == mf.EARCH
+    # a table without matrices is a no-op
+    tails = mf.make_desc_array([pr.desc[j] for j in range(n) if pr.desc[j].role == mf.ROLE_TAIL])
+    assert lib.mfsdp_shampoo_step(tails, tails._n, None, None, None, 0, None, 0, ctypes.byref(ok), None) == 0
