@@ -201,3 +201,38 @@ def test_shampoo_argument_errors():
     with pytest.raises(mf.MfsdpError) as e:
         mf.mfsdp_shampoo_step(sess.desc, sess.W, sess.G, sess.state[:1024], sess.ws, mf.ShampooHParams(step=1))
     assert e.value.code == mf.ECAP
+
+
+def test_shampoo_c2_shapes_full_oracle():
+    """One matrix of every distinct shape of BASELINE.json config 2 (GPT-2-small: 768 x 2304, 768 x 768, 768 x 3072,
+    3072 x 768) against the oracle, two steps: roots up to 3072 x 3072 (24 x 24 tiles, 48 k chunks per tile)."""
+    shapes = [(768, 2304), (768, 768), (768, 3072), (3072, 768)]
+    wl = workloads.Workload("c2_shapes", [(i, 2, r, c, workloads.BF16, 0) for i, (r, c) in enumerate(shapes)], seed=1)
+    sess = ShampooSession(wl)
+    _run_and_check(sess, 2, 2e-2, 2e-3, "c2shapes")
+
+
+def test_shampoo_step_is_graph_capturable():
+    """The step enqueues a fixed launch sequence and never synchronises: once its launch tables exist it can be
+    captured into a CUDA graph; replaying the graph gives the bits of the eager step."""
+    a = ShampooSession(workloads.medium_ragged(), eps=1e-3)
+    b = ShampooSession(workloads.medium_ragged(), eps=1e-3)
+    hG = workloads.fill_flat(a.wl, a.descs, workloads.KIND_G, step=1)
+    a.G, b.G = hG.cuda(), hG.cuda()
+    hp = mf.ShampooHParams(step=1, flags=a.flags, **a.hp_kw)
+    mf.mfsdp_shampoo_step(a.desc, a.W, a.G, a.state, a.ws, hp)          # eager
+    torch.cuda.synchronize()
+    W0, st0 = b.W.clone(), b.state.clone()
+    mf.mfsdp_shampoo_step(b.desc, b.W, b.G, b.state, b.ws, hp)          # builds b's tables
+    torch.cuda.synchronize()
+    b.W.copy_(W0)
+    b.state.copy_(st0)
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            mf.mfsdp_shampoo_step(b.desc, b.W, b.G, b.state, b.ws, hp, s)
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(a.W.view(torch.int16), b.W.view(torch.int16))
+    assert torch.equal(a.state, b.state)
