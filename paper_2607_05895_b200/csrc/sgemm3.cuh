@@ -74,7 +74,7 @@ constexpr uint32_t kSgBox = 16384;  // one term of one operand of one stage: 128
 template <int AT, int BT> struct SgCfg {
   static constexpr uint32_t kStage = (AT + BT) * kSgBox;
   static constexpr uint32_t kStages = (AT + BT) == 2 ? 6 : (AT + BT) == 4 ? 3 : 2;
-  static constexpr uint32_t kSmem = kStages * kStage + 256 + 1024;
+  static constexpr uint32_t kSmem = kStages * kStage + 256 + 1024 + 8 * 32 * 33 * 4;   // ring, barriers, alignment, 8 transposition tiles
   // k blocks per TMEM chunk.  One: at most four truncating adds of leading-term products per partial sum.  (With one
   // term per operand a block is 256 cycles of UMMA, less than the epilogue warps need to fold it -- 4 tcgen05.ld of 32
   // columns + 128 adds -- so the statistics GEMM of a bf16 gradient runs fold-bound; it is a few percent of a step.)
@@ -119,6 +119,157 @@ __device__ __forceinline__ void store_split1(__nv_bfloat16* d, uint64_t plane, f
   d[2 * plane] = __ushort_as_bfloat16((unsigned short)b3);
 }
 }  // namespace sg
+
+
+// The stores of one thread's row of a tile: `acc` = 128 consecutive columns starting at n0 of output row r (this warp's
+// rows start at row0, a multiple of 32), already summed over k.  Worked through in chunks of 32 columns, groups of 8
+// inside, to keep few values live beside the 128 accumulators.  The mirror image of a symmetric output goes through
+// `tbuf` (32 x 33 floats of shared memory per warp): the warp's 32 x 32 block is transposed there, so that a lane owns
+// 32 consecutive elements of one mirrored row and stores them as 16-byte vectors like the direct image (element-wise
+// scattered 2-byte stores of the three planes cost more than the UMMAs of a short-k tile).
+__device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& p, float (&acc)[128], uint32_t row0,
+                                              uint32_t r, uint32_t n0, bool mirror, bool diag, uint32_t lane,
+                                              uint32_t tbuf) {
+  const uint32_t M = pr->M, N = pr->N;
+  const bool row_ok = r < M;
+  uint32_t emax = 0u;                                         // bits of max |v - delta| (NaN sorts above everything)
+  if (row0 >= M) return;                                      // warp-uniform
+  const float* cin = pr->cin;
+  float* of32 = pr->out_f32;
+  __nv_bfloat16* osp = pr->out_split;
+  __nv_bfloat16* tsp = pr->t_split;
+  const uint32_t* errp = pr->err;
+  const uint32_t fp = pr->f32_pitch, spp = pr->sp_pitch;
+  const uint64_t plane = pr->sp_plane;
+#pragma unroll
+  for (int ch = 0; ch < 4; ++ch) {
+    const uint32_t cb = n0 + 32u * ch;
+    if (cb >= N) continue;                                    // warp-uniform
+#pragma unroll
+    for (int gg = 0; gg < 4; ++gg) {
+      const int g = 4 * ch + gg;
+      const uint32_t c0 = n0 + 8u * g;
+      float* v = acc + 8 * g;                                   // compile-time offsets: stays in registers
+#pragma unroll
+      for (int j = 0; j < 8; ++j) v[j] *= p.alpha;
+      if (!row_ok) continue;
+      if (cin != nullptr) {
+        const float4* src = reinterpret_cast<const float4*>(cin + (size_t)r * fp + c0);
+        const float4 a = src[0], b = src[1];
+        v[0] = fmaf(p.beta, a.x, v[0]); v[1] = fmaf(p.beta, a.y, v[1]); v[2] = fmaf(p.beta, a.z, v[2]); v[3] = fmaf(p.beta, a.w, v[3]);
+        v[4] = fmaf(p.beta, b.x, v[4]); v[5] = fmaf(p.beta, b.y, v[5]); v[6] = fmaf(p.beta, b.z, v[6]); v[7] = fmaf(p.beta, b.w, v[7]);
+      }
+      if (errp != nullptr) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          if (c0 + j < N) emax = max(emax, __float_as_uint(fabsf(v[j] - (c0 + j == r ? 1.f : 0.f))));
+      }
+      if (of32 != nullptr) {
+        if (!diag) {
+          float4* dst = reinterpret_cast<float4*>(of32 + (size_t)r * fp + c0);
+          dst[0] = make_float4(v[0], v[1], v[2], v[3]);
+          dst[1] = make_float4(v[4], v[5], v[6], v[7]);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            if (c0 + j < N && c0 + j >= r) of32[(size_t)r * fp + c0 + j] = v[j];
+            if (c0 + j < N && c0 + j > r) of32[(size_t)(c0 + j) * fp + r] = v[j];
+          }
+        }
+      }
+      if (osp != nullptr) {
+        __nv_bfloat16* dst = osp + (size_t)r * spp + c0;
+        if (!diag) sg::store_split8(dst, plane, v);
+        else {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, plane, v[j]);
+            if (c0 + j < N && c0 + j > r) sg::store_split1(osp + (size_t)(c0 + j) * spp + r, plane, v[j]);
+          }
+        }
+      }
+      if (tsp != nullptr) {                                       // T = (5 I - v) / 4
+        __nv_bfloat16* dst = tsp + (size_t)r * spp + c0;
+        if (!diag) {
+          float tv[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) tv[j] = 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]);
+          sg::store_split8(dst, plane, tv);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, plane, 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]));
+            if (c0 + j < N && c0 + j > r) sg::store_split1(tsp + (size_t)(c0 + j) * spp + r, plane, -0.25f * v[j]);
+          }
+        }
+      }
+      if (pr->W != nullptr) {
+        // W <- decay W - lr v (rank-flat, pitch = N: no padding, element-wise predicates at the right edge)
+        if (pr->w_bf16) {
+          __nv_bfloat16* w = reinterpret_cast<__nv_bfloat16*>(pr->W) + (size_t)r * N + c0;
+          if ((N & 7u) == 0u) {                                   // then c0 + 8 <= N
+            if (c0 < N) {
+              const uint4 x = *reinterpret_cast<const uint4*>(w);
+              uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const float w0 = __uint_as_float(xs[i] << 16), w1 = __uint_as_float(xs[i] & 0xffff0000u);
+                const __nv_bfloat162 h = __floats2bfloat162_rn(fmaf(-p.lr, v[2 * i], p.decay * w0),
+                                                               fmaf(-p.lr, v[2 * i + 1], p.decay * w1));
+                xs[i] = *reinterpret_cast<const uint32_t*>(&h);
+              }
+              *reinterpret_cast<uint4*>(w) = make_uint4(xs[0], xs[1], xs[2], xs[3]);
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+              if (c0 + j < N) w[j] = __float2bfloat16_rn(fmaf(-p.lr, v[j], p.decay * __bfloat162float(w[j])));
+          }
+        } else {
+          float* w = reinterpret_cast<float*>(pr->W) + (size_t)r * N + c0;
+#pragma unroll
+          for (int j = 0; j < 8; ++j)
+            if (c0 + j < N) w[j] = fmaf(-p.lr, v[j], p.decay * w[j]);
+        }
+      }
+    }
+    if (mirror && !diag) {
+      // transpose this warp's 32 x 32 block: lane l ends up with column cb + l of rows row0 .. row0 + 31, i.e. with 32
+      // consecutive elements of mirrored row cb + l.  (rows >= M hold alpha * 0 = 0 and land in the pitch padding)
+      float* v = acc + 32 * ch;
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < 32; ++j) ptx::st_shared_u32(tbuf + (lane * 33u + j) * 4u, __float_as_uint(row_ok ? v[j] : 0.f));
+      __syncwarp();
+      float w[32];
+#pragma unroll
+      for (int i = 0; i < 32; ++i) w[i] = __uint_as_float(ptx::ld_shared_u32(tbuf + (i * 33u + lane) * 4u));
+      const uint32_t mr = cb + lane;
+      if (mr < N) {
+        if (of32 != nullptr) {
+          float4* dst = reinterpret_cast<float4*>(of32 + (size_t)mr * fp + row0);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) dst[j] = make_float4(w[4 * j], w[4 * j + 1], w[4 * j + 2], w[4 * j + 3]);
+        }
+        if (osp != nullptr) {
+#pragma unroll
+          for (int g = 0; g < 4; ++g) sg::store_split8(osp + (size_t)mr * spp + row0 + 8 * g, plane, w + 8 * g);
+        }
+        if (tsp != nullptr) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) w[i] *= -0.25f;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) sg::store_split8(tsp + (size_t)mr * spp + row0 + 8 * g, plane, w + 8 * g);
+        }
+      }
+    }
+  }
+  if (errp != nullptr) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) emax = max(emax, __shfl_xor_sync(0xffffffffu, emax, o));
+    if (lane == 0 && emax != 0u) atomicMax(pr->err, emax);
+  }
+}
 
 template <int AT, int BT>
 __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
@@ -195,30 +346,33 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
         for (uint32_t kb = kb0; kb < kb1; ++kb) {
           ptx::mbar_wait(full0 + 8 * stage, ring_phase);
           ptx::tc_fence_after();
-          const uint32_t ksteps = min(4u, (K - 64u * kb + 15u) >> 4);
+          // Descriptors are formed in warp-uniform code and every UMMA of the block is unrolled with constant offsets
+          // (always four k steps: a ragged last block reads TMA's zero fill), so that the elected lane issues from
+          // uniform registers without per-instruction register moves (~200 cycles per UMMA otherwise: issue-bound).
           const uint32_t base = ring0 + stage * Cfg::kStage;
+          uint64_t ad[AT], bd[BT];
+#pragma unroll
+          for (int i = 0; i < AT; ++i) ad[i] = ptx::smem_desc_sw128(base + i * kSgBox, a_lbo, 1024);
+#pragma unroll
+          for (int j = 0; j < BT; ++j) bd[j] = ptx::smem_desc_sw128(base + (AT + j) * kSgBox, b_lbo, 1024);
           if (ptx::elect_one()) {
-            uint32_t fresh = kb == kb0 ? 0u : 1u;                  // the first UMMA of a chunk overwrites the accumulator
             // the small term products first, the leading one last (see "Accumulation" above)
+            bool first = true;
 #pragma unroll
             for (int i = 0; i < AT; ++i)
 #pragma unroll
               for (int j = 0; j < BT; ++j)
                 if (i + j <= 2 && i + j > 0) {
-                  const uint64_t ad0 = ptx::smem_desc_sw128(base + i * kSgBox, a_lbo, 1024);
-                  const uint64_t bd0 = ptx::smem_desc_sw128(base + (AT + j) * kSgBox, b_lbo, 1024);
-                  for (uint32_t ks = 0; ks < ksteps; ++ks) {
-                    ptx::umma_bf16(d_tmem, ad0 + (uint64_t)(ks * a_step), bd0 + (uint64_t)(ks * b_step), idesc, fresh);
-                    fresh = 1u;
+#pragma unroll
+                  for (uint32_t ks = 0; ks < 4; ++ks) {
+                    ptx::umma_bf16(d_tmem, ad[i] + (uint64_t)(ks * a_step), bd[j] + (uint64_t)(ks * b_step), idesc, first ? 0u : 1u);
+                    first = false;
                   }
                 }
-            {
-              const uint64_t ad0 = ptx::smem_desc_sw128(base, a_lbo, 1024);
-              const uint64_t bd0 = ptx::smem_desc_sw128(base + AT * kSgBox, b_lbo, 1024);
-              for (uint32_t ks = 0; ks < ksteps; ++ks) {
-                ptx::umma_bf16(d_tmem, ad0 + (uint64_t)(ks * a_step), bd0 + (uint64_t)(ks * b_step), idesc, fresh);
-                fresh = 1u;
-              }
+#pragma unroll
+            for (uint32_t ks = 0; ks < 4; ++ks) {
+              ptx::umma_bf16(d_tmem, ad[0] + (uint64_t)(ks * a_step), bd[0] + (uint64_t)(ks * b_step), idesc, first ? 0u : 1u);
+              first = false;
             }
             ptx::umma_commit(empty0 + 8 * stage);
             if (kb + 1 == kb1) ptx::umma_commit(tfull0 + 8 * buf);
@@ -231,9 +385,7 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
     } else {
       // ===== epilogue: warp owns TMEM lanes 32 q .. + 31 = rows m0 + 32 q .. of the tile =====
       const uint32_t q = warp & 3u;
-      const uint32_t M = pr->M, N = pr->N;
       const uint32_t r = t.m0 + q * 32u + lane;
-      const bool row_ok = r < M;
       // symmetric outputs: a tile above the block diagonal also stores its mirror image; a tile ON the diagonal stores
       // its upper triangle (c >= r) and the mirror of the strict upper triangle, so that the result is bit-symmetric
       // (with several terms the two triangles of a diagonal tile are summed in different orders)
@@ -263,123 +415,8 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
         if (lane == 0) ptx::mbar_arrive(tempty0 + 8 * buf);
         ++cc;
       }
-      uint32_t emax = 0u;                                         // bits of max |v - delta| (NaN sorts above everything)
-      if (t.m0 + q * 32u < M) {
-#pragma unroll
-        for (int ch = 0; ch < 4; ++ch) {
-          const uint32_t c0 = t.n0 + 32u * ch;
-          if (c0 < N) {
-          float* v = acc + 32 * ch;                                 // compile-time offsets: stays in registers
-#pragma unroll
-          for (int j = 0; j < 32; ++j) v[j] *= p.alpha;
-          if (pr->cin != nullptr && row_ok) {
-            const float4* src = reinterpret_cast<const float4*>(pr->cin + (size_t)r * pr->f32_pitch + c0);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              const float4 c = src[j];
-              v[4 * j] = fmaf(p.beta, c.x, v[4 * j]); v[4 * j + 1] = fmaf(p.beta, c.y, v[4 * j + 1]);
-              v[4 * j + 2] = fmaf(p.beta, c.z, v[4 * j + 2]); v[4 * j + 3] = fmaf(p.beta, c.w, v[4 * j + 3]);
-            }
-          }
-          if (pr->err != nullptr && row_ok) {
-#pragma unroll
-            for (int j = 0; j < 32; ++j)
-              if (c0 + j < N) emax = max(emax, __float_as_uint(fabsf(v[j] - (c0 + j == r ? 1.f : 0.f))));
-          }
-          if (pr->out_f32 != nullptr && row_ok) {
-            if (!diag) {
-              float4* dst = reinterpret_cast<float4*>(pr->out_f32 + (size_t)r * pr->f32_pitch + c0);
-#pragma unroll
-              for (int j = 0; j < 8; ++j) dst[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
-            } else {
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N && c0 + j >= r) pr->out_f32[(size_t)r * pr->f32_pitch + c0 + j] = v[j];
-            }
-            if (mirror) {
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N && (!diag || c0 + j > r)) pr->out_f32[(size_t)(c0 + j) * pr->f32_pitch + r] = v[j];
-            }
-          }
-          if (pr->out_split != nullptr && row_ok) {
-            __nv_bfloat16* dst = pr->out_split + (size_t)r * pr->sp_pitch + c0;
-            if (!diag) {
-#pragma unroll
-              for (int g = 0; g < 4; ++g) sg::store_split8(dst + 8 * g, pr->sp_plane, v + 8 * g);
-            } else {
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, pr->sp_plane, v[j]);
-            }
-            if (mirror) {
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N && (!diag || c0 + j > r))
-                  sg::store_split1(pr->out_split + (size_t)(c0 + j) * pr->sp_pitch + r, pr->sp_plane, v[j]);
-            }
-          }
-          if (pr->t_split != nullptr && row_ok) {                     // T = (5 I - v) / 4
-            __nv_bfloat16* dst = pr->t_split + (size_t)r * pr->sp_pitch + c0;
-            if (!diag) {
-#pragma unroll
-              for (int g = 0; g < 4; ++g) {
-                float tv[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) tv[j] = 0.25f * ((c0 + 8 * g + j == r ? 5.f : 0.f) - v[8 * g + j]);
-                sg::store_split8(dst + 8 * g, pr->sp_plane, tv);
-              }
-            } else {
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N && c0 + j >= r)
-                  sg::store_split1(dst + j, pr->sp_plane, 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]));
-            }
-            if (mirror) {                                             // strictly off the diagonal
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N && (!diag || c0 + j > r))
-                  sg::store_split1(pr->t_split + (size_t)(c0 + j) * pr->sp_pitch + r, pr->sp_plane, -0.25f * v[j]);
-            }
-          }
-          if (pr->W != nullptr && row_ok) {
-            // W <- decay W - lr v (rank-flat, pitch = N: no padding, element-wise predicates at the right edge)
-            if (pr->w_bf16) {
-              __nv_bfloat16* w = reinterpret_cast<__nv_bfloat16*>(pr->W) + (size_t)r * N + c0;
-              if ((N & 7u) == 0u && c0 + 32u <= N) {
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                  uint4 x = reinterpret_cast<const uint4*>(w)[j];
-                  uint32_t xs[4] = {x.x, x.y, x.z, x.w};
-#pragma unroll
-                  for (int i = 0; i < 4; ++i) {
-                    const float w0 = __uint_as_float(xs[i] << 16), w1 = __uint_as_float(xs[i] & 0xffff0000u);
-                    const __nv_bfloat162 h = __floats2bfloat162_rn(fmaf(-p.lr, v[8 * j + 2 * i], p.decay * w0),
-                                                                   fmaf(-p.lr, v[8 * j + 2 * i + 1], p.decay * w1));
-                    xs[i] = *reinterpret_cast<const uint32_t*>(&h);
-                  }
-                  reinterpret_cast<uint4*>(w)[j] = make_uint4(xs[0], xs[1], xs[2], xs[3]);
-                }
-              } else {
-#pragma unroll
-                for (int j = 0; j < 32; ++j)
-                  if (c0 + j < N) w[j] = __float2bfloat16_rn(fmaf(-p.lr, v[j], p.decay * __bfloat162float(w[j])));
-              }
-            } else {
-              float* w = reinterpret_cast<float*>(pr->W) + (size_t)r * N + c0;
-#pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (c0 + j < N) w[j] = fmaf(-p.lr, v[j], p.decay * w[j]);
-            }
-          }
-          }
-        }
-      }
-      if (pr->err != nullptr) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) emax = max(emax, __shfl_xor_sync(0xffffffffu, emax, o));
-        if (lane == 0 && emax != 0u) atomicMax(pr->err, emax);
-      }
+      sg_finish_row(pr, p, acc, t.m0 + q * 32u, r, t.n0, mirror, diag, lane,
+                    ring0 + Cfg::kStages * Cfg::kStage + 256u + (warp - 2u) * (32u * 33u * 4u));
     }
   }
 
@@ -389,6 +426,212 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
   if (warp == 1) {
     ptx::tc_fence_after();
     ptx::tmem_dealloc<512, 1>(tmem_base);
+  }
+}
+
+
+// ---- CTA-pair form ---------------------------------------------------------------------------------------------------
+// The same product on 256 x 256 tiles owned by a cluster of two CTAs (tcgen05 cta_group::2: M = 256 over the two SMs,
+// each CTA stages its 128 rows of A and its 128 rows of B per term and k block).  Per CTA and k block that is the same
+// 96 KB of operands as the single-CTA tile for TWICE the UMMA time (6 x 4 UMMAs of 128 cycles): 31 B/clk/SM asked of
+// the L2 -> SM path instead of 62, which is what keeps the single-CTA form at 52-59 % tensor-pipe activity.  Each CTA
+// holds its 128 rows x 256 columns of the chunk accumulator (2 x 256 TMEM columns); eight epilogue warps per CTA fold
+// and store it (warps w and w + 4 share a TMEM lane quarter and split the columns).  384 threads leave 168 registers
+// per thread, too few beside 128 accumulators: the control warpgroup (producer, issuer, two idle warps) gives its
+// registers back (setmaxnreg.dec 40) and the two epilogue warpgroups take them (setmaxnreg.inc 232).  Used when a
+// launch has at least ~ one wave of 256-tiles; small problem sets stay on the single-CTA kernel.
+#ifndef MFSDP_SG_PROBE
+#define MFSDP_SG_PROBE 0   // timing probes of the pair kernel (results wrong): 1 no loads after the first ring fill, 2 no fold, 3 no UMMAs
+#endif
+constexpr uint32_t kSgPairThreads = 384;   // warps 0-7 epilogue (two warpgroups), 8 producer, 9 UMMA issuer, 10-11 idle
+namespace sg {
+__device__ __forceinline__ void tma_load_3d_cg2(uint32_t dst, const void* tmap, int c0, int c1, int c2, uint32_t bar_cluster) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], "
+      "[%5];" ::"r"(dst),
+      "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar_cluster)
+      : "memory");
+}
+}  // namespace sg
+
+template <int AT, int BT>
+__global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p) {
+  using Cfg = SgCfg<AT, BT>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  const uint32_t ring0 = ptx::smem_u32(smem);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cfg::kStages * Cfg::kStage);
+  const uint32_t full0 = ptx::smem_u32(bars), empty0 = ptx::smem_u32(bars + Cfg::kStages);
+  const uint32_t tfull0 = ptx::smem_u32(bars + 2 * Cfg::kStages), tempty0 = ptx::smem_u32(bars + 2 * Cfg::kStages + 2);
+  uint32_t* tmem_holder = reinterpret_cast<uint32_t*>(bars + 2 * Cfg::kStages + 4);
+  const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = ptx::cluster_ctarank();                  // 0 = leader: owns the full / tempty barriers, issues the UMMAs
+  const uint32_t unit = blockIdx.x >> 1, n_units = gridDim.x >> 1;
+
+  if (threadIdx.x == 0) {
+    for (uint32_t s = 0; s < Cfg::kStages; ++s) { ptx::mbar_init(full0 + 8 * s, 1); ptx::mbar_init(empty0 + 8 * s, 1); }
+    for (uint32_t s = 0; s < 2; ++s) { ptx::mbar_init(tfull0 + 8 * s, 1); ptx::mbar_init(tempty0 + 8 * s, 16); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 9) ptx::tmem_alloc<512, 2>(ptx::smem_u32(tmem_holder));
+  ptx::tc_fence_before();
+  ptx::cluster_sync();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = *tmem_holder;
+  const uint32_t full_lead0 = ptx::mapa(full0, 0), tempty_lead0 = ptx::mapa(tempty0, 0);
+
+  // Every role walks the same static tile sequence in its own loop, so that the register budget of a role is set once,
+  // before its loop (ptxas allocates per region dominated by the setmaxnreg).
+  if (warp >= 8) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+    if (warp == 8) {
+      // ===== TMA producer (both CTAs; the bytes of both are counted on the leader's full barrier) =====
+      uint32_t stage = 0, ring_phase = 0;
+      uint32_t n_loaded = 0;
+      for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
+        const SgTile t = p.tiles[ti];
+        const SgProb* pr = p.probs + t.prob;
+        if (pr->done != nullptr && *pr->done != 0u) continue;   // stable during the launch: every role agrees
+        const uint32_t nkb = (pr->K + 63u) >> 6;
+        const uint32_t a_mn = pr->a_mn, b_mn = pr->b_mn;
+        const int am0 = (int)(t.m0 + rank * 128u), bn0 = (int)(t.n0 + rank * 128u);
+        for (uint32_t kb = 0; kb < nkb; ++kb) {
+          ptx::mbar_wait(empty0 + 8 * stage, ring_phase ^ 1u);
+          if (MFSDP_SG_PROBE == 1 && n_loaded >= Cfg::kStages) {
+            if (rank == 0 && ptx::elect_one()) ptx::mbar_arrive(full0 + 8 * stage);
+          } else
+          if (ptx::elect_one()) {
+            if (rank == 0) ptx::mbar_arrive_expect_tx(full0 + 8 * stage, 2u * Cfg::kStage);
+            const uint32_t dst = ring0 + stage * Cfg::kStage, fb = full_lead0 + 8 * stage;
+#pragma unroll
+            for (int i = 0; i < AT; ++i) {
+              if (!a_mn) sg::tma_load_3d_cg2(dst + i * kSgBox, &pr->ta, (int)(64 * kb), am0, i, fb);
+              else {
+                sg::tma_load_3d_cg2(dst + i * kSgBox, &pr->ta, am0, (int)(64 * kb), i, fb);
+                sg::tma_load_3d_cg2(dst + i * kSgBox + 8192, &pr->ta, am0 + 64, (int)(64 * kb), i, fb);
+              }
+            }
+#pragma unroll
+            for (int j = 0; j < BT; ++j) {
+              const uint32_t d = dst + (AT + j) * kSgBox;
+              if (!b_mn) sg::tma_load_3d_cg2(d, &pr->tb, (int)(64 * kb), bn0, j, fb);
+              else {
+                sg::tma_load_3d_cg2(d, &pr->tb, bn0, (int)(64 * kb), j, fb);
+                sg::tma_load_3d_cg2(d + 8192, &pr->tb, bn0 + 64, (int)(64 * kb), j, fb);
+              }
+            }
+          }
+          __syncwarp();
+          ++n_loaded;
+          if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
+        }
+      }
+    } else if (warp == 9 && rank == 0) {
+      // ===== UMMA issuer: the leader CTA issues for the pair =====
+      uint32_t stage = 0, ring_phase = 0, cc = 0;               // cc = k chunks so far: TMEM accumulator = cc & 1
+      for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
+        const SgTile t = p.tiles[ti];
+        const SgProb* pr = p.probs + t.prob;
+        if (pr->done != nullptr && *pr->done != 0u) continue;
+        const uint32_t nkb = (pr->K + 63u) >> 6;
+        const uint32_t a_mn = pr->a_mn, b_mn = pr->b_mn;
+        const uint32_t idesc = ptx::idesc_bf16_f32(256, 256, a_mn, b_mn);
+        const uint32_t a_step = a_mn ? (2048u >> 4) : (32u >> 4), b_step = b_mn ? (2048u >> 4) : (32u >> 4);
+        const uint32_t a_lbo = a_mn ? 8192u : 16u, b_lbo = b_mn ? 8192u : 16u;
+        for (uint32_t kb = 0; kb < nkb; ++kb) {
+          const uint32_t buf = cc & 1u, use = cc >> 1;
+          ptx::mbar_wait(tempty0 + 8 * buf, (use & 1u) ^ 1u);     // all 16 epilogue warps have folded this accumulator
+          ptx::mbar_wait(full0 + 8 * stage, ring_phase);
+          ptx::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + buf * 256u;
+          // Descriptors are formed in warp-uniform code and every UMMA of the block is unrolled with constant offsets
+          // (always four k steps: a ragged last block reads TMA's zero fill), so that the elected lane issues from
+          // uniform registers without per-instruction register moves (~200 cycles per UMMA otherwise: issue-bound).
+          const uint32_t base = ring0 + stage * Cfg::kStage;
+          uint64_t ad[AT], bd[BT];
+#pragma unroll
+          for (int i = 0; i < AT; ++i) ad[i] = ptx::smem_desc_sw128(base + i * kSgBox, a_lbo, 1024);
+#pragma unroll
+          for (int j = 0; j < BT; ++j) bd[j] = ptx::smem_desc_sw128(base + (AT + j) * kSgBox, b_lbo, 1024);
+          if (ptx::elect_one()) {
+            // the small term products first, the leading one last (see "Accumulation" above)
+            bool first = true;
+            if (MFSDP_SG_PROBE != 3) {
+#pragma unroll
+            for (int i = 0; i < AT; ++i)
+#pragma unroll
+              for (int j = 0; j < BT; ++j)
+                if (i + j <= 2 && i + j > 0) {
+#pragma unroll
+                  for (uint32_t ks = 0; ks < 4; ++ks) {
+                    ptx::umma_bf16_cg2(d_tmem, ad[i] + (uint64_t)(ks * a_step), bd[j] + (uint64_t)(ks * b_step), idesc, first ? 0u : 1u);
+                    first = false;
+                  }
+                }
+#pragma unroll
+            for (uint32_t ks = 0; ks < 4; ++ks) {
+              ptx::umma_bf16_cg2(d_tmem, ad[0] + (uint64_t)(ks * a_step), bd[0] + (uint64_t)(ks * b_step), idesc, first ? 0u : 1u);
+              first = false;
+            }
+            }
+            ptx::umma_commit_cg2(empty0 + 8 * stage);
+            ptx::umma_commit_cg2(tfull0 + 8 * buf);
+          }
+          __syncwarp();
+          if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
+          ++cc;
+        }
+      }
+    }
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+    // ===== epilogue: warps 0 .. 7; TMEM lane quarter q = warp % 4, column half = warp / 4 =====
+    const uint32_t q = warp & 3u, half = warp >> 2;
+    uint32_t cc = 0;
+    for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
+      const SgTile t = p.tiles[ti];
+      const SgProb* pr = p.probs + t.prob;
+      if (pr->done != nullptr && *pr->done != 0u) continue;
+      const uint32_t nkb = (pr->K + 63u) >> 6;
+      const uint32_t row0 = t.m0 + rank * 128u + q * 32u, r = row0 + lane;
+      const uint32_t n0 = t.n0 + half * 128u;
+      const bool diag = pr->sym != 0u && t.n0 == t.m0;
+      const bool mirror = pr->sym != 0u && t.n0 >= t.m0;
+      float acc[128];
+      for (uint32_t kb = 0; kb < nkb; ++kb) {
+        const uint32_t buf = cc & 1u, use = cc >> 1;
+        ptx::mbar_wait(tfull0 + 8 * buf, use & 1u);
+        ptx::tc_fence_after();
+        if (MFSDP_SG_PROBE != 2 || kb == 0)
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+          uint32_t raw[32];
+          ptx::tmem_ld32(tmem_base + ((q * 32u) << 16) + buf * 256u + half * 128u + 32u * h, raw);
+          ptx::tmem_ld_wait();
+          if (kb == 0) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) acc[32 * h + j] = __uint_as_float(raw[j]);
+          } else {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) acc[32 * h + j] += __uint_as_float(raw[j]);
+          }
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster_relaxed(tempty_lead0 + 8 * buf);
+        ++cc;
+      }
+      // (in a 256-wide diagonal tile a warp's 32 x 128 block may lie wholly below the diagonal: nothing is stored)
+      sg_finish_row(pr, p, acc, row0, r, n0, mirror, diag, lane, ring0 + Cfg::kStages * Cfg::kStage + 256u + warp * (32u * 33u * 4u));
+    }
+  }
+
+  __syncwarp();
+  ptx::tc_fence_before();
+  ptx::cluster_sync();
+  if (warp == 9) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc<512, 2>(tmem_base);
   }
 }
 

@@ -166,8 +166,12 @@ __global__ void k_sh_root_ctl(const RootInfo* roots, uint32_t n, ShCtl* ctl, flo
   // converged; or at the fp32-class noise floor (the error no longer falls); or not a number; or out of budget
   // (the stagnation rule only inside the quadratic regime: far from convergence the error sits just below 1 and
   // consecutive values may round to the same float)
+#if MFSDP_SG_PROBE
+  if (c->iters >= max_iters) c->done = 1u;                  // timing probes: a fixed number of iterations on any data
+#else
   if (!(e >= tol) || (e < 1e-2f && !(e < c->prev_err)) || c->iters >= max_iters) c->done = 1u;
   if (!(e == e)) c->done = 2u;
+#endif
   c->prev_err = e;
   c->err = 0u;
 }
@@ -280,7 +284,7 @@ int build_sh_layout(const mfsdp_desc_t* desc, size_t n_desc, bool keep_d, ShLayo
 }
 
 // ---- host: launch tables ----------------------------------------------------------------------------------------------
-struct SgLaunch { uint32_t prob_off = 0, tile_off = 0, n_tiles = 0; int at = 3, bt = 3; };   // offsets into the plan's arrays
+struct SgLaunch { uint32_t prob_off = 0, tile_off = 0, n_tiles = 0; int at = 3, bt = 3; bool pair = false; };   // offsets into the plan's arrays
 struct RootGroup {
   uint32_t root_off = 0, n_roots = 0;      // into the RootInfo array
   SgLaunch a[2], b, c[2];                  // X T and T T (by iteration parity); T^2 T^2; T^4 M (by parity)
@@ -303,19 +307,40 @@ struct ShPlan {
 std::vector<std::unique_ptr<ShPlan>> g_sh_plans;
 constexpr size_t kMaxShPlans = 64;
 
-void sh_tiles(std::vector<SgTile>& v, uint32_t prob, uint32_t M, uint32_t N, bool sym) {
-  const uint32_t tm = (M + 127u) / 128u, tn = (N + 127u) / 128u, band = 12;
+// Tiles of one problem, edge `ts` (128: single CTA, 256: CTA pair).  Bands of row blocks, column-major inside a band:
+// the tiles in flight form a compact block of the output and share operand panels through L2.
+void sh_tiles(std::vector<SgTile>& v, uint32_t prob, uint32_t M, uint32_t N, bool sym, uint32_t ts) {
+  const uint32_t tm = (M + ts - 1) / ts, tn = (N + ts - 1) / ts, band = ts == 128u ? 12u : 8u;
   for (uint32_t i0 = 0; i0 < tm; i0 += band)
     for (uint32_t j = sym ? i0 : 0u; j < tn; ++j)
       for (uint32_t i = i0; i < std::min(tm, i0 + band); ++i)
-        if (!sym || j >= i) v.push_back(SgTile{prob, i * 128u, j * 128u});
+        if (!sym || j >= i) v.push_back(SgTile{prob, i * ts, j * ts});
 }
+uint32_t sh_tile_count(uint32_t M, uint32_t N, bool sym, uint32_t ts) {
+  const uint32_t tm = (M + ts - 1) / ts, tn = (N + ts - 1) / ts;
+  return sym ? tm * (tm + 1) / 2 : tm * tn;
+}
+constexpr uint32_t kPairMinTiles = 64;   // a launch runs on CTA pairs when it has about a wave of 256-tiles (74 pairs)
 
 template <int AT, int BT>
 int sg_setup() {
-  const cudaError_t e = cudaFuncSetAttribute(k_sgemm3<AT, BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)SgCfg<AT, BT>::kSmem);
+  cudaError_t e = cudaFuncSetAttribute(k_sgemm3<AT, BT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)SgCfg<AT, BT>::kSmem);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(k_sgemm3p<AT, BT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SgCfg<AT, BT>::kSmem);
   return e == cudaSuccess ? MFSDP_OK : cuda_fail(e);
+}
+
+template <int AT, int BT>
+cudaError_t sg_launch_pair(const SgParams& p, uint32_t pairs, cudaStream_t st) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * pairs); cfg.blockDim = dim3(kSgPairThreads);
+  cfg.dynamicSmemBytes = SgCfg<AT, BT>::kSmem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, k_sgemm3p<AT, BT>, p);
 }
 
 int sg_launch(const ShPlan& pl, const SgLaunch& L, float alpha, float beta, float decay, float lr, cudaStream_t st) {
@@ -323,6 +348,13 @@ int sg_launch(const ShPlan& pl, const SgLaunch& L, float alpha, float beta, floa
   SgParams p;
   p.probs = pl.d_probs + L.prob_off; p.tiles = pl.d_tiles + L.tile_off; p.n_tiles = L.n_tiles;
   p.alpha = alpha; p.beta = beta; p.decay = decay; p.lr = lr;
+  if (L.pair) {
+    const uint32_t pairs = std::min<uint32_t>(L.n_tiles, (uint32_t)pl.sms / 2);
+    const cudaError_t e = L.at == 1 && L.bt == 1 ? sg_launch_pair<1, 1>(p, pairs, st)
+                          : L.at == 3 && L.bt == 1 ? sg_launch_pair<3, 1>(p, pairs, st) : sg_launch_pair<3, 3>(p, pairs, st);
+    count_launch();
+    return e == cudaSuccess ? check_last_launch() : cuda_fail(e);
+  }
   const uint32_t grid = std::min<uint32_t>(L.n_tiles, (uint32_t)pl.sms);
   if (L.at == 1 && L.bt == 1) k_sgemm3<1, 1><<<grid, kSgThreads, SgCfg<1, 1>::kSmem, st>>>(p);
   else if (L.at == 3 && L.bt == 1) k_sgemm3<3, 1><<<grid, kSgThreads, SgCfg<3, 1>::kSmem, st>>>(p);
@@ -347,8 +379,20 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     std::memset(&q, 0, sizeof(q));
     return q;
   };
-  auto begin = [&](SgLaunch& L, int at, int bt) { L.prob_off = (uint32_t)probs.size(); L.tile_off = (uint32_t)tiles.size(); L.at = at; L.bt = bt; };
-  auto end = [&](SgLaunch& L) { L.n_tiles = (uint32_t)tiles.size() - L.tile_off; };
+  struct Pending { uint32_t prob, M, N; bool sym; };
+  std::vector<Pending> pending;
+  auto begin = [&](SgLaunch& L, int at, int bt) {
+    L.prob_off = (uint32_t)probs.size(); L.tile_off = (uint32_t)tiles.size(); L.at = at; L.bt = bt;
+    pending.clear();
+  };
+  auto add_tiles = [&](uint32_t prob, uint32_t M, uint32_t N, bool sym) { pending.push_back(Pending{prob, M, N, sym}); };
+  auto end = [&](SgLaunch& L) {     // the tile edge is chosen per launch, once its problems are known
+    uint32_t t256 = 0;
+    for (const Pending& q : pending) t256 += sh_tile_count(q.M, q.N, q.sym, 256);
+    L.pair = t256 >= kPairMinTiles;
+    for (const Pending& q : pending) sh_tiles(tiles, q.prob, q.M, q.N, q.sym, L.pair ? 256u : 128u);
+    L.n_tiles = (uint32_t)tiles.size() - L.tile_off;
+  };
   // matrices by size, largest first (static round-robin: the long tiles lead, the short ones fill the tail)
   std::vector<size_t> order(n_mat);
   for (size_t i = 0; i < n_mat; ++i) order[i] = i;
@@ -389,7 +433,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       q.a_mn = q.b_mn = mn; q.sym = 1;
       q.f32_pitch = side ? m.pc : m.pr;
       q.cin = q.out_f32 = reinterpret_cast<float*>(state + (side ? m.R_off : m.L_off));
-      sh_tiles(tiles, (uint32_t)probs.size() - pl.stat.prob_off, q.M, q.N, true);
+      add_tiles((uint32_t)probs.size() - pl.stat.prob_off, q.M, q.N, true);
       probs.push_back(q);
     }
   }
@@ -457,10 +501,10 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
         const Bufs& b = bufs[k - first];
         SgProb q;
         if ((rc = sym_prob(refs[k], b.b[par], b.b[4], b.b[par ^ 1], nullptr, false, q))) return rc;   // X' = X T
-        sh_tiles(tiles, (uint32_t)probs.size() - g.a[par].prob_off, q.M, q.N, true);
+        add_tiles((uint32_t)probs.size() - g.a[par].prob_off, q.M, q.N, true);
         probs.push_back(q);
         if ((rc = sym_prob(refs[k], b.b[4], b.b[4], b.b[5], nullptr, false, q))) return rc;           // T^2 = T T
-        sh_tiles(tiles, (uint32_t)probs.size() - g.a[par].prob_off, q.M, q.N, true);
+        add_tiles((uint32_t)probs.size() - g.a[par].prob_off, q.M, q.N, true);
         probs.push_back(q);
       }
       end(g.a[par]);
@@ -470,7 +514,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       const Bufs& b = bufs[k - first];
       SgProb q;
       if ((rc = sym_prob(refs[k], b.b[5], b.b[5], b.b[6], nullptr, false, q))) return rc;             // T^4 = T^2 T^2
-      sh_tiles(tiles, (uint32_t)probs.size() - g.b.prob_off, q.M, q.N, true);
+      add_tiles((uint32_t)probs.size() - g.b.prob_off, q.M, q.N, true);
       probs.push_back(q);
     }
     end(g.b);
@@ -480,7 +524,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
         const Bufs& b = bufs[k - first];
         SgProb q;
         if ((rc = sym_prob(refs[k], b.b[6], b.b[2 + par], b.b[2 + (par ^ 1)], b.b[4], true, q))) return rc;   // M' = T^4 M
-        sh_tiles(tiles, (uint32_t)probs.size() - g.c[par].prob_off, q.M, q.N, true);
+        add_tiles((uint32_t)probs.size() - g.c[par].prob_off, q.M, q.N, true);
         probs.push_back(q);
       }
       end(g.c[par]);
@@ -499,7 +543,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     q.M = m.rows; q.N = m.cols; q.K = m.rows; q.b_mn = 1;
     q.sp_pitch = m.pc; q.sp_plane = (uint64_t)m.rows * m.pc;
     q.out_split = reinterpret_cast<__nv_bfloat16*>(ws + m.Tm_off);
-    sh_tiles(tiles, (uint32_t)probs.size() - pl.pre1.prob_off, q.M, q.N, false);
+    add_tiles((uint32_t)probs.size() - pl.pre1.prob_off, q.M, q.N, false);
     probs.push_back(q);
   }
   end(pl.pre1);
@@ -514,7 +558,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     q.f32_pitch = m.pc;
     q.out_f32 = keep_d ? reinterpret_cast<float*>(ws + m.D_off) : nullptr;
     q.W = W + m.elem_off * esz; q.w_bf16 = m.dtype == MFSDP_BF16;
-    sh_tiles(tiles, (uint32_t)probs.size() - pl.pre2.prob_off, q.M, q.N, false);
+    add_tiles((uint32_t)probs.size() - pl.pre2.prob_off, q.M, q.N, false);
     probs.push_back(q);
   }
   end(pl.pre2);
