@@ -378,7 +378,7 @@ typedef struct {
   double  root_tol;        /* 0 -> 1e-6                                                                            */
   int64_t step;            /* 1-based                                                                              */
   int32_t root_every;      /* >= 1                                                                                 */
-  int32_t max_root_iters;  /* 0 -> 40                                                                              */
+  int32_t max_root_iters;  /* 0 -> ceil(log(2.5 / eps_floor) / log(2.44)) + 6 (23 at 2^-20), 40 without a floor    */
   uint32_t flags;          /* MFSDP_SHAMPOO_*                                                                      */
   uint32_t reserved;       /* 0                                                                                    */
 } mfsdp_shampoo_hparams_t;

@@ -440,9 +440,6 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
 // per thread, too few beside 128 accumulators: the control warpgroup (producer, issuer, two idle warps) gives its
 // registers back (setmaxnreg.dec 40) and the two epilogue warpgroups take them (setmaxnreg.inc 232).  Used when a
 // launch has at least ~ one wave of 256-tiles; small problem sets stay on the single-CTA kernel.
-#ifndef MFSDP_SG_PROBE
-#define MFSDP_SG_PROBE 0   // timing probes of the pair kernel (results wrong): 1 no loads after the first ring fill, 2 no fold, 3 no UMMAs
-#endif
 constexpr uint32_t kSgPairThreads = 384;   // warps 0-7 epilogue (two warpgroups), 8 producer, 9 UMMA issuer, 10-11 idle
 namespace sg {
 __device__ __forceinline__ void tma_load_3d_cg2(uint32_t dst, const void* tmap, int c0, int c1, int c2, uint32_t bar_cluster) {
@@ -487,7 +484,6 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
     if (warp == 8) {
       // ===== TMA producer (both CTAs; the bytes of both are counted on the leader's full barrier) =====
       uint32_t stage = 0, ring_phase = 0;
-      uint32_t n_loaded = 0;
       for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
         const SgTile t = p.tiles[ti];
         const SgProb* pr = p.probs + t.prob;
@@ -497,9 +493,6 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
         const int am0 = (int)(t.m0 + rank * 128u), bn0 = (int)(t.n0 + rank * 128u);
         for (uint32_t kb = 0; kb < nkb; ++kb) {
           ptx::mbar_wait(empty0 + 8 * stage, ring_phase ^ 1u);
-          if (MFSDP_SG_PROBE == 1 && n_loaded >= Cfg::kStages) {
-            if (rank == 0 && ptx::elect_one()) ptx::mbar_arrive(full0 + 8 * stage);
-          } else
           if (ptx::elect_one()) {
             if (rank == 0) ptx::mbar_arrive_expect_tx(full0 + 8 * stage, 2u * Cfg::kStage);
             const uint32_t dst = ring0 + stage * Cfg::kStage, fb = full_lead0 + 8 * stage;
@@ -522,7 +515,6 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
             }
           }
           __syncwarp();
-          ++n_loaded;
           if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
         }
       }
@@ -556,7 +548,7 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
           if (ptx::elect_one()) {
             // the small term products first, the leading one last (see "Accumulation" above)
             bool first = true;
-            if (MFSDP_SG_PROBE != 3) {
+            {
 #pragma unroll
             for (int i = 0; i < AT; ++i)
 #pragma unroll
@@ -602,7 +594,6 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
         const uint32_t buf = cc & 1u, use = cc >> 1;
         ptx::mbar_wait(tfull0 + 8 * buf, use & 1u);
         ptx::tc_fence_after();
-        if (MFSDP_SG_PROBE != 2 || kb == 0)
 #pragma unroll
         for (int h = 0; h < 4; ++h) {
           uint32_t raw[32];

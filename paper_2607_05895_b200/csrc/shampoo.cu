@@ -166,12 +166,8 @@ __global__ void k_sh_root_ctl(const RootInfo* roots, uint32_t n, ShCtl* ctl, flo
   // converged; or at the fp32-class noise floor (the error no longer falls); or not a number; or out of budget
   // (the stagnation rule only inside the quadratic regime: far from convergence the error sits just below 1 and
   // consecutive values may round to the same float)
-#if MFSDP_SG_PROBE
-  if (c->iters >= max_iters) c->done = 1u;                  // timing probes: a fixed number of iterations on any data
-#else
   if (!(e >= tol) || (e < 1e-2f && !(e < c->prev_err)) || c->iters >= max_iters) c->done = 1u;
   if (!(e == e)) c->done = 2u;
-#endif
   c->prev_err = e;
   c->err = 0u;
 }
@@ -697,7 +693,14 @@ extern "C" int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void*
   if ((rc = sg_launch(*pl, pl->stat, (float)w, (float)hp->beta2, 0.f, 0.f, st))) return rc;
 
   if ((hp->step - 1) % hp->root_every == 0) {                                   // reading S5
-    const uint32_t max_iters = hp->max_root_iters ? (uint32_t)hp->max_root_iters : 40u;
+    // Launch budget.  The smallest eigenvalue of M_0 is at least 2.5 rho / (||S||_F + rho) >= 2.5 eps_floor / (1 + eps_floor)
+    // and grows by (5/4)^4 = 2.44 per iteration until the quadratic phase (<= 6 more iterations): with the default floor
+    // 2^-20 that is 23 iterations (19 observed at most); without a floor 40.  Converged problems skip their tiles anyway;
+    // the budget only bounds the number of (then empty) launches enqueued.
+    uint32_t max_iters = 40u;
+    if (hp->max_root_iters) max_iters = (uint32_t)hp->max_root_iters;
+    else if (hp->eps_floor > 0.0)
+      max_iters = std::min<uint32_t>(40u, (uint32_t)std::ceil(std::log(2.5 * (1.0 + hp->eps_floor) / hp->eps_floor) / std::log(2.44140625)) + 6u);
     const float tol = hp->root_tol > 0.0 ? (float)hp->root_tol : 1e-6f;
     for (const RootGroup& g : pl->groups) {
       const RootInfo* roots = pl->d_roots + g.root_off;
