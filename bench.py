@@ -414,12 +414,15 @@ def passes_record(res, t, pk):
                 adamw=dict(ms=t["adam"], gbs=gbs(b_adam, t["adam"])), ns=dict(ms=t["ns"]))
 
 
-def measure_other_config(torch, mf, name, pk, local, paper=False, reuse=None):
+def measure_other_config(torch, mf, name, pk, local, paper=False, reuse=None, precision=None):
     """One record of `other_configs`: the same step on another BASELINE.json config (or the paper's own setting on the
     headline's resident set), timed long enough to be meaningful (>= 0.3 s or 200 steps), clocks sampled alongside."""
     import workloads
     if reuse is None:
         wl = workloads.get(name)
+        if precision is not None:      # e.g. config 1 (fp32 storage) through the bf16 tensor-core Newton-Schulz kernels
+            wl.precision = precision
+            wl.name += "+ns_bf16" if precision == mf.NS_BF16 else "+ns_fp32"
         res = Resident(mf, wl, choose_plan_rank(rank_order_by_load(mf, wl), wl.rank, 0, 1), pin=False)
     else:
         res = reuse
@@ -635,6 +638,10 @@ def run_ours(args):
             except Exception as e:
                 others.append(dict(workload=name, error=repr(e)))
             torch.cuda.empty_cache()
+        try:      # config 1 is defined in fp32 mode (an FFMA correctness mode here); the same set on the tensor-core path
+            others.append(measure_other_config(torch, mf, "c1", pk, local, precision=mf.NS_BF16))
+        except Exception as e:
+            others.append(dict(workload="c1+ns_bf16", error=repr(e)))
         for name in ("c2", "c4"):
             try:
                 others.append(measure_shampoo(torch, mf, name, pk, local))

@@ -81,6 +81,7 @@ template <int AT, int BT> struct SgCfg {
   static constexpr uint32_t kKC = 1;
 };
 constexpr uint32_t kSgAccs = 4;      // TMEM chunk accumulators of 128 columns
+constexpr uint32_t kSgPrefetch = 3;  // k blocks between the L2 prefetch of a box and its load
 
 namespace sg {
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const void* tmap, int c0, int c1, int c2, uint32_t bar) {
@@ -88,6 +89,13 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const void* tmap, int 
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
       "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
       : "memory");
+}
+// TMA prefetch of one box into L2 (no shared memory, no completion): issued a few k blocks ahead of the load, so that
+// the load itself finds its lines in L2 -- the operand ring holds only two stages, i.e. a load has one k block of UMMA
+// time to land, less than a DRAM round trip under load.
+__device__ __forceinline__ void tma_prefetch_3d(const void* tmap, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tmap), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
 }
 __device__ __forceinline__ void split3(float v, uint32_t& b1, uint32_t& b2, uint32_t& b3) {   // bf16 bit patterns
   const __nv_bfloat16 h1 = __float2bfloat16_rn(v);
@@ -110,6 +118,31 @@ __device__ __forceinline__ void store_split8(__nv_bfloat16* p0, uint64_t plane, 
 #pragma unroll
   for (int t = 0; t < 3; ++t)
     *reinterpret_cast<uint4*>(p0 + t * plane) = make_uint4(w[t][0], w[t][1], w[t][2], w[t][3]);
+}
+// 16 consecutive values of one row -> the three planes, one 32-byte store each: a full L2 sector per lane and plane
+// (the 16-byte form fills half a sector per store; with one row per lane that doubles the write transactions, and the
+// stores of a short-k tile cost as much as its UMMAs)
+__device__ __forceinline__ void st_global_v8(void* p, const uint32_t (&w)[8]) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(w[0]), "r"(w[1]), "r"(w[2]),
+               "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7])
+               : "memory");
+}
+__device__ __forceinline__ void store_split16(__nv_bfloat16* p0, uint64_t plane, const float* v) {
+  uint32_t w[3][8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    uint32_t a1, a2, a3, c1, c2, c3;
+    split3(v[2 * j], a1, a2, a3);
+    split3(v[2 * j + 1], c1, c2, c3);
+    w[0][j] = a1 | (c1 << 16); w[1][j] = a2 | (c2 << 16); w[2][j] = a3 | (c3 << 16);
+  }
+#pragma unroll
+  for (int t = 0; t < 3; ++t) st_global_v8(p0 + t * plane, w[t]);
+}
+__device__ __forceinline__ void store_f32x8(float* p, const float* v) {
+  const uint32_t w[8] = {__float_as_uint(v[0]), __float_as_uint(v[1]), __float_as_uint(v[2]), __float_as_uint(v[3]),
+                         __float_as_uint(v[4]), __float_as_uint(v[5]), __float_as_uint(v[6]), __float_as_uint(v[7])};
+  st_global_v8(p, w);
 }
 __device__ __forceinline__ void store_split1(__nv_bfloat16* d, uint64_t plane, float v) {
   uint32_t b1, b2, b3;
@@ -146,32 +179,34 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
     const uint32_t cb = n0 + 32u * ch;
     if (cb >= N) continue;                                    // warp-uniform
 #pragma unroll
-    for (int gg = 0; gg < 4; ++gg) {
-      const int g = 4 * ch + gg;
-      const uint32_t c0 = n0 + 8u * g;
-      float* v = acc + 8 * g;                                   // compile-time offsets: stays in registers
+    for (int gg = 0; gg < 2; ++gg) {
+      const int g = 2 * ch + gg;
+      const uint32_t c0 = n0 + 16u * g;
+      float* v = acc + 16 * g;                                  // compile-time offsets: stays in registers
 #pragma unroll
-      for (int j = 0; j < 8; ++j) v[j] *= p.alpha;
+      for (int j = 0; j < 16; ++j) v[j] *= p.alpha;
       if (!row_ok) continue;
       if (cin != nullptr) {
         const float4* src = reinterpret_cast<const float4*>(cin + (size_t)r * fp + c0);
-        const float4 a = src[0], b = src[1];
-        v[0] = fmaf(p.beta, a.x, v[0]); v[1] = fmaf(p.beta, a.y, v[1]); v[2] = fmaf(p.beta, a.z, v[2]); v[3] = fmaf(p.beta, a.w, v[3]);
-        v[4] = fmaf(p.beta, b.x, v[4]); v[5] = fmaf(p.beta, b.y, v[5]); v[6] = fmaf(p.beta, b.z, v[6]); v[7] = fmaf(p.beta, b.w, v[7]);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float4 a = src[j];
+          v[4 * j] = fmaf(p.beta, a.x, v[4 * j]); v[4 * j + 1] = fmaf(p.beta, a.y, v[4 * j + 1]);
+          v[4 * j + 2] = fmaf(p.beta, a.z, v[4 * j + 2]); v[4 * j + 3] = fmaf(p.beta, a.w, v[4 * j + 3]);
+        }
       }
       if (errp != nullptr) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
+        for (int j = 0; j < 16; ++j)
           if (c0 + j < N) emax = max(emax, __float_as_uint(fabsf(v[j] - (c0 + j == r ? 1.f : 0.f))));
       }
       if (of32 != nullptr) {
         if (!diag) {
-          float4* dst = reinterpret_cast<float4*>(of32 + (size_t)r * fp + c0);
-          dst[0] = make_float4(v[0], v[1], v[2], v[3]);
-          dst[1] = make_float4(v[4], v[5], v[6], v[7]);
+          sg::store_f32x8(of32 + (size_t)r * fp + c0, v);
+          sg::store_f32x8(of32 + (size_t)r * fp + c0 + 8, v + 8);
         } else {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
+          for (int j = 0; j < 16; ++j) {
             if (c0 + j < N && c0 + j >= r) of32[(size_t)r * fp + c0 + j] = v[j];
             if (c0 + j < N && c0 + j > r) of32[(size_t)(c0 + j) * fp + r] = v[j];
           }
@@ -179,10 +214,10 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
       }
       if (osp != nullptr) {
         __nv_bfloat16* dst = osp + (size_t)r * spp + c0;
-        if (!diag) sg::store_split8(dst, plane, v);
+        if (!diag) sg::store_split16(dst, plane, v);
         else {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
+          for (int j = 0; j < 16; ++j) {
             if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, plane, v[j]);
             if (c0 + j < N && c0 + j > r) sg::store_split1(osp + (size_t)(c0 + j) * spp + r, plane, v[j]);
           }
@@ -191,13 +226,13 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
       if (tsp != nullptr) {                                       // T = (5 I - v) / 4
         __nv_bfloat16* dst = tsp + (size_t)r * spp + c0;
         if (!diag) {
-          float tv[8];
+          float tv[16];
 #pragma unroll
-          for (int j = 0; j < 8; ++j) tv[j] = 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]);
-          sg::store_split8(dst, plane, tv);
+          for (int j = 0; j < 16; ++j) tv[j] = 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]);
+          sg::store_split16(dst, plane, tv);
         } else {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
+          for (int j = 0; j < 16; ++j) {
             if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, plane, 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]));
             if (c0 + j < N && c0 + j > r) sg::store_split1(tsp + (size_t)(c0 + j) * spp + r, plane, -0.25f * v[j]);
           }
@@ -207,28 +242,31 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
         // W <- decay W - lr v (rank-flat, pitch = N: no padding, element-wise predicates at the right edge)
         if (pr->w_bf16) {
           __nv_bfloat16* w = reinterpret_cast<__nv_bfloat16*>(pr->W) + (size_t)r * N + c0;
-          if ((N & 7u) == 0u) {                                   // then c0 + 8 <= N
-            if (c0 < N) {
-              const uint4 x = *reinterpret_cast<const uint4*>(w);
-              uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+          if ((N & 7u) == 0u) {                                   // 16-byte vectors never straddle the row end
 #pragma unroll
-              for (int i = 0; i < 4; ++i) {
-                const float w0 = __uint_as_float(xs[i] << 16), w1 = __uint_as_float(xs[i] & 0xffff0000u);
-                const __nv_bfloat162 h = __floats2bfloat162_rn(fmaf(-p.lr, v[2 * i], p.decay * w0),
-                                                               fmaf(-p.lr, v[2 * i + 1], p.decay * w1));
-                xs[i] = *reinterpret_cast<const uint32_t*>(&h);
+            for (int h = 0; h < 2; ++h) {
+              if (c0 + 8u * h < N) {
+                const uint4 x = reinterpret_cast<const uint4*>(w)[h];
+                uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                  const float w0 = __uint_as_float(xs[i] << 16), w1 = __uint_as_float(xs[i] & 0xffff0000u);
+                  const __nv_bfloat162 hh = __floats2bfloat162_rn(fmaf(-p.lr, v[8 * h + 2 * i], p.decay * w0),
+                                                                  fmaf(-p.lr, v[8 * h + 2 * i + 1], p.decay * w1));
+                  xs[i] = *reinterpret_cast<const uint32_t*>(&hh);
+                }
+                reinterpret_cast<uint4*>(w)[h] = make_uint4(xs[0], xs[1], xs[2], xs[3]);
               }
-              *reinterpret_cast<uint4*>(w) = make_uint4(xs[0], xs[1], xs[2], xs[3]);
             }
           } else {
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
+            for (int j = 0; j < 16; ++j)
               if (c0 + j < N) w[j] = __float2bfloat16_rn(fmaf(-p.lr, v[j], p.decay * __bfloat162float(w[j])));
           }
         } else {
           float* w = reinterpret_cast<float*>(pr->W) + (size_t)r * N + c0;
 #pragma unroll
-          for (int j = 0; j < 8; ++j)
+          for (int j = 0; j < 16; ++j)
             if (c0 + j < N) w[j] = fmaf(-p.lr, v[j], p.decay * w[j]);
         }
       }
@@ -247,19 +285,18 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
       const uint32_t mr = cb + lane;
       if (mr < N) {
         if (of32 != nullptr) {
-          float4* dst = reinterpret_cast<float4*>(of32 + (size_t)mr * fp + row0);
 #pragma unroll
-          for (int j = 0; j < 8; ++j) dst[j] = make_float4(w[4 * j], w[4 * j + 1], w[4 * j + 2], w[4 * j + 3]);
+          for (int g = 0; g < 4; ++g) sg::store_f32x8(of32 + (size_t)mr * fp + row0 + 8 * g, w + 8 * g);
         }
         if (osp != nullptr) {
-#pragma unroll
-          for (int g = 0; g < 4; ++g) sg::store_split8(osp + (size_t)mr * spp + row0 + 8 * g, plane, w + 8 * g);
+          sg::store_split16(osp + (size_t)mr * spp + row0, plane, w);
+          sg::store_split16(osp + (size_t)mr * spp + row0 + 16, plane, w + 16);
         }
         if (tsp != nullptr) {
 #pragma unroll
           for (int i = 0; i < 32; ++i) w[i] *= -0.25f;
-#pragma unroll
-          for (int g = 0; g < 4; ++g) sg::store_split8(tsp + (size_t)mr * spp + row0 + 8 * g, plane, w + 8 * g);
+          sg::store_split16(tsp + (size_t)mr * spp + row0, plane, w);
+          sg::store_split16(tsp + (size_t)mr * spp + row0 + 16, plane, w + 16);
         }
       }
     }
@@ -326,6 +363,19 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
             else {
               sg::tma_load_3d(d, &pr->tb, (int)t.n0, (int)(64 * kb), j, fb);
               sg::tma_load_3d(d + 8192, &pr->tb, (int)t.n0 + 64, (int)(64 * kb), j, fb);
+            }
+          }
+          if (kb + kSgPrefetch < nkb) {
+            const int kp = (int)(64 * (kb + kSgPrefetch));
+#pragma unroll
+            for (int i = 0; i < AT; ++i) {
+              if (!a_mn) sg::tma_prefetch_3d(&pr->ta, kp, (int)t.m0, i);
+              else { sg::tma_prefetch_3d(&pr->ta, (int)t.m0, kp, i); sg::tma_prefetch_3d(&pr->ta, (int)t.m0 + 64, kp, i); }
+            }
+#pragma unroll
+            for (int j = 0; j < BT; ++j) {
+              if (!b_mn) sg::tma_prefetch_3d(&pr->tb, kp, (int)t.n0, j);
+              else { sg::tma_prefetch_3d(&pr->tb, (int)t.n0, kp, j); sg::tma_prefetch_3d(&pr->tb, (int)t.n0 + 64, kp, j); }
             }
           }
         }
@@ -511,6 +561,19 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
               else {
                 sg::tma_load_3d_cg2(d, &pr->tb, bn0, (int)(64 * kb), j, fb);
                 sg::tma_load_3d_cg2(d + 8192, &pr->tb, bn0 + 64, (int)(64 * kb), j, fb);
+              }
+            }
+            if (kb + kSgPrefetch < nkb) {
+              const int kp = (int)(64 * (kb + kSgPrefetch));
+#pragma unroll
+              for (int i = 0; i < AT; ++i) {
+                if (!a_mn) sg::tma_prefetch_3d(&pr->ta, kp, am0, i);
+                else { sg::tma_prefetch_3d(&pr->ta, am0, kp, i); sg::tma_prefetch_3d(&pr->ta, am0 + 64, kp, i); }
+              }
+#pragma unroll
+              for (int j = 0; j < BT; ++j) {
+                if (!b_mn) sg::tma_prefetch_3d(&pr->tb, kp, bn0, j);
+                else { sg::tma_prefetch_3d(&pr->tb, bn0, kp, j); sg::tma_prefetch_3d(&pr->tb, bn0 + 64, kp, j); }
               }
             }
           }
