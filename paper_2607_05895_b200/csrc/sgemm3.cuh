@@ -44,6 +44,7 @@ namespace mfsdp {
 
 struct alignas(64) SgProb {
   CUtensorMap ta, tb;               // operand storage: dims (cols, rows, planes)
+  CUtensorMap to, tt;               // store maps of out_split / t_split: box 32 cols x 32 rows x 1 plane, no swizzle
   uint32_t M, N, K;                 // output rows, columns; reduction length
   uint32_t a_mn, b_mn;              // 1: operand stored [k][m] (MN-major) instead of [m][k]
   uint32_t sym;                     // symmetric output: tiles with n0 >= m0 only, mirrored by the epilogue
@@ -67,6 +68,8 @@ struct SgParams {
   uint32_t n_tiles;
   float alpha, beta;                // v = alpha acc + beta Cin
   float decay, lr;                  // W <- decay W - lr v
+  unsigned long long* trace;        // mfsdp_debug_trace target or null: [0] = record counter, then 6-word records
+  uint32_t trace_cap;               // (k_sgemm3p: per tile and role {role << 32 | tile, begin, end, wait a, wait b, sm})
 };
 
 constexpr uint32_t kSgThreads = 192;
@@ -95,6 +98,11 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const void* tmap, int 
 // time to land, less than a DRAM round trip under load.
 __device__ __forceinline__ void tma_prefetch_3d(const void* tmap, int c0, int c1, int c2) {
   asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tmap), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const void* tmap, int c0, int c1, int c2, uint32_t src_smem) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tmap), "r"(c0), "r"(c1),
+               "r"(c2), "r"(src_smem)
                : "memory");
 }
 __device__ __forceinline__ void split3(float v, uint32_t& b1, uint32_t& b2, uint32_t& b3) {   // bf16 bit patterns
@@ -154,6 +162,67 @@ __device__ __forceinline__ void store_split1(__nv_bfloat16* d, uint64_t plane, f
 }  // namespace sg
 
 
+// One warp's 32 x 32 block of a three-plane output (lane = row, v = its 32 columns) -> global memory through TMA
+// stores: per plane the block is staged in shared memory (32 rows x 64 bytes, dense) and stored asynchronously, so the
+// warp is not held up by the write burst (all CTAs finish their tiles together: with plain stores the epilogue of a
+// tile took ~55 K cycles, during which the UMMAs of the next tile wait for the fold).  TMA clips at the matrix edges.
+//   mode 0: the block as it is, at (row0, cb)
+//   mode 1: as it is at (row0, cb) AND transposed at (cb, row0)          (strictly above the diagonal of a symmetric output)
+//   mode 2: a block ON the diagonal: upper triangle from the rows themselves, lower triangle = its mirror image
+//           (bit-symmetric although the two triangles were summed in different orders)
+// `stg`: two 2 KB staging tiles of this warp; `n_st`: TMA stores issued so far by this warp (staging tile parity).
+__device__ __forceinline__ void sg_store_block(const CUtensorMap* tm, const float* v, uint32_t row0, uint32_t cb, int mode,
+                                               uint32_t lane, uint32_t stg, uint32_t& n_st, bool as_t) {
+  // as_t: store T = (5 I - v) / 4 instead of v (formed on the fly; r = row0 + lane is this lane's row)
+  const uint32_t dcol = row0 + lane - cb;                      // column offset of the diagonal element in this block, if any
+#pragma unroll 1
+  for (int t = 0; t < 3; ++t) {                                // not unrolled: one plane's 16 packed words live at a time
+    uint32_t w[16];                                            // plane t of the lane's 32 values, packed pairs
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      float x0 = v[2 * j], x1 = v[2 * j + 1];
+      if (as_t) {
+        x0 = 0.25f * (((uint32_t)(2 * j) == dcol ? 5.f : 0.f) - x0);
+        x1 = 0.25f * (((uint32_t)(2 * j + 1) == dcol ? 5.f : 0.f) - x1);
+      }
+      uint32_t a[3], c[3];
+      sg::split3(x0, a[0], a[1], a[2]);
+      sg::split3(x1, c[0], c[1], c[2]);
+      w[j] = (t == 0 ? a[0] : t == 1 ? a[1] : a[2]) | ((t == 0 ? c[0] : t == 1 ? c[1] : c[2]) << 16);
+    }
+    {   // the block itself
+      const uint32_t buf = stg + (n_st & 1u) * 2048u;
+      if (lane == 0) ptx::bulk_wait_read<1>();                 // the store issued two stores ago has read this tile
+      __syncwarp();
+#pragma unroll
+      for (int qd = 0; qd < 4; ++qd)
+        ptx::st_shared_v4(buf + lane * 64u + 16u * qd, w[4 * qd], w[4 * qd + 1], w[4 * qd + 2], w[4 * qd + 3]);
+      if (mode == 2) {
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 32; ++j)                           // element (lane, j), j > lane, also is element (j, lane)
+          if (j > (int)lane) ptx::st_shared_b16(buf + (uint32_t)j * 64u + lane * 2u, (uint16_t)(j & 1 ? w[j >> 1] >> 16 : w[j >> 1] & 0xffffu));
+      }
+      ptx::fence_async_smem();
+      __syncwarp();
+      if (lane == 0) { sg::tma_store_3d(tm, (int)cb, (int)row0, t, buf); ptx::bulk_commit(); }
+      ++n_st;
+    }
+    if (mode == 1) {   // the transposed block
+      const uint32_t buf = stg + (n_st & 1u) * 2048u;
+      if (lane == 0) ptx::bulk_wait_read<1>();
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < 32; ++j)
+        ptx::st_shared_b16(buf + (uint32_t)j * 64u + lane * 2u, (uint16_t)(j & 1 ? w[j >> 1] >> 16 : w[j >> 1] & 0xffffu));
+      ptx::fence_async_smem();
+      __syncwarp();
+      if (lane == 0) { sg::tma_store_3d(tm, (int)row0, (int)cb, t, buf); ptx::bulk_commit(); }
+      ++n_st;
+    }
+  }
+}
+
 // The stores of one thread's row of a tile: `acc` = 128 consecutive columns starting at n0 of output row r (this warp's
 // rows start at row0, a multiple of 32), already summed over k.  Worked through in chunks of 32 columns, groups of 8
 // inside, to keep few values live beside the 128 accumulators.  The mirror image of a symmetric output goes through
@@ -162,7 +231,7 @@ __device__ __forceinline__ void store_split1(__nv_bfloat16* d, uint64_t plane, f
 // scattered 2-byte stores of the three planes cost more than the UMMAs of a short-k tile).
 __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& p, float (&acc)[128], uint32_t row0,
                                               uint32_t r, uint32_t n0, bool mirror, bool diag, uint32_t lane,
-                                              uint32_t tbuf) {
+                                              uint32_t tbuf, uint32_t& n_st) {
   const uint32_t M = pr->M, N = pr->N;
   const bool row_ok = r < M;
   uint32_t emax = 0u;                                         // bits of max |v - delta| (NaN sorts above everything)
@@ -172,8 +241,7 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
   __nv_bfloat16* osp = pr->out_split;
   __nv_bfloat16* tsp = pr->t_split;
   const uint32_t* errp = pr->err;
-  const uint32_t fp = pr->f32_pitch, spp = pr->sp_pitch;
-  const uint64_t plane = pr->sp_plane;
+  const uint32_t fp = pr->f32_pitch;
 #pragma unroll
   for (int ch = 0; ch < 4; ++ch) {
     const uint32_t cb = n0 + 32u * ch;
@@ -212,32 +280,6 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
           }
         }
       }
-      if (osp != nullptr) {
-        __nv_bfloat16* dst = osp + (size_t)r * spp + c0;
-        if (!diag) sg::store_split16(dst, plane, v);
-        else {
-#pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, plane, v[j]);
-            if (c0 + j < N && c0 + j > r) sg::store_split1(osp + (size_t)(c0 + j) * spp + r, plane, v[j]);
-          }
-        }
-      }
-      if (tsp != nullptr) {                                       // T = (5 I - v) / 4
-        __nv_bfloat16* dst = tsp + (size_t)r * spp + c0;
-        if (!diag) {
-          float tv[16];
-#pragma unroll
-          for (int j = 0; j < 16; ++j) tv[j] = 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]);
-          sg::store_split16(dst, plane, tv);
-        } else {
-#pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            if (c0 + j < N && c0 + j >= r) sg::store_split1(dst + j, plane, 0.25f * ((c0 + j == r ? 5.f : 0.f) - v[j]));
-            if (c0 + j < N && c0 + j > r) sg::store_split1(tsp + (size_t)(c0 + j) * spp + r, plane, -0.25f * v[j]);
-          }
-        }
-      }
       if (pr->W != nullptr) {
         // W <- decay W - lr v (rank-flat, pitch = N: no padding, element-wise predicates at the right edge)
         if (pr->w_bf16) {
@@ -271,10 +313,11 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
         }
       }
     }
-    if (mirror && !diag) {
-      // transpose this warp's 32 x 32 block: lane l ends up with column cb + l of rows row0 .. row0 + 31, i.e. with 32
-      // consecutive elements of mirrored row cb + l.  (rows >= M hold alpha * 0 = 0 and land in the pitch padding)
+    if (of32 != nullptr && mirror && !diag) {
+      // fp32 mirror image: transpose this warp's 32 x 32 block through the scratch tile, so that a lane owns 32
+      // consecutive elements of one mirrored row.  (rows >= M hold alpha * 0 = 0 and land in the pitch padding)
       float* v = acc + 32 * ch;
+      if (lane == 0) ptx::bulk_wait_read<0>();                  // no TMA store of this warp still reads the scratch
       __syncwarp();
 #pragma unroll
       for (int j = 0; j < 32; ++j) ptx::st_shared_u32(tbuf + (lane * 33u + j) * 4u, __float_as_uint(row_ok ? v[j] : 0.f));
@@ -282,24 +325,24 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
       float w[32];
 #pragma unroll
       for (int i = 0; i < 32; ++i) w[i] = __uint_as_float(ptx::ld_shared_u32(tbuf + (i * 33u + lane) * 4u));
+      __syncwarp();
       const uint32_t mr = cb + lane;
       if (mr < N) {
-        if (of32 != nullptr) {
 #pragma unroll
-          for (int g = 0; g < 4; ++g) sg::store_f32x8(of32 + (size_t)mr * fp + row0 + 8 * g, w + 8 * g);
-        }
-        if (osp != nullptr) {
-          sg::store_split16(osp + (size_t)mr * spp + row0, plane, w);
-          sg::store_split16(osp + (size_t)mr * spp + row0 + 16, plane, w + 16);
-        }
-        if (tsp != nullptr) {
-#pragma unroll
-          for (int i = 0; i < 32; ++i) w[i] *= -0.25f;
-          sg::store_split16(tsp + (size_t)mr * spp + row0, plane, w);
-          sg::store_split16(tsp + (size_t)mr * spp + row0 + 16, plane, w + 16);
-        }
+        for (int g = 0; g < 4; ++g) sg::store_f32x8(of32 + (size_t)mr * fp + row0 + 8 * g, w + 8 * g);
       }
     }
+    // three-plane outputs: asynchronous TMA stores of 32 x 32 blocks (see sg_store_block)
+    const int mode = !mirror ? 0 : cb > row0 ? 1 : cb == row0 ? 2 : -1;   // below the diagonal: the mirror image covers it
+    if (mode == 0 && osp != nullptr) {
+      // a general (non-symmetric) output has no mirror image and no write burst worth hiding: plain 32-byte stores
+      if (row_ok) {
+        sg::store_split16(osp + (size_t)r * pr->sp_pitch + cb, pr->sp_plane, acc + 32 * ch);
+        sg::store_split16(osp + (size_t)r * pr->sp_pitch + cb + 16, pr->sp_plane, acc + 32 * ch + 16);
+      }
+    } else
+    if (mode >= 0 && osp != nullptr) sg_store_block(&pr->to, acc + 32 * ch, row0, cb, mode, lane, tbuf, n_st, false);
+    if (mode >= 0 && tsp != nullptr) sg_store_block(&pr->tt, acc + 32 * ch, row0, cb, mode, lane, tbuf, n_st, true);   // T = (5 I - v) / 4
   }
   if (errp != nullptr) {
 #pragma unroll
@@ -333,6 +376,7 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
 
   uint32_t stage = 0, ring_phase = 0;   // producer, issuer
   uint32_t cc = 0;                      // k chunks this CTA has worked on: TMEM accumulator = cc % 4 (issuer, epilogue)
+  uint32_t n_st = 0;                    // TMA stores issued by this (epilogue) warp
 
   for (uint32_t ti = blockIdx.x; ti < p.n_tiles; ti += gridDim.x) {
     const SgTile t = p.tiles[ti];
@@ -466,10 +510,11 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
         ++cc;
       }
       sg_finish_row(pr, p, acc, t.m0 + q * 32u, r, t.n0, mirror, diag, lane,
-                    ring0 + Cfg::kStages * Cfg::kStage + 256u + (warp - 2u) * (32u * 33u * 4u));
+                    ring0 + Cfg::kStages * Cfg::kStage + 256u + (warp - 2u) * (32u * 33u * 4u), n_st);
     }
   }
 
+  if (warp >= 2 && lane == 0) ptx::bulk_wait<0>();          // this warp's TMA stores have been performed
   __syncwarp();
   ptx::tc_fence_before();
   __syncthreads();
@@ -500,6 +545,16 @@ __device__ __forceinline__ void tma_load_3d_cg2(uint32_t dst, const void* tmap, 
       : "memory");
 }
 }  // namespace sg
+
+__device__ __forceinline__ void sg_trace(const SgParams& p, uint32_t role, uint32_t tile, long long t0, long long t1,
+                                         long long wa, long long wb) {
+  const unsigned long long i = atomicAdd(p.trace, 1ull);
+  if (i < p.trace_cap) {
+    unsigned long long* r = p.trace + 1 + 6 * i;
+    r[0] = ((unsigned long long)role << 32) | tile; r[1] = (unsigned long long)t0; r[2] = (unsigned long long)t1;
+    r[3] = (unsigned long long)wa; r[4] = (unsigned long long)wb; r[5] = ptx::smid();
+  }
+}
 
 template <int AT, int BT>
 __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p) {
@@ -541,8 +596,11 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
         const uint32_t nkb = (pr->K + 63u) >> 6;
         const uint32_t a_mn = pr->a_mn, b_mn = pr->b_mn;
         const int am0 = (int)(t.m0 + rank * 128u), bn0 = (int)(t.n0 + rank * 128u);
+        const long long tr0 = p.trace ? clock64() : 0;
+        long long wa = 0;
         for (uint32_t kb = 0; kb < nkb; ++kb) {
-          ptx::mbar_wait(empty0 + 8 * stage, ring_phase ^ 1u);
+          if (p.trace) { const long long c0 = clock64(); ptx::mbar_wait(empty0 + 8 * stage, ring_phase ^ 1u); wa += clock64() - c0; }
+          else ptx::mbar_wait(empty0 + 8 * stage, ring_phase ^ 1u);
           if (ptx::elect_one()) {
             if (rank == 0) ptx::mbar_arrive_expect_tx(full0 + 8 * stage, 2u * Cfg::kStage);
             const uint32_t dst = ring0 + stage * Cfg::kStage, fb = full_lead0 + 8 * stage;
@@ -580,6 +638,7 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
           __syncwarp();
           if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
         }
+        if (p.trace && rank == 0 && lane == 0) sg_trace(p, 0, ti, tr0, clock64(), wa, 0);
       }
     } else if (warp == 9 && rank == 0) {
       // ===== UMMA issuer: the leader CTA issues for the pair =====
@@ -593,10 +652,20 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
         const uint32_t idesc = ptx::idesc_bf16_f32(256, 256, a_mn, b_mn);
         const uint32_t a_step = a_mn ? (2048u >> 4) : (32u >> 4), b_step = b_mn ? (2048u >> 4) : (32u >> 4);
         const uint32_t a_lbo = a_mn ? 8192u : 16u, b_lbo = b_mn ? 8192u : 16u;
+        const long long tr0 = p.trace ? clock64() : 0;
+        long long wa = 0, wb = 0;
         for (uint32_t kb = 0; kb < nkb; ++kb) {
           const uint32_t buf = cc & 1u, use = cc >> 1;
+          if (p.trace) {
+            const long long c0 = clock64();
+            ptx::mbar_wait(tempty0 + 8 * buf, (use & 1u) ^ 1u);
+            const long long c1 = clock64();
+            ptx::mbar_wait(full0 + 8 * stage, ring_phase);
+            wa += c1 - c0; wb += clock64() - c1;
+          } else {
           ptx::mbar_wait(tempty0 + 8 * buf, (use & 1u) ^ 1u);     // all 16 epilogue warps have folded this accumulator
           ptx::mbar_wait(full0 + 8 * stage, ring_phase);
+          }
           ptx::tc_fence_after();
           const uint32_t d_tmem = tmem_base + buf * 256u;
           // Descriptors are formed in warp-uniform code and every UMMA of the block is unrolled with constant offsets
@@ -636,13 +705,14 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
           if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1u; }
           ++cc;
         }
+        if (p.trace && lane == 0) sg_trace(p, 1, ti, tr0, clock64(), wa, wb);
       }
     }
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
     // ===== epilogue: warps 0 .. 7; TMEM lane quarter q = warp % 4, column half = warp / 4 =====
     const uint32_t q = warp & 3u, half = warp >> 2;
-    uint32_t cc = 0;
+    uint32_t cc = 0, n_st = 0;
     for (uint32_t ti = unit; ti < p.n_tiles; ti += n_units) {
       const SgTile t = p.tiles[ti];
       const SgProb* pr = p.probs + t.prob;
@@ -653,9 +723,12 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
       const bool diag = pr->sym != 0u && t.n0 == t.m0;
       const bool mirror = pr->sym != 0u && t.n0 >= t.m0;
       float acc[128];
+      const long long tr0 = p.trace ? clock64() : 0;
+      long long wa = 0;
       for (uint32_t kb = 0; kb < nkb; ++kb) {
         const uint32_t buf = cc & 1u, use = cc >> 1;
-        ptx::mbar_wait(tfull0 + 8 * buf, use & 1u);
+        if (p.trace) { const long long c0 = clock64(); ptx::mbar_wait(tfull0 + 8 * buf, use & 1u); wa += clock64() - c0; }
+        else ptx::mbar_wait(tfull0 + 8 * buf, use & 1u);
         ptx::tc_fence_after();
 #pragma unroll
         for (int h = 0; h < 4; ++h) {
@@ -676,8 +749,11 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
         ++cc;
       }
       // (in a 256-wide diagonal tile a warp's 32 x 128 block may lie wholly below the diagonal: nothing is stored)
-      sg_finish_row(pr, p, acc, row0, r, n0, mirror, diag, lane, ring0 + Cfg::kStages * Cfg::kStage + 256u + warp * (32u * 33u * 4u));
+      const long long tr1 = p.trace ? clock64() : 0;
+      sg_finish_row(pr, p, acc, row0, r, n0, mirror, diag, lane, ring0 + Cfg::kStages * Cfg::kStage + 256u + warp * (32u * 33u * 4u), n_st);
+      if (p.trace && rank == 0 && warp == 0 && lane == 0) sg_trace(p, 2, ti, tr0, clock64(), wa, tr1 - tr0);
     }
+    if (lane == 0) ptx::bulk_wait<0>();                        // this warp's TMA stores have been performed
   }
 
   __syncwarp();

@@ -222,6 +222,20 @@ int make_tmap3(CUtensorMap* out, const void* base, uint32_t rows, uint32_t cols,
   return r == CUDA_SUCCESS ? MFSDP_OK : cuda_fail(cudaErrorInvalidValue);
 }
 
+// store map of a three-plane output: box 32 cols x 32 rows x 1 plane, dense (no swizzle); stores are clipped at the edges
+int make_store_tmap3(CUtensorMap* out, const void* base, uint32_t rows, uint32_t cols, uint32_t pitch, uint64_t plane_elems) {
+  EncodeTiledFn enc = sh_encode();
+  if (!enc) return cuda_fail(cudaErrorSymbolNotFound);
+  const cuuint64_t dims[3] = {cols, rows, 3};
+  const cuuint64_t strides[2] = {(cuuint64_t)pitch * 2, (cuuint64_t)plane_elems * 2};
+  const cuuint32_t box[3] = {32, 32, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? MFSDP_OK : cuda_fail(cudaErrorInvalidValue);
+}
+
 // ---- host: layout ---------------------------------------------------------------------------------------------------
 inline uint32_t pitch64(uint32_t n) { return (n + 63u) / 64u * 64u; }
 
@@ -344,6 +358,7 @@ int sg_launch(const ShPlan& pl, const SgLaunch& L, float alpha, float beta, floa
   SgParams p;
   p.probs = pl.d_probs + L.prob_off; p.tiles = pl.d_tiles + L.tile_off; p.n_tiles = L.n_tiles;
   p.alpha = alpha; p.beta = beta; p.decay = decay; p.lr = lr;
+  get_trace(&p.trace, &p.trace_cap);
   if (L.pair) {
     const uint32_t pairs = std::min<uint32_t>(L.n_tiles, (uint32_t)pl.sms / 2);
     const cudaError_t e = L.at == 1 && L.bt == 1 ? sg_launch_pair<1, 1>(p, pairs, st)
@@ -486,6 +501,8 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       q.M = q.N = q.K = r.d; q.sym = 1;
       q.sp_pitch = r.pitch; q.sp_plane = plane;
       q.out_split = out; q.t_split = tsplit;
+      if ((e = make_store_tmap3(&q.to, out, r.d, r.d, r.pitch, plane))) return e;
+      if (tsplit && (e = make_store_tmap3(&q.tt, tsplit, r.d, r.d, r.pitch, plane))) return e;
       ShCtl* c = d_ctl + (2 * r.mat + r.side);
       q.done = &c->done;
       q.err = err ? &c->err : nullptr;
@@ -539,6 +556,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     q.M = m.rows; q.N = m.cols; q.K = m.rows; q.b_mn = 1;
     q.sp_pitch = m.pc; q.sp_plane = (uint64_t)m.rows * m.pc;
     q.out_split = reinterpret_cast<__nv_bfloat16*>(ws + m.Tm_off);
+    if ((rc = make_store_tmap3(&q.to, q.out_split, m.rows, m.cols, m.pc, (uint64_t)m.rows * m.pc))) return rc;
     add_tiles((uint32_t)probs.size() - pl.pre1.prob_off, q.M, q.N, false);
     probs.push_back(q);
   }
