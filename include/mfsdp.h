@@ -443,6 +443,11 @@ int mfsdp_get_tune(int knob);
  *   (phase index 3 * iteration + {0 GRAM, 1 POLY, 2 APPLY} << 32 | tile index within the launch), (walking unit << 32 | SM id),
  *   %globaltimer ns when the tile's accumulator was complete, %globaltimer ns when its first epilogue warp was done,
  *   the SM's clock64 at the first instant, (k blocks of the tile << 32 | UMMA N).
+ * The CTA-pair GEMM of the Shampoo step (k_sgemm3p) appends, per tile and per role of the pair's leader CTA, a record
+ *   (role {0 TMA producer, 1 UMMA issuer, 2 first epilogue warp} << 32 | tile index), clock64 at the start and at the
+ *   end of the role's work on the tile, cycles spent waiting (producer: for a free ring stage; issuer: for a folded
+ *   TMEM accumulator; epilogue: for a complete accumulator), a second figure (issuer: cycles waiting for operands;
+ *   epilogue: cycles until its stores began), SM id.
  * Records beyond the capacity are dropped (the counter keeps counting).  Returns MFSDP_EINVAL on a misaligned or
  * too-small buffer. */
 int mfsdp_debug_trace(void* dev_buf, size_t bytes);
