@@ -482,8 +482,13 @@ def measure_shampoo(torch, mf, name, pk, local, ws_cap_bytes=64e9):
     sampler = ClockSampler(local)
     sampler.start()
     recs = []
+    G = None
     for t in (1, 2):
-        G = workloads.fill_flat(wl, descs, workloads.KIND_G, step=t).cuda()
+        hG = workloads.fill_flat(wl, descs, workloads.KIND_G, step=t)
+        if G is None:
+            G = hG.cuda()
+        else:
+            G.copy_(hG)      # same gradient buffer every step, as in training: the launch tables are keyed by its address
         torch.cuda.synchronize()
         n0 = mf.mfsdp_launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -25,6 +25,14 @@ from helpers import bf16_rne, rel_fro
 pytestmark = pytest.mark.gpu
 
 
+@pytest.fixture(autouse=True)
+def _release_launch_tables():
+    """Every session here has its own buffers, hence its own cached launch tables (at most 64 per process)."""
+    yield
+    torch.cuda.synchronize()
+    mf.mfsdp_release_plans()
+
+
 class ShampooSession:
     def __init__(self, wl, ws_mode="full", **hp):
         pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, wl.rank)
@@ -56,7 +64,10 @@ class ShampooSession:
 
     def step(self, t):
         self.hG = workloads.fill_flat(self.wl, self.descs, workloads.KIND_G, step=t)
-        self.G = self.hG.cuda()
+        if self.G is None:
+            self.G = self.hG.cuda()
+        else:
+            self.G.copy_(self.hG)     # one gradient buffer per session: the launch tables are keyed by its address
         hp = mf.ShampooHParams(step=t, flags=self.flags, **self.hp_kw)
         mf.mfsdp_shampoo_step(self.desc, self.W, self.G, self.state, self.ws, hp)
         torch.cuda.synchronize()
@@ -262,6 +273,7 @@ def test_shampoo_c4_full_size_properties():
     sess.ws = gh.aligned_bytes(int(max(lo, min(hi, 64e9))))
     sess.hW = workloads.fill_flat(wl, sess.descs, workloads.KIND_W)
     sess.W = sess.hW.cuda()
+    sess.G = None
     sess.step(1)
     rng = np.random.default_rng(0)
     kw = sess.hp_kw
