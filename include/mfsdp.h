@@ -366,8 +366,11 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  *                               full_bytes processes them all at once (fewest launches), min_bytes one at a time.
  *   hp          HOST in.
  * Enqueues on cuda_stream and does not synchronise (the number of launches is fixed: converged problems are skipped
- * on the device).  Launch tables are cached per (table, W, G, state, workspace, ws_bytes, flags); at most 64 keys
- * (MFSDP_ECACHE beyond; mfsdp_release_plans frees them).  Errors as mfsdp_muon_step. */
+ * on the device).  Launch tables are cached per (table, state, workspace, ws_bytes, flags); at most 64 keys
+ * (MFSDP_ECACHE beyond; mfsdp_release_plans frees them).  W and G may be other buffers from call to call: the records that
+ * hold their addresses are re-pointed and re-uploaded in stream order (a few hundred KB, only when they change; calls
+ * on one table must then be ordered on one stream).  A captured CUDA graph keeps the addresses it was captured with.
+ * Errors as mfsdp_muon_step. */
 enum { MFSDP_SHAMPOO_KEEP_D = 1u };      /* flags bit0: also leave D = P_L G P_R (fp32) in the workspace              */
 typedef struct {
   double  lr;              /* eta                                                                                  */

@@ -313,6 +313,14 @@ struct ShPlan {
   SgTile* d_tiles = nullptr;
   RootInfo* d_roots = nullptr;
   GprepItem* d_gprep = nullptr;
+  // W and G are not part of the cache key (training code often hands over a fresh gradient tensor every step): the
+  // records that hold their addresses are kept on the host as well and re-pointed + re-uploaded when they change
+  uint8_t* W = nullptr;
+  const uint8_t* G = nullptr;
+  std::vector<SgProb> h_probs;
+  std::vector<GprepItem> h_gprep;
+  struct GwRef { uint32_t prob, mat, kind; };   // kind 0: statistics (both maps, side in bit 8), 1: P_L G (map b), 2: W
+  std::vector<GwRef> gw;
 };
 std::vector<std::unique_ptr<ShPlan>> g_sh_plans;
 constexpr size_t kMaxShPlans = 64;
@@ -444,6 +452,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       q.a_mn = q.b_mn = mn; q.sym = 1;
       q.f32_pitch = side ? m.pc : m.pr;
       q.cin = q.out_f32 = reinterpret_cast<float*>(state + (side ? m.R_off : m.L_off));
+      pl.gw.push_back(ShPlan::GwRef{(uint32_t)probs.size(), (uint32_t)i, (uint32_t)(side << 8)});
       add_tiles((uint32_t)probs.size() - pl.stat.prob_off, q.M, q.N, true);
       probs.push_back(q);
     }
@@ -557,6 +566,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     q.sp_pitch = m.pc; q.sp_plane = (uint64_t)m.rows * m.pc;
     q.out_split = reinterpret_cast<__nv_bfloat16*>(ws + m.Tm_off);
     if ((rc = make_store_tmap3(&q.to, q.out_split, m.rows, m.cols, m.pc, (uint64_t)m.rows * m.pc))) return rc;
+    pl.gw.push_back(ShPlan::GwRef{(uint32_t)probs.size(), (uint32_t)i, 1u});
     add_tiles((uint32_t)probs.size() - pl.pre1.prob_off, q.M, q.N, false);
     probs.push_back(q);
   }
@@ -572,6 +582,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     q.f32_pitch = m.pc;
     q.out_f32 = keep_d ? reinterpret_cast<float*>(ws + m.D_off) : nullptr;
     q.W = W + m.elem_off * esz; q.w_bf16 = m.dtype == MFSDP_BF16;
+    pl.gw.push_back(ShPlan::GwRef{(uint32_t)probs.size(), (uint32_t)i, 2u});
     add_tiles((uint32_t)probs.size() - pl.pre2.prob_off, q.M, q.N, false);
     probs.push_back(q);
   }
@@ -592,6 +603,40 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
   if (!roots.empty() && (e = cudaMemcpy(pl.d_roots, roots.data(), roots.size() * sizeof(RootInfo), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e);
   if (!gprep.empty() && (e = cudaMemcpy(pl.d_gprep, gprep.data(), gprep.size() * sizeof(GprepItem), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e);
   if ((rc = sg_setup<1, 1>()) || (rc = sg_setup<3, 1>()) || (rc = sg_setup<3, 3>())) return rc;
+  pl.W = W; pl.G = G;
+  pl.h_probs = std::move(probs);
+  pl.h_gprep = std::move(gprep);
+  return MFSDP_OK;
+}
+
+// The caller came with other W / G buffers than the tables were built for: re-point the records that hold their
+// addresses (tensor maps of an in-place bf16 gradient, staging sources, weight pointers) and upload them in stream order.
+int repoint_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, cudaStream_t st) {
+  const size_t esz = pl.lay.dtype == MFSDP_BF16 ? 2 : 4;
+  int rc;
+  for (const ShPlan::GwRef& ref : pl.gw) {
+    const ShMat& m = pl.lay.mats[ref.mat];
+    SgProb& q = pl.h_probs[ref.prob];
+    const uint8_t* g = G + m.elem_off * esz;
+    if ((ref.kind & 0xffu) == 0u) {
+      if (!m.g_direct) continue;
+      if ((rc = make_tmap3(&q.ta, g, m.rows, m.cols, m.cols, (uint64_t)m.rows * m.cols, 1, (ref.kind >> 8) != 0u))) return rc;
+      q.tb = q.ta;
+    } else if (ref.kind == 1u) {
+      if (!m.g_direct) continue;
+      if ((rc = make_tmap3(&q.tb, g, m.rows, m.cols, m.cols, (uint64_t)m.rows * m.cols, 1, true))) return rc;
+    } else {
+      q.W = W + m.elem_off * esz;
+    }
+  }
+  size_t k = 0;
+  for (const ShMat& m : pl.lay.mats)
+    if (!m.g_direct) pl.h_gprep[k++].src = G + m.elem_off * esz;
+  cudaError_t e = cudaMemcpyAsync(pl.d_probs, pl.h_probs.data(), pl.h_probs.size() * sizeof(SgProb), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess && !pl.h_gprep.empty())
+    e = cudaMemcpyAsync(pl.d_gprep, pl.h_gprep.data(), pl.h_gprep.size() * sizeof(GprepItem), cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) return cuda_fail(e);
+  pl.W = W; pl.G = G;
   return MFSDP_OK;
 }
 
@@ -605,7 +650,7 @@ int get_sh_plan(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G,
   if (major != 10) return MFSDP_EARCH;
   std::vector<uint8_t> key(n_desc * sizeof(mfsdp_desc_t) + 64);
   if (n_desc) std::memcpy(key.data(), desc, n_desc * sizeof(mfsdp_desc_t));
-  const uint64_t tail[8] = {(uint64_t)dev, (uint64_t)(uintptr_t)W, (uint64_t)(uintptr_t)G, (uint64_t)(uintptr_t)state,
+  const uint64_t tail[8] = {(uint64_t)dev, 0u, 0u, (uint64_t)(uintptr_t)state,
                             (uint64_t)(uintptr_t)ws, (uint64_t)ws_bytes, keep_d ? 1u : 0u, 0u};
   std::memcpy(key.data() + n_desc * sizeof(mfsdp_desc_t), tail, 64);
   std::lock_guard<std::mutex> lock(plan_mutex());
@@ -698,6 +743,10 @@ extern "C" int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void*
   if (rc) return rc;
   if (state_bytes < pl->lay.state_bytes) return MFSDP_ECAP;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (pl->W != W || pl->G != G) {
+    std::lock_guard<std::mutex> lock(plan_mutex());
+    if ((rc = repoint_sh_plan(*pl, reinterpret_cast<uint8_t*>(W), reinterpret_cast<const uint8_t*>(G), st))) return rc;
+  }
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
   ShCtl* d_ctl = reinterpret_cast<ShCtl*>(ws + pl->lay.ctl_off);
   double* d_part = reinterpret_cast<double*>(ws + pl->lay.partial_off);

@@ -317,3 +317,22 @@ def test_shampoo_c4_full_size_properties():
         assert max(res) <= 1.6e-1
         assert eD <= 1e-5
         assert np.all((got >= bf16_rne(want - delta)) & (got <= bf16_rne(want + delta)))
+
+
+def test_shampoo_fresh_weight_and_gradient_buffers_reuse_the_tables():
+    """W and G are not part of the cache key: a caller that hands over a new gradient tensor every step (and moves its
+    weights) gets the bits of a caller with persistent buffers, from the same cached launch tables."""
+    for wl in (workloads.medium_ragged(), workloads.small_ragged(dtype=workloads.F32)):   # in-place bf16 G / staged G
+        a, b = ShampooSession(wl, eps=1e-3), ShampooSession(wl, eps=1e-3)
+        keep = []                                        # earlier tensors stay alive: every new one has a new address
+        for t in (1, 2, 3):
+            a.step(t)
+            keep.append(b.G)
+            b.G = None                                   # step() then uploads into a new tensor
+            if t == 2:
+                keep.append(b.W)
+                b.W = b.W.clone()
+            b.step(t)
+            assert all(k is None or k.data_ptr() != b.G.data_ptr() for k in keep)
+        assert torch.equal(a.W.view(torch.uint8), b.W.view(torch.uint8))
+        assert torch.equal(a.state, b.state)
