@@ -336,3 +336,41 @@ def test_shampoo_fresh_weight_and_gradient_buffers_reuse_the_tables():
             assert all(k is None or k.data_ptr() != b.G.data_ptr() for k in keep)
         assert torch.equal(a.W.view(torch.uint8), b.W.view(torch.uint8))
         assert torch.equal(a.state, b.state)
+
+
+def test_shampoo_poisoned_workspace_and_guard_bands():
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer_closed.md); what stands in for memcheck /
+    initcheck here: (a) the workspace is scratch -- filled with NaN bit patterns before every step it must give the
+    bits of a zero-filled one (no kernel reads a byte it has not written: pitch padding, unwritten tile edges, stale
+    root buffers); (b) 64 KB guard bands around W, the state and the workspace stay intact and G is never written."""
+    guard = 65536
+
+    def banded(nbytes, fill):
+        raw = torch.empty(nbytes + 2 * guard + 1024, dtype=torch.uint8, device="cuda")
+        off = (-(raw.data_ptr() + guard)) % 1024
+        raw.fill_(0xA5)
+        mid = raw[off + guard: off + guard + nbytes]
+        mid.fill_(fill)
+        return raw, mid, (off, nbytes)
+
+    def bands_intact(raw, where):
+        off, nbytes = where
+        return bool((raw[:off + guard] == 0xA5).all()) and bool((raw[off + guard + nbytes:] == 0xA5).all())
+
+    outs = []
+    for poison in (0x00, 0xFF):                          # 0xFFFF = a bf16 NaN, 0xFFFFFFFF = an fp32 NaN
+        s = ShampooSession(workloads.small_ragged())
+        raw_ws, s.ws, w_ws = banded(s.ws.numel(), poison)
+        raw_st, s.state, w_st = banded(s.state.numel(), 0x00)
+        raw_w, wbytes, w_w = banded(s.W.numel() * 2, 0x00)
+        wbytes.view(torch.bfloat16).copy_(s.W)
+        s.W = wbytes.view(torch.bfloat16)
+        for t in (1, 2):
+            if t == 2:
+                s.ws.fill_(poison)
+            s.step(t)
+            assert torch.equal(s.G.cpu(), s.hG), "G is read-only"
+        assert bands_intact(raw_ws, w_ws) and bands_intact(raw_st, w_st) and bands_intact(raw_w, w_w)
+        outs.append((s.W.clone(), s.state.clone()))
+    assert torch.equal(outs[0][0].view(torch.int16), outs[1][0].view(torch.int16))
+    assert torch.equal(outs[0][1], outs[1][1])
