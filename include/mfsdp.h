@@ -353,7 +353,9 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  *   S5  the roots are recomputed at steps with (step - 1) % root_every == 0, from statistics that include G_step;
  *       other steps reuse the stored roots
  *   S6  the roots are computed by the coupled Newton iteration  M_0 = z S~, X_0 = z^{1/4} I, z = 5 / (2 (||S||_F + rho)),
- *       T = (5 I - M) / 4, X <- X T, M <- T^4 M  until max |M - I| < root_tol, the error stops falling (fp32-class
+ *       T = (5 I - M) / 4, X <- X T, M <- T^4 M  (the first iterations additionally scale M by 2.5 and X by 2.5^(1/4):
+ *       every eigenvalue of M is <= 1 after an iteration, so the scaled M stays inside the convergence region and
+ *       its small eigenvalues grow 6.1 x instead of 2.44 x per iteration)  until max |M - I| < root_tol, the error stops falling (fp32-class
  *       noise floor) or max_root_iters is reached; X -> S~^{-1/4}.
  * Arithmetic: every matrix product runs on the bf16 tensor cores with fp32 values carried as three bf16 terms
  * (24 significand bits, fp32 exponent range) and fp32 accumulation -- fp32-class, not bit-identical to an fp32 FFMA loop.
@@ -381,7 +383,7 @@ typedef struct {
   double  root_tol;        /* 0 -> 1e-6                                                                            */
   int64_t step;            /* 1-based                                                                              */
   int32_t root_every;      /* >= 1                                                                                 */
-  int32_t max_root_iters;  /* 0 -> ceil(log(2.5 / eps_floor) / log(2.44)) + 6 (23 at 2^-20), 40 without a floor    */
+  int32_t max_root_iters;  /* 0 -> ceil(log(0.08 / eps_floor) / log(6.1)) + 9 (16 at 2^-20), 40 without a floor     */
   uint32_t flags;          /* MFSDP_SHAMPOO_*                                                                      */
   uint32_t reserved;       /* 0                                                                                    */
 } mfsdp_shampoo_hparams_t;
@@ -395,7 +397,8 @@ int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const v
  * rows x out[4] bf16, out[6] elements apart), P_R (3 planes of cols x out[5] bf16, out[7] elements apart);
  * out[8] = byte offset in the workspace of D (rows x out[5] floats; MFSDP_SHAMPOO_KEEP_D only);
  * out[9] = byte offset in the workspace of the root control records of this matrix (L then R), out[10] bytes each:
- *   { double tr, fro2; float rho, z, x0, last_err; uint32 err_bits, iters, done (1 converged / stopped, 2 NaN), identity }. */
+ *   { double tr, fro2; float rho, z, x0, last_err; uint32 err_bits, iters, done (1 converged / stopped, 2 NaN), identity;
+ *     float alpha_m, alpha_x; uint32 n_scaled, pad }. */
 int mfsdp_shampoo_view(const mfsdp_desc_t* desc, size_t n_desc, uint32_t flags, size_t index, size_t out[12]);
 
 /* Debug / test aid (HOST): byte offsets inside the workspace of the `index`-th matrix' NS buffers:

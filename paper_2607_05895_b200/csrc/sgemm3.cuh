@@ -57,6 +57,7 @@ struct alignas(64) SgProb {
   __nv_bfloat16* t_split;           // optional: split of (5 I - v) / 4
   uint32_t* err;                    // optional: atomicMax of the bits of max |v - delta|
   const uint32_t* done;             // optional: non-zero -> the problem is finished, its tiles are skipped
+  const float* alpha_dev;           // optional: per-problem factor on top of the launch's alpha (read at tile start)
   void* W;                          // optional: rank-flat weights of this matrix (pitch = N), updated in place
   uint32_t w_bf16;                  // dtype of W
   uint32_t pad;
@@ -236,6 +237,7 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
   const bool row_ok = r < M;
   uint32_t emax = 0u;                                         // bits of max |v - delta| (NaN sorts above everything)
   if (row0 >= M) return;                                      // warp-uniform
+  const float alpha = pr->alpha_dev != nullptr ? p.alpha * *pr->alpha_dev : p.alpha;
   const float* cin = pr->cin;
   float* of32 = pr->out_f32;
   __nv_bfloat16* osp = pr->out_split;
@@ -252,7 +254,7 @@ __device__ __forceinline__ void sg_finish_row(const SgProb* pr, const SgParams& 
       const uint32_t c0 = n0 + 16u * g;
       float* v = acc + 16 * g;                                  // compile-time offsets: stays in registers
 #pragma unroll
-      for (int j = 0; j < 16; ++j) v[j] *= p.alpha;
+      for (int j = 0; j < 16; ++j) v[j] *= alpha;
       if (!row_ok) continue;
       if (cin != nullptr) {
         const float4* src = reinterpret_cast<const float4*>(cin + (size_t)r * fp + c0);

@@ -6,7 +6,8 @@
 //   S2  A = S + eps (tr S / d) I                                              k_sh_reduce, k_sh_root_init
 //   S3  P = A^{-1/4}  by the coupled Newton iteration (reading S6):           3 grouped GEMM launches + k_sh_root_ctl
 //         M_0 = z A, X_0 = z^{1/4} I, z = 5 / (2 (||S||_F + rho));           per iteration, for every L and R of the
-//         T = (5 I - M) / 4 ; X <- X T ; M <- T^4 M ; stop at max |M - I| < tol  group at once
+//         T = (5 I - M) / 4 ; X <- X T ; M <- T^4 M ; stop at max |M - I| < tol  group at once; the first iterations
+//         also scale M by 2.5 and X by 2.5^(1/4) (k_sh_root_init: 6.1 x instead of 2.44 x growth of small eigenvalues)
 //   S4  D = P_L G P_R ; W <- W (1 - lr wd) - lr D                             two grouped GEMM launches, update fused
 //   S5  roots only at steps with (t - 1) % root_every == 0; P_L, P_R are kept (as three bf16 planes) in the state.
 // All matrix products run on the tensor cores with three-term bf16 operands (sgemm3.cuh).  Every problem of a launch is
@@ -29,13 +30,17 @@ namespace {
 
 constexpr uint32_t kRedBlocks = 64;      // row groups of the trace / Frobenius reduction (fixed: deterministic sums)
 constexpr uint32_t kRootBufs = 7;        // X ping-pong, M ping-pong, T, T^2, T^4
+constexpr uint32_t kPartWords = 4;       // per row group: sum of squares, trace, |S x|^2 of the even / odd power iterations
+constexpr uint32_t kPowerIters = 8;      // power iterations for the bound on lambda_max (reading S6)
 
 struct ShCtl {                           // per root problem, device (layout documented in mfsdp.h: tests read it)
   double tr, fro2;
   float rho, z, x0, prev_err;
   uint32_t err, iters, done, identity;
+  float alpha_m, alpha_x;                // factors on the NEXT iteration's M' and X' (scaled phase: 2.5 and 2.5^(1/4))
+  uint32_t n_scaled, pad;                // iterations whose outputs are scaled
 };
-static_assert(sizeof(ShCtl) == 48, "ShCtl layout is part of the debug ABI");
+static_assert(sizeof(ShCtl) == 64, "ShCtl layout is part of the debug ABI");
 
 struct RootInfo {                        // per root problem, device
   const float* S;                        // statistic, d x pitch fp32
@@ -45,6 +50,7 @@ struct RootInfo {                        // per root problem, device
   __nv_bfloat16* M0;
   __nv_bfloat16* T;
   __nv_bfloat16* P;                      // state: the root, three planes
+  float* vec;                            // two vectors of `pitch` floats for the power iteration (inside the T^2 buffer)
   uint32_t ctl;                          // index into the ShCtl array
   uint32_t pad;
 };
@@ -96,9 +102,49 @@ __global__ void __launch_bounds__(256) k_sh_reduce(const RootInfo* roots, double
     __syncthreads();
   }
   if (threadIdx.x == 0) {
-    double* out = partials + ((size_t)ri.ctl * kRedBlocks + blockIdx.x) * 2;
+    double* out = partials + ((size_t)ri.ctl * kRedBlocks + blockIdx.x) * kPartWords;
     out[0] = sh[0][0]; out[1] = sh[1][0];
   }
+}
+
+// One step of the power iteration y = S x / |x| for every statistic of the group (a lower bound on lambda_max: the
+// Frobenius norm alone costs 4-5 extra Newton iterations).  x of step 0 is a fixed pseudo-random vector; the squared
+// norm of y is left as per-block partials (fixed order: deterministic) and divides the next step's x on the fly.
+__global__ void __launch_bounds__(256) k_sh_power(const RootInfo* roots, double* partials, uint32_t it) {
+  const RootInfo ri = roots[blockIdx.y];
+  const float* xin = ri.vec + (it & 1u) * ri.pitch;
+  float* yout = ri.vec + ((it + 1u) & 1u) * ri.pitch;
+  __shared__ float red[8];
+  __shared__ float scale_sh;
+  if (threadIdx.x == 0) {
+    double n2 = 0.0;
+    if (it > 0)
+      for (uint32_t b = 0; b < kRedBlocks; ++b) n2 += partials[((size_t)ri.ctl * kRedBlocks + b) * kPartWords + 2 + ((it - 1u) & 1u)];
+    scale_sh = it > 0 ? (n2 > 0.0 ? (float)(1.0 / sqrt(n2)) : 0.f) : 1.f;
+  }
+  __syncthreads();
+  const float sc = scale_sh;
+  double acc2 = 0.0;
+  for (uint32_t r = blockIdx.x; r < ri.d; r += gridDim.x) {
+    const float* row = ri.S + (size_t)r * ri.pitch;
+    float sum = 0.f;
+    for (uint32_t c = threadIdx.x; c < ri.d; c += blockDim.x) {
+      const float x = it > 0 ? xin[c] * sc : (float)((c * 2654435761u + 0x9e3779b9u) >> 16 & 0xffffu) * (1.f / 32768.f) - 1.f;
+      sum = fmaf(row[c], x, sum);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if ((threadIdx.x & 31u) == 0) red[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      float y = 0.f;
+      for (int w = 0; w < 8; ++w) y += red[w];
+      yout[r] = y;
+      acc2 += (double)y * (double)y;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partials[((size_t)ri.ctl * kRedBlocks + blockIdx.x) * kPartWords + 2 + (it & 1u)] = acc2;
 }
 
 __global__ void k_sh_root_init(const RootInfo* roots, uint32_t n, ShCtl* ctl, const double* partials, double eps,
@@ -106,22 +152,41 @@ __global__ void k_sh_root_init(const RootInfo* roots, uint32_t n, ShCtl* ctl, co
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const RootInfo ri = roots[i];
-  double s2 = 0.0, tr = 0.0;
+  double s2 = 0.0, tr = 0.0, lam2 = 0.0;
   for (uint32_t b = 0; b < kRedBlocks; ++b) {
-    s2 += partials[((size_t)ri.ctl * kRedBlocks + b) * 2];
-    tr += partials[((size_t)ri.ctl * kRedBlocks + b) * 2 + 1];
+    s2 += partials[((size_t)ri.ctl * kRedBlocks + b) * kPartWords];
+    tr += partials[((size_t)ri.ctl * kRedBlocks + b) * kPartWords + 1];
+    lam2 += partials[((size_t)ri.ctl * kRedBlocks + b) * kPartWords + 2 + ((kPowerIters - 1u) & 1u)];
   }
   ShCtl c;
   c.tr = tr; c.fro2 = s2;
   c.err = 0u; c.iters = 0u; c.prev_err = 3.0e38f;
   if (!(tr > 0.0)) {                      // reading S2: no gradient seen yet -> the preconditioner is I
     c.identity = 1u; c.done = 1u; c.rho = 0.f; c.z = 1.f; c.x0 = 1.f;
+    c.alpha_m = c.alpha_x = 1.f; c.n_scaled = 0u; c.pad = 0u;
   } else {
     const double rho = fmax(eps * tr / (double)ri.d, eps_floor * sqrt(s2));   // readings S2, S7
-    const double bound = sqrt(s2) + rho;  // >= lambda_max(S + rho I)
+    // lambda_max(S) <= ||S||_F always; the power iteration gives |S x| <= lambda_max from below, within a factor of
+    // d^(1 / 2k) = 1.8 of it at worst after k = 8 steps from a start vector with a 1 / sqrt(d) component along the top
+    // eigenvector (d = 14336) and within a few percent on spectra with a cluster at the top; M_0's eigenvalues have to
+    // stay below 5 for the iteration to converge: bound / lambda_max >= 1.6 / 1.8 * ... is ample (2.5 lambda_max /
+    // bound < 5 needs bound > lambda_max / 2).  A tighter bound saves iterations: ||S||_F overestimates a flat
+    // rank-r spectrum by sqrt(r), i.e. log(sqrt(r)) / log(2.44) = 4-5 of ~18 iterations.
+    const double lam = sqrt(lam2);
+    const double top = lam > 0.0 && lam == lam ? fmin(sqrt(s2), 1.6 * lam) : sqrt(s2);
+    const double bound = top + rho;       // taken as lambda_max(S + rho I)
     const double z = 2.5 / bound;         // (1 + p) / (2 ||A||), p = 4
     c.identity = 0u; c.done = 0u;
     c.rho = (float)rho; c.z = (float)z; c.x0 = (float)sqrt(sqrt(z));
+    // Scaled phase.  After any iteration every eigenvalue of M is <= 1 (mu ((5 - mu) / 4)^4 <= 1 on (0, 5)), so M may
+    // be multiplied by 2.5 (and X by 2.5^(1/4): X^4 S~ z = M is kept) without leaving the convergence region: small
+    // eigenvalues then grow by 2.5 x 2.44 = 6.1 per iteration instead of 2.44.  The smallest eigenvalue of M_0 is at
+    // least mu0 = 2.5 rho / bound; scaling stops when that lower bound has reached 0.2, the plain iteration finishes.
+    const double mu0 = 2.5 * rho / bound;
+    c.n_scaled = mu0 > 0.0 && mu0 < 0.2 ? (uint32_t)floor(log(0.2 / mu0) / log(6.103515625)) : 0u;
+    c.alpha_m = c.n_scaled >= 1u ? 2.5f : 1.f;
+    c.alpha_x = c.n_scaled >= 1u ? 1.2574334f : 1.f;        // 2.5^(1/4)
+    c.pad = 0u;
   }
   ctl[ri.ctl] = c;
 }
@@ -170,6 +235,9 @@ __global__ void k_sh_root_ctl(const RootInfo* roots, uint32_t n, ShCtl* ctl, flo
   if (!(e == e)) c->done = 2u;
   c->prev_err = e;
   c->err = 0u;
+  const bool scale_next = c->iters + 1u <= c->n_scaled;      // the outputs of iteration iters + 1
+  c->alpha_m = scale_next ? 2.5f : 1.f;
+  c->alpha_x = scale_next ? 1.2574334f : 1.f;
 }
 
 // P <- X[iters & 1].  A root whose iteration produced a NaN (done == 2: S + rho I was not positive definite in this
@@ -281,7 +349,7 @@ int build_sh_layout(const mfsdp_desc_t* desc, size_t n_desc, bool keep_d, ShLayo
   const uint64_t n_prob = 2 * out.mats.size();
   uint64_t ws = 0;
   out.ctl_off = ws; ws = align_up_u64(ws + n_prob * sizeof(ShCtl), kBufAlign);
-  out.partial_off = ws; ws = align_up_u64(ws + n_prob * kRedBlocks * 2 * sizeof(double), kBufAlign);
+  out.partial_off = ws; ws = align_up_u64(ws + n_prob * kRedBlocks * kPartWords * sizeof(double), kBufAlign);
   for (ShMat& m : out.mats) {
     if (!m.g_direct) { m.Gs_off = ws; ws = align_up_u64(ws + (uint64_t)m.g_terms * m.rows * m.pc * 2, kBufAlign); }
     m.Tm_off = ws; ws = align_up_u64(ws + (uint64_t)3 * m.rows * m.pc * 2, kBufAlign);
@@ -494,6 +562,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       ri.d = r.d; ri.pitch = r.pitch; ri.plane = (uint64_t)r.d * r.pitch;
       ri.X[0] = b.b[0]; ri.X[1] = b.b[1]; ri.M0 = b.b[2]; ri.T = b.b[4];
       ri.P = reinterpret_cast<__nv_bfloat16*>(state + (r.side ? m.PR_off : m.PL_off));
+      ri.vec = reinterpret_cast<float*>(b.b[5]);
       ri.ctl = (uint32_t)(2 * r.mat + r.side); ri.pad = 0;
       roots.push_back(ri);
       g.max_d = std::max(g.max_d, r.d);
@@ -501,7 +570,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     g.n_roots = (uint32_t)(at - first);
     // buffer roles: 0, 1 = X ping-pong; 2, 3 = M ping-pong; 4 = T; 5 = T^2; 6 = T^4
     auto sym_prob = [&](const RootRef& r, const __nv_bfloat16* a, const __nv_bfloat16* b, __nv_bfloat16* out,
-                        __nv_bfloat16* tsplit, bool err, SgProb& q) -> int {
+                        __nv_bfloat16* tsplit, bool err, SgProb& q, int scaled = 0) -> int {
       q = zero_prob();
       const uint64_t plane = (uint64_t)r.d * r.pitch;
       int e;
@@ -515,6 +584,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       ShCtl* c = d_ctl + (2 * r.mat + r.side);
       q.done = &c->done;
       q.err = err ? &c->err : nullptr;
+      q.alpha_dev = scaled == 1 ? &c->alpha_x : scaled == 2 ? &c->alpha_m : nullptr;
       return MFSDP_OK;
     };
     for (int par = 0; par < 2; ++par) {
@@ -522,7 +592,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       for (size_t k = first; k < at; ++k) {
         const Bufs& b = bufs[k - first];
         SgProb q;
-        if ((rc = sym_prob(refs[k], b.b[par], b.b[4], b.b[par ^ 1], nullptr, false, q))) return rc;   // X' = X T
+        if ((rc = sym_prob(refs[k], b.b[par], b.b[4], b.b[par ^ 1], nullptr, false, q, 1))) return rc;   // X' = X T
         add_tiles((uint32_t)probs.size() - g.a[par].prob_off, q.M, q.N, true);
         probs.push_back(q);
         if ((rc = sym_prob(refs[k], b.b[4], b.b[4], b.b[5], nullptr, false, q))) return rc;           // T^2 = T T
@@ -545,7 +615,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
       for (size_t k = first; k < at; ++k) {
         const Bufs& b = bufs[k - first];
         SgProb q;
-        if ((rc = sym_prob(refs[k], b.b[6], b.b[2 + par], b.b[2 + (par ^ 1)], b.b[4], true, q))) return rc;   // M' = T^4 M
+        if ((rc = sym_prob(refs[k], b.b[6], b.b[2 + par], b.b[2 + (par ^ 1)], b.b[4], true, q, 2))) return rc;   // M' = T^4 M
         add_tiles((uint32_t)probs.size() - g.c[par].prob_off, q.M, q.N, true);
         probs.push_back(q);
       }
@@ -760,18 +830,20 @@ extern "C" int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void*
   if ((rc = sg_launch(*pl, pl->stat, (float)w, (float)hp->beta2, 0.f, 0.f, st))) return rc;
 
   if ((hp->step - 1) % hp->root_every == 0) {                                   // reading S5
-    // Launch budget.  The smallest eigenvalue of M_0 is at least 2.5 rho / (||S||_F + rho) >= 2.5 eps_floor / (1 + eps_floor)
-    // and grows by (5/4)^4 = 2.44 per iteration until the quadratic phase (<= 6 more iterations): with the default floor
-    // 2^-20 that is 23 iterations (19 observed at most); without a floor 40.  Converged problems skip their tiles anyway;
-    // the budget only bounds the number of (then empty) launches enqueued.
+    // Launch budget.  The smallest eigenvalue of M_0 is at least mu0 = 2.5 rho / bound >= 2.5 eps_floor / (1 + eps_floor);
+    // the scaled phase takes it to 0.2 in log(0.2 / mu0) / log(6.1) iterations (7 with the default floor 2^-20), the
+    // plain iteration needs at most 9 more down to the noise floor: 16 (13 observed at most); without a floor 40.
+    // Converged problems skip their tiles anyway; the budget only bounds the number of (then empty) launches enqueued.
     uint32_t max_iters = 40u;
     if (hp->max_root_iters) max_iters = (uint32_t)hp->max_root_iters;
     else if (hp->eps_floor > 0.0)
-      max_iters = std::min<uint32_t>(40u, (uint32_t)std::ceil(std::log(2.5 * (1.0 + hp->eps_floor) / hp->eps_floor) / std::log(2.44140625)) + 6u);
+      max_iters = std::min<uint32_t>(40u, (uint32_t)std::ceil(std::log(0.08 * (1.0 + hp->eps_floor) / hp->eps_floor) / std::log(6.103515625)) + 9u);
     const float tol = hp->root_tol > 0.0 ? (float)hp->root_tol : 1e-6f;
     for (const RootGroup& g : pl->groups) {
       const RootInfo* roots = pl->d_roots + g.root_off;
       k_sh_reduce<<<dim3(kRedBlocks, g.n_roots), 256, 0, st>>>(roots, d_part);
+      for (uint32_t it = 0; it < kPowerIters; ++it) k_sh_power<<<dim3(kRedBlocks, g.n_roots), 256, 0, st>>>(roots, d_part, it);
+      count_launch(kPowerIters);
       k_sh_root_init<<<(g.n_roots + 127) / 128, 128, 0, st>>>(roots, g.n_roots, d_ctl, d_part, hp->eps, hp->eps_floor);
       k_sh_root_prep<<<dim3(std::min<uint32_t>(g.max_d, 1024u), g.n_roots), 256, 0, st>>>(roots, d_ctl);
       count_launch(3);

@@ -328,7 +328,7 @@ def test_shampoo_layout_and_argument_checks_without_a_gpu():
         v = mf.mfsdp_shampoo_view(pr.desc, mf.SHAMPOO_KEEP_D, i)
         pr_, pc_ = v[4], v[5]
         assert pr_ >= d.rows and pc_ >= d.cols and pr_ % 64 == 0 and pc_ % 64 == 0
-        assert v[6] == d.rows * pr_ and v[7] == d.cols * pc_ and v[10] == 48
+        assert v[6] == d.rows * pr_ and v[7] == d.cols * pc_ and v[10] == 64
         for off, nbytes in ((v[0], d.rows * pr_ * 4), (v[1], d.cols * pc_ * 4), (v[2], 3 * v[6] * 2), (v[3], 3 * v[7] * 2)):
             assert off % 1024 == 0 and off + nbytes <= total
             spans.append((off, off + nbytes))
