@@ -456,7 +456,8 @@ def measure_shampoo(torch, mf, name, pk, local, ws_cap_bytes=64e9):
     """One record of `other_configs` for the owner-local Shampoo step on a
     BASELINE.json config: step 1 recomputes every inverse fourth root (root_every = 2), step 2 reuses them.  Flops are
     counted from the iteration counts the device reports: fp32-class flops (symmetric products count once) and the
-    bf16 UMMA flops actually issued for them (x6 for three-term operands, x3 / x1 where the bf16 gradient is one term),
+    bf16 UMMA flops actually issued for them (x6 for three-term operands, x3 / x2 for the two-term preconditioning
+    products, x1 for the statistics of a bf16 gradient),
     the latter against the bf16 tensor peak."""
     import numpy as np
     import workloads
@@ -511,7 +512,7 @@ def measure_shampoo(torch, mf, name, pk, local, ws_cap_bytes=64e9):
             stat = float(d.rows) * d.rows * d.cols + float(d.cols) * d.cols * d.rows
             p1, p2 = 2.0 * d.rows * d.rows * d.cols, 2.0 * d.rows * d.cols * d.cols
             f32 += stat + p1 + p2
-            umma += stat * gt * (gt + 1) / 2 + p1 * 3 * (1 if gt == 1 else 2) + p2 * 6
+            umma += stat * gt * (gt + 1) / 2 + p1 * (2 if gt == 1 else 3) + p2 * 3      # S4 runs on two-term operands
         recs.append(dict(ms=ms, launches=mf.mfsdp_launch_count() - n0, f32_class_tflops=f32 / ms / 1e9,
                          umma_bf16_tflops=umma / ms / 1e9, root_iters_max=max(iters), root_iters_mean=float(np.mean(iters))))
     clocks = sampler.stop()

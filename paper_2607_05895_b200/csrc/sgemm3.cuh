@@ -77,7 +77,10 @@ constexpr uint32_t kSgThreads = 192;
 constexpr uint32_t kSgBox = 16384;  // one term of one operand of one stage: 128 rows x 64 k, or 2 x (64 k x 64 mn)
 template <int AT, int BT> struct SgCfg {
   static constexpr uint32_t kStage = (AT + BT) * kSgBox;
-  static constexpr uint32_t kStages = (AT + BT) == 2 ? 6 : (AT + BT) == 4 ? 3 : 2;
+  static constexpr uint32_t kStages = (AT + BT) == 2 ? 6 : (AT + BT) == 3 ? 4 : (AT + BT) == 4 ? 3 : 2;
+  // term products kept: i + j <= kOrder.  Three terms: the six with i + j <= 2 (2^-24-class); two terms: the three with
+  // i + j <= 1 (2^-16-class, for the products around a preconditioner that is itself accurate to 1e-3 at best)
+  static constexpr int kOrder = (AT > BT ? AT : BT) - 1;
   static constexpr uint32_t kSmem = kStages * kStage + 256 + 1024 + 8 * 32 * 33 * 4;   // ring, barriers, alignment, 8 transposition tiles
   // k blocks per TMEM chunk.  One: at most four truncating adds of leading-term products per partial sum.  (With one
   // term per operand a block is 256 cycles of UMMA, less than the epilogue warps need to fold it -- 4 tcgen05.ld of 32
@@ -458,7 +461,7 @@ __global__ void __launch_bounds__(kSgThreads, 1) k_sgemm3(const SgParams p) {
             for (int i = 0; i < AT; ++i)
 #pragma unroll
               for (int j = 0; j < BT; ++j)
-                if (i + j <= 2 && i + j > 0) {
+                if (i + j <= Cfg::kOrder && i + j > 0) {
 #pragma unroll
                   for (uint32_t ks = 0; ks < 4; ++ks) {
                     ptx::umma_bf16(d_tmem, ad[i] + (uint64_t)(ks * a_step), bd[j] + (uint64_t)(ks * b_step), idesc, first ? 0u : 1u);
@@ -687,7 +690,7 @@ __global__ void __launch_bounds__(kSgPairThreads, 1) k_sgemm3p(const SgParams p)
             for (int i = 0; i < AT; ++i)
 #pragma unroll
               for (int j = 0; j < BT; ++j)
-                if (i + j <= 2 && i + j > 0) {
+                if (i + j <= Cfg::kOrder && i + j > 0) {
 #pragma unroll
                   for (uint32_t ks = 0; ks < 4; ++ks) {
                     ptx::umma_bf16_cg2(d_tmem, ad[i] + (uint64_t)(ks * a_step), bd[j] + (uint64_t)(ks * b_step), idesc, first ? 0u : 1u);

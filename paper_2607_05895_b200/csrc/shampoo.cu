@@ -438,13 +438,15 @@ int sg_launch(const ShPlan& pl, const SgLaunch& L, float alpha, float beta, floa
   if (L.pair) {
     const uint32_t pairs = std::min<uint32_t>(L.n_tiles, (uint32_t)pl.sms / 2);
     const cudaError_t e = L.at == 1 && L.bt == 1 ? sg_launch_pair<1, 1>(p, pairs, st)
-                          : L.at == 3 && L.bt == 1 ? sg_launch_pair<3, 1>(p, pairs, st) : sg_launch_pair<3, 3>(p, pairs, st);
+                          : L.at == 2 && L.bt == 1 ? sg_launch_pair<2, 1>(p, pairs, st)
+                          : L.at == 2 && L.bt == 2 ? sg_launch_pair<2, 2>(p, pairs, st) : sg_launch_pair<3, 3>(p, pairs, st);
     count_launch();
     return e == cudaSuccess ? check_last_launch() : cuda_fail(e);
   }
   const uint32_t grid = std::min<uint32_t>(L.n_tiles, (uint32_t)pl.sms);
   if (L.at == 1 && L.bt == 1) k_sgemm3<1, 1><<<grid, kSgThreads, SgCfg<1, 1>::kSmem, st>>>(p);
-  else if (L.at == 3 && L.bt == 1) k_sgemm3<3, 1><<<grid, kSgThreads, SgCfg<3, 1>::kSmem, st>>>(p);
+  else if (L.at == 2 && L.bt == 1) k_sgemm3<2, 1><<<grid, kSgThreads, SgCfg<2, 1>::kSmem, st>>>(p);
+  else if (L.at == 2 && L.bt == 2) k_sgemm3<2, 2><<<grid, kSgThreads, SgCfg<2, 2>::kSmem, st>>>(p);
   else k_sgemm3<3, 3><<<grid, kSgThreads, SgCfg<3, 3>::kSmem, st>>>(p);
   count_launch();
   return check_last_launch();
@@ -625,7 +627,10 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
   }
 
   // S4: Tm = P_L G, then D = Tm P_R with the weight update in the epilogue
-  begin(pl.pre1, 3, gt);
+  // S4 runs with TWO terms per operand (products with i + j <= 1: 2^-16-class).  The roots themselves carry a relative
+  // error of 1e-3 .. 1e-2 in their ridge directions (Shampoo tolerances); a third term in the products
+  // around them buys nothing and costs twice the UMMAs.
+  begin(pl.pre1, 2, gt == 1 ? 1 : 2);
   for (size_t oi = 0; oi < n_mat; ++oi) {
     const size_t i = order[oi];
     const ShMat& m = lay.mats[i];
@@ -641,7 +646,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
     probs.push_back(q);
   }
   end(pl.pre1);
-  begin(pl.pre2, 3, 3);
+  begin(pl.pre2, 2, 2);
   for (size_t oi = 0; oi < n_mat; ++oi) {
     const size_t i = order[oi];
     const ShMat& m = lay.mats[i];
@@ -672,7 +677,7 @@ int build_sh_plan(ShPlan& pl, uint8_t* W, const uint8_t* G, uint8_t* state, uint
   if (!tiles.empty() && (e = cudaMemcpy(pl.d_tiles, tiles.data(), tiles.size() * sizeof(SgTile), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e);
   if (!roots.empty() && (e = cudaMemcpy(pl.d_roots, roots.data(), roots.size() * sizeof(RootInfo), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e);
   if (!gprep.empty() && (e = cudaMemcpy(pl.d_gprep, gprep.data(), gprep.size() * sizeof(GprepItem), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e);
-  if ((rc = sg_setup<1, 1>()) || (rc = sg_setup<3, 1>()) || (rc = sg_setup<3, 3>())) return rc;
+  if ((rc = sg_setup<1, 1>()) || (rc = sg_setup<2, 1>()) || (rc = sg_setup<2, 2>()) || (rc = sg_setup<3, 3>())) return rc;
   pl.W = W; pl.G = G;
   pl.h_probs = std::move(probs);
   pl.h_gprep = std::move(gprep);

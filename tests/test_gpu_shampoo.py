@@ -315,7 +315,7 @@ def test_shampoo_c4_full_size_properties():
         # statistic is rank-deficient; the derived bound is 4 x 6e-2 (module docstring), measured 7e-2 at d = 4096 with
         # three quarters of the spectrum at the ridge (the rounding noise of the statistic grows like sqrt(d))
         assert max(res) <= 1.6e-1
-        assert eD <= 1e-5
+        assert eD <= 1e-4         # the two preconditioning products carry their operands to two bf16 terms (2^-16-class)
         assert np.all((got >= bf16_rne(want - delta)) & (got <= bf16_rne(want + delta)))
 
 
