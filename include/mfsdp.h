@@ -313,8 +313,11 @@ int mfsdp_muon_update_pass(const mfsdp_desc_t* desc, size_t n_desc, void* W, voi
                            const mfsdp_muon_hparams_t* hp, void* cuda_stream);
 
 /* The same step with HOST buffers (pinned for overlap; pageable works, serialised by the driver): copies G (and W, M
- * when `upload_state` != 0) to the caller's device staging buffers dW/dG/dM (128-byte aligned), runs the step on
- * `cuda_stream`, copies W and M back and synchronises the stream before returning.  The resident set is cut into up
+ * when `upload_state` == 1) to the caller's device staging buffers dW/dG/dM (128-byte aligned), runs the step on
+ * `cuda_stream`, copies W and M back and synchronises the stream before returning.  upload_state: 1 = W and M travel
+ * both ways every step; 0 = W and M stay in dW / dM between calls (only G goes up), both still come back; 2 = as 0 but
+ * the momentum never leaves the device (hM may be NULL): G up, W down -- the traffic of a deployment that keeps the
+ * optimizer state in HBM.  The resident set is cut into up
  * to 8 groups of consecutive matrices which are pipelined over two internal copy streams and the caller's stream: the
  * upload of group g + 1, the step of group g and the download of group g - 1 overlap (PCIe is full duplex; inside a
  * group W rides in under Newton-Schulz and M goes out right after the momentum pass).  That needs one workspace slice

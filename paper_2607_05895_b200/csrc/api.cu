@@ -462,7 +462,8 @@ extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, voi
   int rc = muon_front(desc, n_desc, workspace, ws_bytes, hp, &full);
   if (rc) return rc;
   if (!full || full->lay.mats.empty()) return MFSDP_OK;
-  if (!hW || !hG || !hM || !dW || !dG || !dM) return MFSDP_EINVAL;
+  if (upload_state < 0 || upload_state > 2) return MFSDP_EINVAL;
+  if (!hW || !hG || (!hM && upload_state != 2) || !dW || !dG || !dM) return MFSDP_EINVAL;
   if (!aligned(dW, 128) || !aligned(dG, 128) || !aligned(dM, 128)) return MFSDP_EINVAL;
   const size_t es = full->lay.mat_dtype == MFSDP_BF16 ? 2 : 4;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -508,9 +509,9 @@ extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, voi
   for (size_t g = 0; g < ng; ++g) {          // in: G, M of the group (momentum pass), then W (update pass only)
     const uint64_t e0 = groups[g].e0, n = groups[g].e1 - groups[g].e0;
     MFSDP_TRY(cudaMemcpyAsync(dGb + e0 * es, hGb + e0 * es, n * es, cudaMemcpyHostToDevice, q.in));
-    if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dMb + e0 * 4, hMb + e0 * 4, n * 4, cudaMemcpyHostToDevice, q.in));
+    if (upload_state == 1) MFSDP_TRY(cudaMemcpyAsync(dMb + e0 * 4, hMb + e0 * 4, n * 4, cudaMemcpyHostToDevice, q.in));
     MFSDP_TRY(cudaEventRecord(q.gm_in[g], q.in));
-    if (upload_state) MFSDP_TRY(cudaMemcpyAsync(dWb + e0 * es, hWb + e0 * es, n * es, cudaMemcpyHostToDevice, q.in));
+    if (upload_state == 1) MFSDP_TRY(cudaMemcpyAsync(dWb + e0 * es, hWb + e0 * es, n * es, cudaMemcpyHostToDevice, q.in));
     MFSDP_TRY(cudaEventRecord(q.w_in[g], q.in));
   }
   for (size_t g = 0; g < ng; ++g) {
@@ -525,8 +526,10 @@ extern "C" int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, voi
     if ((rc = launch_update(pl, dW, *hp, st))) return bail(rc);
     MFSDP_TRY(cudaEventRecord(q.done[g], st));
     // out: M is final after the momentum pass, W after the update
-    MFSDP_TRY(cudaStreamWaitEvent(q.out, q.mom[g], 0));
-    MFSDP_TRY(cudaMemcpyAsync(hMb + e0 * 4, dMb + e0 * 4, n * 4, cudaMemcpyDeviceToHost, q.out));
+    if (upload_state != 2) {                 // 2: the momentum never leaves the device
+      MFSDP_TRY(cudaStreamWaitEvent(q.out, q.mom[g], 0));
+      MFSDP_TRY(cudaMemcpyAsync(hMb + e0 * 4, dMb + e0 * 4, n * 4, cudaMemcpyDeviceToHost, q.out));
+    }
     MFSDP_TRY(cudaStreamWaitEvent(q.out, q.done[g], 0));
     MFSDP_TRY(cudaMemcpyAsync(hWb + e0 * es, dWb + e0 * es, n * es, cudaMemcpyDeviceToHost, q.out));
   }

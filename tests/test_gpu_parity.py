@@ -542,6 +542,13 @@ def test_host_buffer_entry_point(wname, grouped):
         mf.mfsdp_muon_step_host(a.desc, hW, hG, hM, dW, dG, dM, 1 if step < 2 else 0, ws, a.hp)
         a.muon_step()
         assert torch.equal(hW, a.W.cpu()) and torch.equal(hM, a.M.cpu())
+    # fourth step: upload_state = 2 -- the momentum never leaves the device (hM is neither read nor written, may be None)
+    a.load_grads(3)
+    hG = a.hG.clone().pin_memory()
+    hM_before = hM.clone()
+    mf.mfsdp_muon_step_host(a.desc, hW, hG, None, dW, dG, dM, 2, ws, a.hp)
+    a.muon_step()
+    assert torch.equal(hW, a.W.cpu()) and torch.equal(dM, a.M) and torch.equal(hM, hM_before)
 
 
 def test_plan_cache_never_evicts_and_release_plans():
