@@ -344,7 +344,7 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  * single-device matrix optimizer runs there with no gather and no distributed variant.  We verify this by swapping
  * owner-Muon for Shampoo (full L/R preconditioners with inverse fourth root) ... float32".  The
  * paper prints neither formulas nor hyper-parameters; what is computed is Algorithm 1 of Gupta et al. (2018) for
- * matrices under the readings S1-S6 of DESIGN.md section 4.  For every MATRIX descriptor (tails are ignored):
+ * matrices under the readings S1-S7 of DESIGN.md section 4.  For every MATRIX descriptor (tails are ignored):
  *   S1  L <- beta2 L + w G G^T ;  R <- beta2 R + w G^T G ;  w = 1 if beta2 == 1 (running sum) else 1 - beta2
  *   S2  ridge relative to the mean eigenvalue: S~ = S + rho I, rho = eps tr S / d ;  tr S <= 0 -> the preconditioner is I
  *   S7  float32 floor of the ridge: rho = max(eps tr S / d, eps_floor ||S||_F).  The statistic carries rounding noise of
@@ -355,11 +355,12 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  *   S4  D = P_L G P_R ;  W <- W (1 - lr weight_decay) - lr D
  *   S5  the roots are recomputed at steps with (step - 1) % root_every == 0, from statistics that include G_step;
  *       other steps reuse the stored roots
- *   S6  the roots are computed by the coupled Newton iteration  M_0 = z S~, X_0 = z^{1/4} I, z = 5 / (2 (||S||_F + rho)),
- *       T = (5 I - M) / 4, X <- X T, M <- T^4 M  (the first iterations additionally scale M by 2.5 and X by 2.5^(1/4):
- *       every eigenvalue of M is <= 1 after an iteration, so the scaled M stays inside the convergence region and
- *       its small eigenvalues grow 6.1 x instead of 2.44 x per iteration)  until max |M - I| < root_tol, the error stops falling (fp32-class
- *       noise floor) or max_root_iters is reached; X -> S~^{-1/4}.
+ *   S6  the roots are computed by the coupled Newton iteration  M_0 = z S~, X_0 = z^{1/4} I, z = 5 / (2 bound),
+ *       bound = min(||S||_F, 1.6 |S x_8|) + rho (x_8: eight power-iteration steps from a fixed start vector),
+ *       T = (5 I - M) / 4, X <- X T, M <- T^4 M.  The first iterations additionally scale M by 2.5 and X by 2.5^(1/4):
+ *       every eigenvalue of M is <= 1 after an iteration, so the scaled M stays inside the convergence region and its
+ *       small eigenvalues grow 6.1 x instead of 2.44 x per iteration.  It stops at max |M - I| < root_tol, when the error
+ *       no longer falls (fp32-class noise floor) or after max_root_iters; X -> S~^{-1/4}.  11-13 iterations.
  * Arithmetic: every matrix product runs on the bf16 tensor cores with fp32 values carried as three bf16 terms
  * (24 significand bits, fp32 exponent range) and fp32 accumulation -- fp32-class, not bit-identical to an fp32 FFMA loop;
  * the two products of S4 carry their operands to two terms (2^-16-class: the roots are no more accurate than 1e-3).
