@@ -364,7 +364,9 @@ int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, cons
  * Arithmetic: every matrix product runs on the bf16 tensor cores with fp32 values carried as three bf16 terms
  * (24 significand bits, fp32 exponent range) and fp32 accumulation -- fp32-class, not bit-identical to an fp32 FFMA loop;
  * the two products of S4 carry their operands to two terms (2^-16-class: the roots are no more accurate than 1e-3).
- * L and R are fp32; P_L, P_R are kept as three bf16 planes (their sum is the fp32 value).
+ * L and R are fp32; P_L, P_R are kept as three bf16 planes (their sum is the fp32 value).  Dynamic range: G G^T is
+ * accumulated in fp32, so rms(G) must stay within about 1e-17 .. 1e+16 (as for the Muon path); inside it the first step's
+ * D is invariant under power-of-two scalings of G bit for bit (tested).
  *   W, G        DEVICE.  rank-flat matrix parameters (in/out) / gradients (in), 16-byte aligned; dtype of the descriptors.
  *   state       DEVICE in/out.  mfsdp_shampoo_state_bytes, 1024-byte aligned, caller-owned, ZEROED before the first
  *                               step (L_0 = R_0 = 0); layout per matrix: mfsdp_shampoo_view.

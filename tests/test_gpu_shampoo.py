@@ -374,3 +374,28 @@ def test_shampoo_poisoned_workspace_and_guard_bands():
         outs.append((s.W.clone(), s.state.clone()))
     assert torch.equal(outs[0][0].view(torch.int16), outs[1][0].view(torch.int16))
     assert torch.equal(outs[0][1], outs[1][1])
+
+
+def test_shampoo_first_step_is_scale_invariant():
+    """D = P_L G P_R of the first step does not depend on the scale of G (the statistics scale with its square, the
+    roots with its inverse square root: oracle pin test_scale_invariance_of_first_step).  For power-of-two scalings the
+    GPU path is invariant BIT FOR BIT: every quantity it forms is an exact power-of-two multiple of the unscaled one
+    (statistics, trace, Frobenius norm, ridge, z, the three-term planes), until fp32 under- / overflows -- the supported
+    range is rms(G) ~ 1e-17 .. 1e+16 as for the Muon path (reading D1)."""
+    base = None
+    for e in (0, 24, -24, 40):
+        s = ShampooSession(workloads.small_ragged(), lr=0.0, weight_decay=0.0)
+        hG = workloads.fill_flat(s.wl, s.descs, workloads.KIND_G, step=1)
+        s.hG = (hG.float() * (2.0 ** e)).to(hG.dtype)
+        assert torch.equal((s.hG.float() * (2.0 ** -e)).to(hG.dtype), hG), "the scaling itself must be exact"
+        s.G = s.hG.cuda()
+        mf.mfsdp_shampoo_step(s.desc, s.W, s.G, s.state, s.ws, mf.ShampooHParams(step=1, flags=s.flags, **s.hp_kw))
+        torch.cuda.synchronize()
+        Ds = [s.read_all(i)[4] for i in range(len(s.mats))]
+        iters = [tuple(c["iters"] for c in s.read_all(i)[5]) for i in range(len(s.mats))]
+        if base is None:
+            base = (Ds, iters)
+        else:
+            assert iters == base[1]
+            for D, D0 in zip(Ds, base[0]):
+                assert np.array_equal(D, D0), "2^%d" % e
