@@ -114,7 +114,6 @@ __global__ void __launch_bounds__(256) k_sh_power(const RootInfo* roots, double*
   const RootInfo ri = roots[blockIdx.y];
   const float* xin = ri.vec + (it & 1u) * ri.pitch;
   float* yout = ri.vec + ((it + 1u) & 1u) * ri.pitch;
-  __shared__ float red[8];
   __shared__ float scale_sh;
   if (threadIdx.x == 0) {
     double n2 = 0.0;
@@ -124,27 +123,36 @@ __global__ void __launch_bounds__(256) k_sh_power(const RootInfo* roots, double*
   }
   __syncthreads();
   const float sc = scale_sh;
+  // one warp per row (8 rows in flight per block), float4 loads, shuffle reduction; fixed orders throughout
+  const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
   double acc2 = 0.0;
-  for (uint32_t r = blockIdx.x; r < ri.d; r += gridDim.x) {
+  for (uint32_t r = blockIdx.x * 8u + warp; r < ri.d; r += gridDim.x * 8u) {
     const float* row = ri.S + (size_t)r * ri.pitch;
     float sum = 0.f;
-    for (uint32_t c = threadIdx.x; c < ri.d; c += blockDim.x) {
-      const float x = it > 0 ? xin[c] * sc : (float)((c * 2654435761u + 0x9e3779b9u) >> 16 & 0xffffu) * (1.f / 32768.f) - 1.f;
-      sum = fmaf(row[c], x, sum);
+    for (uint32_t c = 4u * lane; c < ri.d; c += 128u) {          // pitch is a multiple of 64: a float4 never leaves the row
+      const float4 a = *reinterpret_cast<const float4*>(row + c);
+      const float av[4] = {a.x, a.y, a.z, a.w};
+#pragma unroll
+      for (uint32_t k = 0; k < 4; ++k) {
+        const uint32_t cc = c + k;
+        if (cc < ri.d) {
+          const float x = it > 0 ? xin[cc] * sc : (float)((cc * 2654435761u + 0x9e3779b9u) >> 16 & 0xffffu) * (1.f / 32768.f) - 1.f;
+          sum = fmaf(av[k], x, sum);
+        }
+      }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-    if ((threadIdx.x & 31u) == 0) red[threadIdx.x >> 5] = sum;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      float y = 0.f;
-      for (int w = 0; w < 8; ++w) y += red[w];
-      yout[r] = y;
-      acc2 += (double)y * (double)y;
-    }
-    __syncthreads();
+    if (lane == 0) { yout[r] = sum; acc2 += (double)sum * (double)sum; }
   }
-  if (threadIdx.x == 0) partials[((size_t)ri.ctl * kRedBlocks + blockIdx.x) * kPartWords + 2 + (it & 1u)] = acc2;
+  __shared__ double red2[8];
+  if (lane == 0) red2[warp] = acc2;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int w = 0; w < 8; ++w) t += red2[w];
+    partials[((size_t)ri.ctl * kRedBlocks + blockIdx.x) * kPartWords + 2 + (it & 1u)] = t;
+  }
 }
 
 __global__ void k_sh_root_init(const RootInfo* roots, uint32_t n, ShCtl* ctl, const double* partials, double eps,
@@ -197,25 +205,21 @@ __global__ void __launch_bounds__(256) k_sh_root_prep(const RootInfo* roots, con
   const ShCtl c = ctl[ri.ctl];
   for (uint32_t r = blockIdx.x; r < ri.d; r += gridDim.x) {
     const float* row = ri.S + (size_t)r * ri.pitch;
-    for (uint32_t col = threadIdx.x; col < ri.pitch; col += blockDim.x) {   // the pitch padding is written too (zeros)
-      const float diag = col == r ? 1.f : 0.f;
-      const float m = col >= ri.d ? 0.f : c.identity ? diag : c.z * (row[col] + c.rho * diag);
-      const float t = 0.25f * (5.f * diag - m);
-      const float x = c.x0 * diag;
+    for (uint32_t col = 8u * threadIdx.x; col < ri.pitch; col += 8u * blockDim.x) {   // 8 columns per thread; the pitch
+      float m[8], t[8], x[8];                                                          // padding is written too (zeros)
+      const float4 a = *reinterpret_cast<const float4*>(row + col), b = *reinterpret_cast<const float4*>(row + col + 4);
+      const float sv[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const float diag = col + k == r ? 1.f : 0.f;
+        m[k] = col + k >= ri.d ? 0.f : c.identity ? diag : c.z * (sv[k] + c.rho * diag);
+        t[k] = 0.25f * (5.f * diag - m[k]);
+        x[k] = c.x0 * diag;
+      }
       const size_t o = (size_t)r * ri.pitch + col;
-      uint32_t b1, b2, b3;
-      sg::split3(m, b1, b2, b3);
-      ri.M0[o] = __ushort_as_bfloat16((unsigned short)b1);
-      ri.M0[o + ri.plane] = __ushort_as_bfloat16((unsigned short)b2);
-      ri.M0[o + 2 * ri.plane] = __ushort_as_bfloat16((unsigned short)b3);
-      sg::split3(t, b1, b2, b3);
-      ri.T[o] = __ushort_as_bfloat16((unsigned short)b1);
-      ri.T[o + ri.plane] = __ushort_as_bfloat16((unsigned short)b2);
-      ri.T[o + 2 * ri.plane] = __ushort_as_bfloat16((unsigned short)b3);
-      sg::split3(x, b1, b2, b3);
-      ri.X[0][o] = __ushort_as_bfloat16((unsigned short)b1);
-      ri.X[0][o + ri.plane] = __ushort_as_bfloat16((unsigned short)b2);
-      ri.X[0][o + 2 * ri.plane] = __ushort_as_bfloat16((unsigned short)b3);
+      sg::store_split8(ri.M0 + o, ri.plane, m);
+      sg::store_split8(ri.T + o, ri.plane, t);
+      sg::store_split8(ri.X[0] + o, ri.plane, x);
     }
   }
 }
@@ -254,10 +258,23 @@ __global__ void __launch_bounds__(256) k_sh_root_finish(const RootInfo* roots, c
     }
     return;
   }
-  const __nv_bfloat16* src = ri.X[c.iters & 1u];
-  const __nv_bfloat16 zero = __ushort_as_bfloat16((unsigned short)0);
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < 3 * ri.plane; i += (size_t)gridDim.x * blockDim.x)
-    ri.P[i] = (uint32_t)(i % ri.pitch) < ri.d ? src[i] : zero;              // the pitch padding of the state is zero
+  const uint4* src = reinterpret_cast<const uint4*>(ri.X[c.iters & 1u]);
+  uint4* dst = reinterpret_cast<uint4*>(ri.P);
+  const size_t n8 = 3 * ri.plane / 8;                             // planes are rows x pitch, pitch a multiple of 64
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+    const uint32_t col = (uint32_t)((i * 8) % ri.pitch);
+    uint4 v = src[i];
+    if (col + 8u > ri.d) {                                        // the pitch padding of the state is zero
+      uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (uint32_t k = 0; k < 4; ++k) {
+        if (col + 2 * k >= ri.d) w[k] = 0u;
+        else if (col + 2 * k + 1 >= ri.d) w[k] &= 0xffffu;
+      }
+      v = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+    dst[i] = v;
+  }
 }
 
 // ---- host: tensor maps ------------------------------------------------------------------------------------------
