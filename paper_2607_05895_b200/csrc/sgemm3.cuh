@@ -30,7 +30,10 @@
 // Epilogue (all optional, per problem): v = alpha acc + beta Cin;  fp32 store;  three-term split store;  the split of
 // T = (5 I - v) / 4 (the next coupled-Newton step matrix);  max |v - I| into an error word;  the weight update
 // W <- decay W - lr v.  Symmetric problems compute only the tiles on and above the block diagonal and store the
-// mirror image as well.
+// mirror image as well; their three-plane outputs leave through asynchronous TMA stores of 32 x 32 blocks staged in
+// shared memory (sg_store_block).  Two kernels share all of this: k_sgemm3 (single CTA, 128 x 128 tiles, below) and
+// k_sgemm3p (CTA pair, 256 x 256 tiles, further down), chosen per launch by the host; instances <3, 3> (root
+// iteration), <2, 2> / <2, 1> (preconditioning products on two-term operands), <1, 1> (statistics of a bf16 gradient).
 #ifndef MFSDP_SGEMM3_CUH_
 #define MFSDP_SGEMM3_CUH_
 

@@ -1,11 +1,12 @@
 // Owner-local Shampoo on the descriptor table of the Muon step ("swapping owner-Muon for Shampoo (full
-// L/R preconditioners with inverse fourth root)"; readings S1-S6 of DESIGN.md section 4).
+// L/R preconditioners with inverse fourth root)"; readings S1-S7 of DESIGN.md section 4).
 //
 // Per resident matrix G (rows x cols), statistics L (rows x rows), R (cols x cols) in fp32:
 //   S1  L <- beta2 L + w G G^T ; R <- beta2 R + w G^T G                       one grouped GEMM launch (k_sgemm3)
-//   S2  A = S + eps (tr S / d) I                                              k_sh_reduce, k_sh_root_init
+//   S2  A = S + rho I, rho = max(eps tr S / d, eps_floor ||S||_F) (S7)         k_sh_reduce, k_sh_power, k_sh_root_init
 //   S3  P = A^{-1/4}  by the coupled Newton iteration (reading S6):           3 grouped GEMM launches + k_sh_root_ctl
-//         M_0 = z A, X_0 = z^{1/4} I, z = 5 / (2 (||S||_F + rho));           per iteration, for every L and R of the
+//         M_0 = z A, X_0 = z^{1/4} I, z = 5 / (2 bound), bound from ||S||_F and   per iteration, for every L and R of the
+//         eight power-iteration steps;
 //         T = (5 I - M) / 4 ; X <- X T ; M <- T^4 M ; stop at max |M - I| < tol  group at once; the first iterations
 //         also scale M by 2.5 and X by 2.5^(1/4) (k_sh_root_init: 6.1 x instead of 2.44 x growth of small eigenvalues)
 //   S4  D = P_L G P_R ; W <- W (1 - lr wd) - lr D                             two grouped GEMM launches, update fused
