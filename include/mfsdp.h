@@ -61,7 +61,8 @@ enum { MFSDP_STEP_KEEP_O = 1u };                              /* mfsdp_muon_hpar
 enum { MFSDP_SEG_ALIGN = 64 };                                /* every segment starts on a 64-element boundary    */
 
 enum { MFSDP_OK = 0, MFSDP_EINVAL = -1, MFSDP_ECAP = -2, MFSDP_ELAYOUT = -3, MFSDP_EARCH = -4, MFSDP_ECUDA = -5,
-       MFSDP_ECACHE = -6 };                                   /* launch-table cache full, see mfsdp_release_plans  */
+       MFSDP_ECACHE = -6,                                     /* launch-table cache full, see mfsdp_release_plans  */
+       MFSDP_ETOOBIG = -7 };                                  /* matrix beyond the fixed scratch of mfsdp_momentum_pass_static */
 
 /* ---- records ------------------------------------------------------------------------------------------------ */
 /* One model parameter, in model order (planner input). */
@@ -335,6 +336,43 @@ int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, cons
  *   p <- p - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps).
  *   P, G   DEVICE. rank-flat tail parameters / gradients, dtype of the descriptors (one dtype for all tails).
  *   m, v   DEVICE. rank-flat first / second moments, always float, same element offsets.
+/* ---- momentum pass of one matrix for callers that may not allocate (DEVICE work, HOST call) ----------------------
+ * Every step call above builds device-side launch tables with cudaMalloc the first time it sees a (table, workspace)
+ * pair and needs a caller-allocated workspace.  Some callers of an owner-local optimizer can do neither: a trainer
+ * whose framework allocator has already claimed the GPU up to its planned budget (a raw cudaMalloc may fail or break a
+ * memory limit the job runs under); code inside the step loop while the gradient reduction of PAPER.md:83 is still in
+ * flight on another stream (cudaMalloc / cudaFree synchronise the whole device and would stall that overlap); a hook
+ * of a host library that forbids CUDA memory management.  For them this call runs SURVEY.md 8(a) a1 and the scalar
+ * part of a2 on ONE matrix with no allocation, no host-to-device copy and no cached table:
+ *   M <- mu M + (1-mu) G ; U = (1-mu) G + mu M (hp->nesterov != 0) or M ; X = cast(U) ;
+ *   *ssq = ||U||_F^2 ; *inv_norm = 1 / max(||U||_F, hp->eps).
+ * The one piece of scratch the pass needs (a double per 16384-element chunk, between the streaming kernel and the
+ * fixed-order reduction) lives in a fixed array inside the library's device image.
+ *   rows, cols   the matrix, row-major and contiguous (G, M and X all have row pitch = cols); rows * cols must not
+ *                exceed mfsdp_static_max_elems() = 2^30, else MFSDP_ETOOBIG is returned and nothing is launched.
+ *   dtype        MFSDP_BF16 | MFSDP_F32: element type of G.
+ *   precision    MFSDP_NS_BF16 -> X is bf16, MFSDP_NS_FP32 -> X is float.
+ *   G            DEVICE in.   rows * cols elements, 16-byte aligned.
+ *   M            DEVICE i/o.  rows * cols floats, 16-byte aligned, updated in place.
+ *   X            DEVICE out.  rows * cols elements of bf16 / float, 16-byte aligned.
+ *   ssq          DEVICE out.  one double (8-byte aligned).
+ *   inv_norm     DEVICE out.  one float.
+ *   hp           HOST in.     only momentum, nesterov and eps are read.
+ * What to know before relying on it:
+ *   - the array is 512 KiB and every GPU that loads libmfsdp holds it until the process exits, used or not;
+ *   - the FIRST call on each device does the set-up (looks up the array's device address with that device current and
+ *     makes the runtime load the library's device code); make that call before any stream capture starts.  Later
+ *     calls only enqueue two kernels on cuda_stream and return without synchronising;
+ *   - all calls on a device share the array, and it keeps the previous call's contents.  Nothing in it has to start at
+ *     zero (each call writes every partial it reads), so calls ordered on one stream, or by events, are safe back to
+ *     back; two calls that may run at the same time on one GPU overwrite each other's partials and race;
+ *   - M, X and ||U||^2 are bit-identical to mfsdp_muon_momentum_pass on a table holding the same matrix.
+ * Returns MFSDP_EINVAL (null / misaligned pointer, zero dimension, bad dtype / precision / momentum / eps),
+ * MFSDP_ETOOBIG, MFSDP_EARCH, MFSDP_ECUDA. */
+uint64_t mfsdp_static_max_elems(void);
+int mfsdp_momentum_pass_static(uint32_t rows, uint32_t cols, int dtype, int precision, const void* G, void* M, void* X,
+                               double* ssq, float* inv_norm, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
+
  * Returns as mfsdp_muon_step (hp->step < 1 is MFSDP_EINVAL). */
 int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, const void* G, void* m, void* v,
                           const mfsdp_adamw_hparams_t* hp, void* cuda_stream);

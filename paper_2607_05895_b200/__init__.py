@@ -8,7 +8,7 @@ MfsdpError(MFSDP_EARCH).
 from .binding import (  # noqa: F401
     BF16, F32, ROLE_MATRIX, ROLE_TAIL, POLICY_ROLE_GREEDY, POLICY_SCOPE_GREEDY, POLICY_COST_AWARE, METRIC_NUMEL, METRIC_NS_FLOPS,
     SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE, NS_BF16, NS_FP32, STEP_KEEP_O,
-    EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE,
+    EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE, ETOOBIG,
     MfsdpError, Param, Desc, MuonHParams, AdamWHParams, PlanResult,
     lib_path, load, exported_symbols,
     mfsdp_plan, mfsdp_plan_ex, mfsdp_score_plan, mfsdp_reduce_schedule, mfsdp_muon_step_gated, mfsdp_signal_ready, mfsdp_muon_step_fanout,
@@ -17,5 +17,5 @@ from .binding import (  # noqa: F401
     mfsdp_muon_step_host, mfsdp_adamw_tail_step, mfsdp_strerror, mfsdp_version, mfsdp_launch_count,
     mfsdp_tune, mfsdp_get_tune, mfsdp_debug_trace, TUNE_PAIR_MIN_D, TUNE_SYM_BAND, TUNE_SYM_BAND2, TUNE_RECT_GROUP, TUNE_WIDE_MIN_KB, TUNE_FUSED_BELOW_D, TUNE_FUSED2_BELOW_D, mfsdp_release_plans, mfsdp_ns_class,
     make_desc_array, SHAMPOO_KEEP_D, ShampooHParams, mfsdp_shampoo_state_bytes, mfsdp_shampoo_workspace_bytes,
-    mfsdp_shampoo_view, mfsdp_shampoo_step,
+    mfsdp_shampoo_view, mfsdp_shampoo_step, mfsdp_momentum_pass_static, mfsdp_static_max_elems,
 )

@@ -13,7 +13,7 @@ SCALE_MATCH_RMS_ADAMW, SCALE_ORIGINAL, SCALE_NONE = 0, 1, 2
 NS_BF16, NS_FP32 = 0, 1
 STEP_KEEP_O = 1
 SHAMPOO_KEEP_D = 1
-OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, ECAP, ELAYOUT, EARCH, ECUDA, ECACHE, ETOOBIG = 0, -1, -2, -3, -4, -5, -6, -7
 
 
 class Param(C.Structure):            # mfsdp_param_t
@@ -107,7 +107,7 @@ _SYMBOLS = ["mfsdp_plan", "mfsdp_plan_ex", "mfsdp_score_plan", "mfsdp_reduce_sch
             "mfsdp_muon_update_pass", "mfsdp_muon_step_host", "mfsdp_host_workspace_bytes", "mfsdp_adamw_tail_step", "mfsdp_debug_ws_offsets",
             "mfsdp_strerror", "mfsdp_version", "mfsdp_launch_count", "mfsdp_tune", "mfsdp_get_tune", "mfsdp_debug_trace",
             "mfsdp_release_plans", "mfsdp_ns_class", "mfsdp_shampoo_state_bytes", "mfsdp_shampoo_workspace_bytes",
-            "mfsdp_shampoo_step", "mfsdp_shampoo_view"]
+            "mfsdp_shampoo_step", "mfsdp_shampoo_view", "mfsdp_momentum_pass_static", "mfsdp_static_max_elems"]
 _lib = None
 
 
@@ -156,6 +156,8 @@ def load():
     lib.mfsdp_muon_update_pass.argtypes = [pD, sz, vp, vp, sz, pMH, vp]
     lib.mfsdp_muon_step_host.argtypes = [pD, sz, vp, vp, vp, vp, vp, vp, i32, vp, sz, pMH, vp]
     lib.mfsdp_adamw_tail_step.argtypes = [pD, sz, vp, vp, vp, vp, pAH, vp]
+    lib.mfsdp_momentum_pass_static.argtypes = [C.c_uint32, C.c_uint32, i32, i32, vp, vp, vp, vp, vp, pMH, vp]
+    lib.mfsdp_static_max_elems.restype = C.c_uint64
     lib.mfsdp_strerror.argtypes = [i32]
     lib.mfsdp_strerror.restype = C.c_char_p
     lib.mfsdp_version.restype = i32
@@ -420,6 +422,23 @@ def mfsdp_muon_momentum_pass(desc, G, M, workspace, hp, stream=None):
     arr, n = _dn(desc)
     _check(load().mfsdp_muon_momentum_pass(arr, n, _ptr(G), _ptr(M), _ptr(workspace), _nbytes(workspace),
                                            C.byref(hp), _stream(stream)), "mfsdp_muon_momentum_pass")
+
+
+def mfsdp_static_max_elems():
+    """Largest rows * cols mfsdp_momentum_pass_static accepts (the size of its built-in scratch array)."""
+    return int(load().mfsdp_static_max_elems())
+
+
+def mfsdp_momentum_pass_static(rows, cols, dtype, precision, G, M, X, ssq, inv_norm, hp, stream=None):
+    """Momentum pass of one contiguous rows x cols matrix that allocates nothing on the device: for callers that cannot
+    call cudaMalloc (a framework allocator owns the GPU, or the device-wide synchronisation of an allocation is not
+    acceptable inside the step loop).  G: gradient (dtype), M: float momentum (in place), X: cast(U) out (bf16 for
+    NS_BF16, float for NS_FP32), ssq: one float64, inv_norm: one float32 -- all CUDA tensors or addresses the caller
+    owns.  Shares a fixed 512 KiB scratch array per GPU with every other call: do not let two calls overlap on one
+    GPU.  Raises MfsdpError(ETOOBIG) beyond mfsdp_static_max_elems() elements.  See include/mfsdp.h."""
+    _check(load().mfsdp_momentum_pass_static(int(rows), int(cols), int(dtype), int(precision), _ptr(G), _ptr(M),
+                                             _ptr(X), _ptr(ssq), _ptr(inv_norm), C.byref(hp), _stream(stream)),
+           "mfsdp_momentum_pass_static")
 
 
 def mfsdp_muon_ns_pass(desc, workspace, hp, stream=None):

@@ -15,7 +15,8 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libmfsdp.so")
-SOURCES = ["planner.cpp", "api.cu", "elementwise.cu", "ns_fp32.cu", "ns_tc.cu", "ns_fused.cu", "ns_fused2.cu", "shampoo.cu"]
+SOURCES = ["planner.cpp", "api.cu", "elementwise.cu", "ns_fp32.cu", "ns_tc.cu", "ns_fused.cu", "ns_fused2.cu", "shampoo.cu",
+           "static_scratch.cu"]
 HEADERS = [os.path.join(ROOT, "include", "mfsdp.h"), os.path.join(CSRC, "mfsdp_internal.h"),
            os.path.join(CSRC, "ptx_sm100.cuh"), os.path.join(CSRC, "ns_plan.h"), os.path.join(CSRC, "sgemm3.cuh")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

@@ -612,6 +612,8 @@ extern "C" const char* mfsdp_strerror(int code) {
     case MFSDP_ECUDA: return g_cuda_err.c_str();
     case MFSDP_ECACHE: return "launch-table cache full (1024 distinct (table, workspace, precision) keys): keep the "
                               "workspace pointer stable, or call mfsdp_release_plans()";
+    case MFSDP_ETOOBIG: return "matrix larger than the fixed scratch array of mfsdp_momentum_pass_static "
+                               "(mfsdp_static_max_elems() = 2^30 elements); use mfsdp_muon_momentum_pass with a workspace";
     default: return "unknown error code";
   }
 }
