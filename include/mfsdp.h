@@ -271,6 +271,9 @@ int mfsdp_muon_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void
  *                       ready[i] >= epoch (acquire at system scope, so that writes of a copy engine, a peer GPU or
  *                       the host made before the flag write are visible); G is read through L2 only.
  *   epoch               the value the producer writes for this step (e.g. the step number; flags never need a reset).
+ * The matrices are taken in the order their flags go up, whatever the table order: each waiting thread block sweeps the
+ * matrices it has chunks of and works on those that have landed (with the reverse-block order of mfsdp_reduce_schedule
+ * the last matrices of the table land first).  The order changes no value.
  * The producer -- the reduction's completion, or a host-to-device copy -- raises flag i with
  * mfsdp_signal_ready(ready, i, epoch, producer_stream) AFTER the work that fills matrix i's gradient, on the stream
  * that does that work.  The producer's work must not depend on SM resources that the waiting kernel occupies: enqueue

@@ -1,5 +1,6 @@
 // HBM-bound passes of the owner-local step, one grid over all resident segments.
 //   k_momentum  M <- mu M + (1-mu) G ; U = (1-mu) G + mu M | M ; X~ = cast(U) ; partial sums of U^2
+//               (k_momentum_gated: the same per chunk, matrices taken in the order their gradients land)
 //   k_ssq       fixed-order reduction of the partials -> ||U||_F^2 (double), 1 / max(||U||_F, eps) (float)
 //   k_update    W <- W (1 - lr wd) - lr s(rows, cols) O
 //   k_adamw     decoupled-decay Adam on the packed tails
@@ -137,97 +138,171 @@ __device__ __forceinline__ double block_sum(double x, double* smem) {
 }
 
 // ---- a1: momentum + Nesterov + cast + partial squared norm ---------------------------------------------------------
-// kGated: the chunks of matrix i wait until ready[i] >= epoch (mfsdp_muon_step_gated), and G is read through L2.
-template <typename GT, typename XT, bool kGated>
+// One chunk.  kL2: G is read through L2 only (gated pass: the gradient is written by another agent while the kernel runs).
+template <typename GT, typename XT, bool kL2>
+__device__ __forceinline__ void momentum_chunk(const MatLayout* __restrict__ mats, uint32_t mi, uint32_t c,
+                                               const GT* __restrict__ G, float* __restrict__ M,
+                                               uint8_t* __restrict__ ws, double* __restrict__ partial, float mu,
+                                               float omm, int nesterov, double* red) {
+  const MatLayout L = mats[mi];
+  const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
+  const GT* g = G + L.elem_off;
+  float* m = M + L.elem_off;
+  XT* x = reinterpret_cast<XT*>(ws + L.x_off[0]);
+  const bool vec = (L.cols % 8u) == 0u;      // then pitch_x == cols and a vector never straddles a row
+  double acc = 0.0;
+  if (vec && base + kChunk <= L.numel) {     // full chunk: batched 128-bit accesses
+#pragma unroll
+    for (int b = 0; b < kVecPerThread / kBatch; ++b) {
+      F8 gv[kBatch], mv[kBatch];
+#pragma unroll
+      for (int v = 0; v < kBatch; ++v) {
+        const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
+        gv[v] = kL2 ? load8_cg(g + e0) : load8_ro(g + e0);
+        mv[v] = load8_cs(m + e0);
+      }
+#pragma unroll
+      for (int v = 0; v < kBatch; ++v) {
+        const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
+        F8 uv;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float gs = omm * gv[v].v[i];
+          mv[v].v[i] = fmaf(mu, mv[v].v[i], gs);                       // M <- mu M + (1-mu) G
+          uv.v[i] = nesterov ? fmaf(mu, mv[v].v[i], gs) : mv[v].v[i];  // U = (1-mu) G + mu M   |   U = M
+          acc = fma((double)uv.v[i], (double)uv.v[i], acc);
+        }
+        store8_cs(m + e0, mv[v]);        // M is touched once per step: evict-first
+        store8(x + e0, uv);              // X~ is the next kernel's input: keep it in L2 (small sets fit)
+      }
+    }
+  } else {                                   // ragged chunk or odd pitch: same element -> thread mapping, guarded
+    for (int it = 0; it < kVecPerThread; ++it) {
+      const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
+      if (e0 >= L.numel) break;
+      if (vec && e0 + 8 <= L.numel) {
+        const F8 gv = kL2 ? load8_cg(g + e0) : load8_ro(g + e0);
+        F8 mv = load8(m + e0);
+        F8 uv;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float gs = omm * gv.v[i];
+          mv.v[i] = fmaf(mu, mv.v[i], gs);
+          uv.v[i] = nesterov ? fmaf(mu, mv.v[i], gs) : mv.v[i];
+          acc = fma((double)uv.v[i], (double)uv.v[i], acc);
+        }
+        store8(m + e0, mv);
+        store8(x + e0, uv);
+      } else {
+        const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
+        for (uint64_t e = e0; e < e1; ++e) {
+          const float gs = omm * (kL2 ? load1_cg(g + e) : load1(g + e));
+          const float mn = fmaf(mu, m[e], gs);
+          const float u = nesterov ? fmaf(mu, mn, gs) : mn;
+          acc = fma((double)u, (double)u, acc);
+          m[e] = mn;
+          const uint64_t r = e / L.cols, col = e - r * L.cols;
+          store1(x + r * L.pitch_x + col, u);
+        }
+      }
+    }
+  }
+  const double s = block_sum(acc, red);
+  if (threadIdx.x == 0) partial[c] = s;
+}
+
+template <typename GT, typename XT>
 __global__ void __launch_bounds__(kEwThreads) k_momentum(const MatLayout* __restrict__ mats,
                                                          const uint32_t* __restrict__ chunk_mat, uint32_t n_chunks,
                                                          const GT* __restrict__ G, float* __restrict__ M,
                                                          uint8_t* __restrict__ ws, double* __restrict__ partial,
-                                                         float mu, float omm, int nesterov,
-                                                         const uint32_t* __restrict__ ready, uint32_t epoch) {
+                                                         float mu, float omm, int nesterov) {
   __shared__ double red[kEwThreads / 32];
-  for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
-    if constexpr (kGated) {
-      if (threadIdx.x == 0) {
-        const uint32_t* flag = ready + chunk_mat[c];
-        uint32_t v;
-        asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
-        if ((int32_t)(v - epoch) < 0) {
-          const long long t0 = clock64();
-          do {
-            __nanosleep(200);
-            if (clock64() - t0 > 20000000000ll) __trap();       // ~10 s: the producer never signalled
-            asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
-          } while ((int32_t)(v - epoch) < 0);
-        }
+  for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x)
+    momentum_chunk<GT, XT, false>(mats, chunk_mat[c], c, G, M, ws, partial, mu, omm, nesterov, red);
+}
+
+// Gated form (mfsdp_muon_step_gated): the chunks of matrix i may be touched once ready[i] >= epoch.  A CTA owns the
+// chunks c = blockIdx.x + k gridDim.x; consecutive ones of one matrix form a RUN.  The CTA lists its runs once, then
+// sweeps the list: a run whose flag is up is processed and dropped, the others stay for the next sweep.  So the order
+// in which the gradients land does not matter -- with the reduction's reverse block order (mfsdp_reduce_schedule) the
+// LAST matrices of the table arrive first, and a CTA that waited for its first chunk's matrix would idle until the very
+// last gradient.  Which run is processed when changes no value: every chunk's partial sum is written by the one CTA
+// that owns it, in a fixed order.  More than kGateRuns runs per CTA (a table of thousands of tiny matrices): that CTA
+// falls back to waiting in table order.
+constexpr uint32_t kGateRuns = 2048;
+
+__device__ __forceinline__ bool flag_up(const uint32_t* flag, uint32_t epoch) {
+  uint32_t v;
+  asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+  return (int32_t)(v - epoch) >= 0;
+}
+
+template <typename GT, typename XT>
+__global__ void __launch_bounds__(kEwThreads) k_momentum_gated(const MatLayout* __restrict__ mats,
+                                                               const uint32_t* __restrict__ chunk_mat,
+                                                               const uint32_t* __restrict__ chunk_begin,
+                                                               uint32_t n_chunks, const GT* __restrict__ G,
+                                                               float* __restrict__ M, uint8_t* __restrict__ ws,
+                                                               double* __restrict__ partial, float mu, float omm,
+                                                               int nesterov, const uint32_t* __restrict__ ready,
+                                                               uint32_t epoch) {
+  __shared__ double red[kEwThreads / 32];
+  __shared__ uint32_t run_first[kGateRuns];      // first chunk of each pending run
+  __shared__ uint32_t n_runs_s;
+  if (threadIdx.x == 0) n_runs_s = 0;
+  __syncthreads();
+  const uint32_t mine = blockIdx.x < n_chunks ? (n_chunks - blockIdx.x + gridDim.x - 1) / gridDim.x : 0u;
+  for (uint32_t k = threadIdx.x; k < mine; k += kEwThreads) {
+    const uint32_t c = blockIdx.x + k * gridDim.x;
+    if (k == 0 || chunk_mat[c] != chunk_mat[c - gridDim.x]) {
+      const uint32_t slot = atomicAdd(&n_runs_s, 1u);
+      if (slot < kGateRuns) run_first[slot] = c;
+    }
+  }
+  __syncthreads();
+  uint32_t n_runs = n_runs_s;
+  if (n_runs > kGateRuns) {                      // too many runs to list: wait in table order
+    for (uint32_t c = blockIdx.x; c < n_chunks; c += gridDim.x) {
+      const uint32_t mi = chunk_mat[c];
+      if (threadIdx.x == 0 && !flag_up(ready + mi, epoch)) {
+        const long long t0 = clock64();
+        do {
+          __nanosleep(200);
+          if (clock64() - t0 > 20000000000ll) __trap();       // ~10 s: the producer never signalled
+        } while (!flag_up(ready + mi, epoch));
       }
       __syncthreads();
+      momentum_chunk<GT, XT, true>(mats, mi, c, G, M, ws, partial, mu, omm, nesterov, red);
     }
-    const MatLayout L = mats[chunk_mat[c]];
-    const uint64_t base = (uint64_t)(c - L.chunk_begin) * kChunk;
-    const GT* g = G + L.elem_off;
-    float* m = M + L.elem_off;
-    XT* x = reinterpret_cast<XT*>(ws + L.x_off[0]);
-    const bool vec = (L.cols % 8u) == 0u;      // then pitch_x == cols and a vector never straddles a row
-    double acc = 0.0;
-    if (vec && base + kChunk <= L.numel) {     // full chunk: batched 128-bit accesses
-#pragma unroll
-      for (int b = 0; b < kVecPerThread / kBatch; ++b) {
-        F8 gv[kBatch], mv[kBatch];
-#pragma unroll
-        for (int v = 0; v < kBatch; ++v) {
-          const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
-          gv[v] = kGated ? load8_cg(g + e0) : load8_ro(g + e0);
-          mv[v] = load8_cs(m + e0);
-        }
-#pragma unroll
-        for (int v = 0; v < kBatch; ++v) {
-          const uint64_t e0 = base + ((uint64_t)(b * kBatch + v) * kEwThreads + threadIdx.x) * 8;
-          F8 uv;
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const float gs = omm * gv[v].v[i];
-            mv[v].v[i] = fmaf(mu, mv[v].v[i], gs);                       // M <- mu M + (1-mu) G
-            uv.v[i] = nesterov ? fmaf(mu, mv[v].v[i], gs) : mv[v].v[i];  // U = (1-mu) G + mu M   |   U = M
-            acc = fma((double)uv.v[i], (double)uv.v[i], acc);
-          }
-          store8_cs(m + e0, mv[v]);        // M is touched once per step: evict-first
-          store8(x + e0, uv);              // X~ is the next kernel's input: keep it in L2 (small sets fit)
-        }
+    return;
+  }
+  long long idle_since = 0;
+  bool idle = false;
+  while (n_runs) {
+    uint32_t kept = 0;
+    for (uint32_t j = 0; j < n_runs; ++j) {
+      const uint32_t c0 = run_first[j];
+      const uint32_t mi = chunk_mat[c0];
+      const int up = __syncthreads_or(threadIdx.x == 0 ? (int)flag_up(ready + mi, epoch) : 0);
+      if (!up) {                                 // every thread has read run_first[j] (barrier above); kept <= j
+        if (threadIdx.x == 0) run_first[kept] = c0;
+        ++kept;
+        continue;
       }
-    } else {                                   // ragged chunk or odd pitch: same element -> thread mapping, guarded
-      for (int it = 0; it < kVecPerThread; ++it) {
-        const uint64_t e0 = base + ((uint64_t)it * kEwThreads + threadIdx.x) * 8;
-        if (e0 >= L.numel) break;
-        if (vec && e0 + 8 <= L.numel) {
-          const F8 gv = kGated ? load8_cg(g + e0) : load8_ro(g + e0);
-          F8 mv = load8(m + e0);
-          F8 uv;
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const float gs = omm * gv.v[i];
-            mv.v[i] = fmaf(mu, mv.v[i], gs);
-            uv.v[i] = nesterov ? fmaf(mu, mv.v[i], gs) : mv.v[i];
-            acc = fma((double)uv.v[i], (double)uv.v[i], acc);
-          }
-          store8(m + e0, mv);
-          store8(x + e0, uv);
-        } else {
-          const uint64_t e1 = (e0 + 8 < L.numel) ? e0 + 8 : L.numel;
-          for (uint64_t e = e0; e < e1; ++e) {
-            const float gs = omm * (kGated ? load1_cg(g + e) : load1(g + e));
-            const float mn = fmaf(mu, m[e], gs);
-            const float u = nesterov ? fmaf(mu, mn, gs) : mn;
-            acc = fma((double)u, (double)u, acc);
-            m[e] = mn;
-            const uint64_t r = e / L.cols, col = e - r * L.cols;
-            store1(x + r * L.pitch_x + col, u);
-          }
-        }
-      }
+      const uint32_t ce = chunk_begin[mi + 1];
+      for (uint32_t c = c0; c < ce; c += gridDim.x)
+        momentum_chunk<GT, XT, true>(mats, mi, c, G, M, ws, partial, mu, omm, nesterov, red);
     }
-    const double s = block_sum(acc, red);
-    if (threadIdx.x == 0) partial[c] = s;
+    __syncthreads();                             // run_first[0 .. kept) complete before the next sweep reads it
+    if (kept == n_runs) {                        // a sweep without progress
+      if (!idle) { idle = true; idle_since = clock64(); }
+      else if (clock64() - idle_since > 20000000000ll) __trap();   // ~10 s: the producer never signalled
+      __nanosleep(500);
+    } else {
+      idle = false;
+    }
+    n_runs = kept;
   }
 }
 
@@ -385,13 +460,13 @@ int launch_momentum(const Plan& pl, const void* G, void* M, const mfsdp_muon_hpa
 #define MOM(GT, XT)                                                                                                    \
   do {                                                                                                                 \
     if (ready)                                                                                                         \
-      k_momentum<GT, XT, true><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                   \
+      k_momentum_gated<GT, XT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, pl.d_chunk_begin, lay.n_chunks, \
                                                             static_cast<const GT*>(G), static_cast<float*>(M), ws,     \
                                                             partial, mu, omm, hp.nesterov, ready, epoch);              \
     else                                                                                                               \
-      k_momentum<GT, XT, false><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                  \
-                                                             static_cast<const GT*>(G), static_cast<float*>(M), ws,    \
-                                                             partial, mu, omm, hp.nesterov, nullptr, 0u);              \
+      k_momentum<GT, XT><<<grid, kEwThreads, 0, st>>>(pl.d_mats, pl.d_chunk_mat, lay.n_chunks,                         \
+                                                      static_cast<const GT*>(G), static_cast<float*>(M), ws,           \
+                                                      partial, mu, omm, hp.nesterov);                                  \
   } while (0)
   if (gbf && xbf) MOM(__nv_bfloat16, __nv_bfloat16);
   else if (gbf) MOM(__nv_bfloat16, float);

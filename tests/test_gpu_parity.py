@@ -218,7 +218,7 @@ def test_edge_shapes(pair_min_d, precision, min_d):
 
 
 @pytest.mark.parametrize("below_d,below_d2", [(129, 257), (65, 193), (1, 1)])
-@pytest.mark.parametrize("wname", ["fused", "fused2", "small", "medium", "edge"])
+@pytest.mark.parametrize("wname", ["fused", "fused2", "fused8", "small", "medium", "edge"])
 def test_whole_matrix_class_bf16(fused_below_d, wname, below_d, below_d2):
     """The whole-matrix kernels (one CTA per matrix for all K iterations: d <= 128 with X, A, P on chip; 128 < d <= 256
     with A, P on chip and X streamed) on every shape they accept -- all size classes, tall / wide, ragged d and n,
@@ -419,11 +419,13 @@ def test_paper_setting_parity():
                 assert ulps.max() <= 1 and (ulps > 0).mean() <= 2e-3
 
 
-@pytest.mark.parametrize("wname", ["small", "medium", "fused", "fused2", "c3"])
+@pytest.mark.parametrize("wname", ["small", "medium", "fused", "fused2", "fused8", "c3"])
 def test_separate_passes_equal_fused_step(wname):
     """mfsdp_muon_step == momentum pass + NS pass + update pass, bit for bit -- also where the step applies the weight
     update inside the last Newton-Schulz epilogue (bf16 weights, every cols % 8 == 0: medium, c3) instead of running
-    k_update, with and without MFSDP_STEP_KEEP_O."""
+    k_update, with and without MFSDP_STEP_KEEP_O.  `fused8` is the set that reaches the update fused into the whole-matrix
+    kernel (ns_fused.cu update_row64) on ragged shapes: every matrix in that class, every cols % 8 == 0, nothing else
+    aligned."""
     wl = workloads.get(wname)
     b = gh.Session(wl)
     b.load_grads(0)
@@ -468,6 +470,8 @@ def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
         def produce():
             with torch.cuda.stream(side):
                 for wave in waves:
+    if wname == "fused8":
+        assert all(mf.mfsdp_ns_class(d.rows, d.cols) == 0 and d.cols % 8 == 0 for d in b.mats)
                     for i in wave:
                         d = b.mats[i]
                         sl = slice(d.elem_off, d.elem_off + d.rows * d.cols)
@@ -491,8 +495,53 @@ def test_gated_step_gradients_arrive_in_waves(wname, consumer_first):
             assert torch.equal(x, y)
 
 
-@pytest.mark.parametrize("wname", ["medium", "small", "fused", "fused2", "c3", "c1"])
-def test_fanout_copy_of_the_updated_weights(wname):
+def test_gated_pass_takes_matrices_in_arrival_order():
+    """The gated momentum pass must not wait for the table's FIRST matrix before it touches the others: the library's own
+    reduction order (mfsdp_reduce_schedule, reverse_blocks = 1) lands the LAST block first.  GPT-2-small
+    set (48 matrices, about 5000 chunks, far more than the 296 waiting CTAs, so every CTA owns chunks of many matrices).
+    The step is enqueued with no flag raised; then the flags go up in three waves, last third of the table first, and
+    BEFORE the next wave is signalled the momentum of the current wave's matrices must already hold its final value
+    (read with copy engines on a side stream while the kernel still waits for the rest)."""
+    import time
+    wl = workloads.get("c2")
+    a = gh.Session(wl)
+    a.load_grads(0)
+    a.muon_step()
+    want_M = a.M.cpu()
+    b = gh.Session(wl)
+    b.load_grads(0)
+    n_mat = len(b.mats)
+    ready = torch.zeros(n_mat, dtype=torch.int32, device="cuda")
+    side = torch.cuda.Stream()
+    host = torch.empty(b.M.numel(), dtype=torch.float32).pin_memory()
+    third = (n_mat + 2) // 3
+    waves = [list(range(n_mat))[max(0, n_mat - (k + 1) * third):n_mat - k * third] for k in range(3)]   # last third first
+    assert sorted(sum(waves, [])) == list(range(n_mat))
+    torch.cuda.synchronize()
+    mf.mfsdp_muon_step_gated(b.desc, b.W, b.G, b.M, b.ws, b.hp, ready, 1)      # waits: nothing has been signalled
+    late = []
+    for k, wave in enumerate(waves):
+        for i in wave:
+            mf.mfsdp_signal_ready(ready, i, 1, side)
+        lo = min(b.mats[i].elem_off for i in wave)
+        hi = max(b.mats[i].elem_off + b.mats[i].rows * b.mats[i].cols for i in wave)
+        done, t0 = False, time.time()
+        while not done and time.time() - t0 < 3.0:
+            with torch.cuda.stream(side):
+                host[lo:hi].copy_(b.M[lo:hi], non_blocking=True)
+            side.synchronize()
+            done = all(torch.equal(host[d.elem_off:d.elem_off + d.rows * d.cols],
+                                   want_M[d.elem_off:d.elem_off + d.rows * d.cols]) for d in (b.mats[i] for i in wave))
+        if not done:
+            late.append(k)          # keep signalling, so that the kernel ends instead of running into its watchdog
+    torch.cuda.synchronize()
+    assert not late, "waves %s were not finished before the next wave was signalled" % late
+    assert torch.equal(a.W, b.W) and torch.equal(a.M, b.M)
+
+
+@pytest.mark.parametrize("flags", [mf.STEP_KEEP_O, 0])
+@pytest.mark.parametrize("wname", ["medium", "small", "fused", "fused2", "fused8", "c3", "c1"])
+def test_fanout_copy_of_the_updated_weights(wname, flags):
     """SURVEY 8(f) f2, single-GPU half: mfsdp_muon_step_fanout writes every updated matrix into its fan-out destination
     from the same registers that update the owner's shard -- in the Newton-Schulz epilogue where the update is fused
     (medium, c3, the whole-matrix class of `fused`), in k_update otherwise (small: odd column counts).  Every second
@@ -502,7 +551,7 @@ def test_fanout_copy_of_the_updated_weights(wname):
     a = gh.Session(wl)
     a.load_grads(0)
     a.muon_step()
-    b = gh.Session(wl)
+    b = gh.Session(wl, hp_over=dict(flags=flags))
     b.load_grads(0)
     guard = 64
     bufs, fan = [], []
@@ -625,12 +674,15 @@ def test_tile_trace_covers_every_tile_once():
     assert (np.diff(first_ready) > 0).all()
 
 
-@pytest.mark.parametrize("wname", ["small", "medium", "edge"])
-def test_no_write_outside_the_buffers(wname):
+@pytest.mark.parametrize("wname,flags", [("small", mf.STEP_KEEP_O), ("medium", mf.STEP_KEEP_O), ("edge", mf.STEP_KEEP_O),
+                                         ("medium", 0), ("fused8", mf.STEP_KEEP_O), ("fused8", 0), ("fused2", 0)])
+def test_no_write_outside_the_buffers(wname, flags):
     """Guard bands around W, M and the workspace stay intact (the TMA stores are clipped by the tensor maps, the
-    elementwise passes by the segment tables), and the gradient is never written."""
+    elementwise passes by the segment tables, the update fused into the Newton-Schulz epilogues -- flags = 0: O is not
+    stored, W is written straight from the accumulator -- by its own row / column guards), and the gradient is never
+    written."""
     wl = workloads.get(wname)
-    sess = gh.Session(wl, precision=mf.NS_BF16)
+    sess = gh.Session(wl, precision=mf.NS_BF16, hp_over=dict(flags=flags))
     sess.load_grads(0)
     guard = 1 << 16
 

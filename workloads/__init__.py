@@ -162,6 +162,19 @@ def fused2_shapes(seed=23, dtype=BF16, precision=NS_BF16):
 
 
 def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
+def fused8_shapes(seed=29, dtype=BF16, precision=NS_BF16):
+    """Whole-matrix class (min(rows, cols) <= 128, padded X <= 128 KB) with EVERY column count a multiple of 8, so that
+    the weight update runs inside that kernel's last epilogue (one odd column count anywhere in a table sends the whole
+    table to the separate update pass), and with nothing else aligned: d not a multiple of 16, n not a multiple of 64,
+    tall row counts not multiples of 128, both shared-memory size classes (X <= 64 KB and <= 128 KB), tall / wide twins."""
+    shapes = [(100, 304), (304, 72), (72, 256), (120, 200), (200, 120), (8, 24), (104, 488), (488, 104), (56, 56),
+              (24, 8), (40, 504), (300, 88)]
+    params = [(i // 4, 2, r, c, dtype, 0) for i, (r, c) in enumerate(shapes)]
+    params += [(1, 1, 77, 1, dtype, 0)]
+    params.sort(key=lambda p: p[0])
+    return Workload("fused8_shapes", params, seed=seed, precision=precision, dtype=dtype, row_lognormal=True)
+
+
     """The paper's convergence model puts the 50,257 x 768 embedding and the untied LM head on Muon (PAPER.md:121):
     a very tall matrix with an odd row count (GRAM k loop of 786 blocks) next to one ordinary matrix."""
     params = [(0, 2, 50257, 768, dtype, 0), (1, 2, 768, 3072, dtype, 0), (1, 1, 768, 1, dtype, 0)]
@@ -171,6 +184,7 @@ def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
 CONFIGS = {"paper16l": paper_qwen16l, "c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
            "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes, "fused": fused_shapes, "fused2": fused2_shapes,
            "vocab": vocab_embedding}
+           "fused8": fused8_shapes,
 
 
 def get(name):
