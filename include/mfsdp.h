@@ -299,7 +299,10 @@ int mfsdp_signal_ready(uint32_t* ready, size_t index, uint32_t epoch, void* cuda
  *   fanout   HOST in.  one DEVICE pointer per MATRIX descriptor, in table order; NULL entries = no copy for that matrix.
  * The transfer order for non-multicast fan-out is the forward-order schedule of mfsdp_reduce_schedule
  * (reverse_blocks = 0); its per-block cost estimate is C_B^owner of mfsdp_score_plan.  Not CUDA-graph capturable (the
- * destination table is copied from the host array on every call).  Bit-identical W to mfsdp_muon_step. */
+ * destination table is copied from the host array on every call).  The device copy of that table belongs to the cached
+ * launch tables of (table, workspace): fan-out calls that share them must be ordered on ONE stream -- a second call on
+ * another stream or thread would overwrite the table under the first call's kernels (they share the workspace anyway).
+ * Bit-identical W to mfsdp_muon_step. */
 int mfsdp_muon_step_fanout(const mfsdp_desc_t* desc, size_t n_desc, void* W, const void* G, void* M,
                            void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp,
                            void* const* fanout, void* cuda_stream);
@@ -333,12 +336,6 @@ int mfsdp_muon_step_host(const mfsdp_desc_t* desc, size_t n_desc, void* hW, cons
                          void* dW, void* dG, void* dM, int upload_state,
                          void* workspace, size_t ws_bytes, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
 
-/* ---- AdamW on packed tails (DEVICE work, HOST call) ------------------------------------------------------------
- * For every TAIL descriptor (matrix descriptors are ignored), element-wise (PAPER.md:45, 47, 121; SURVEY.md O-3):
- *   p <- p (1 - lr wd) ; m <- b1 m + (1-b1) g ; v <- b2 v + (1-b2) g^2 ;
- *   p <- p - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps).
- *   P, G   DEVICE. rank-flat tail parameters / gradients, dtype of the descriptors (one dtype for all tails).
- *   m, v   DEVICE. rank-flat first / second moments, always float, same element offsets.
 /* ---- momentum pass of one matrix for callers that may not allocate (DEVICE work, HOST call) ----------------------
  * Every step call above builds device-side launch tables with cudaMalloc the first time it sees a (table, workspace)
  * pair and needs a caller-allocated workspace.  Some callers of an owner-local optimizer can do neither: a trainer
@@ -376,6 +373,12 @@ uint64_t mfsdp_static_max_elems(void);
 int mfsdp_momentum_pass_static(uint32_t rows, uint32_t cols, int dtype, int precision, const void* G, void* M, void* X,
                                double* ssq, float* inv_norm, const mfsdp_muon_hparams_t* hp, void* cuda_stream);
 
+/* ---- AdamW on packed tails (DEVICE work, HOST call) ------------------------------------------------------------
+ * For every TAIL descriptor (matrix descriptors are ignored), element-wise (PAPER.md:45, 47, 121; SURVEY.md O-3):
+ *   p <- p (1 - lr wd) ; m <- b1 m + (1-b1) g ; v <- b2 v + (1-b2) g^2 ;
+ *   p <- p - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps).
+ *   P, G   DEVICE. rank-flat tail parameters / gradients, dtype of the descriptors (one dtype for all tails).
+ *   m, v   DEVICE. rank-flat first / second moments, always float, same element offsets.
  * Returns as mfsdp_muon_step (hp->step < 1 is MFSDP_EINVAL). */
 int mfsdp_adamw_tail_step(const mfsdp_desc_t* desc, size_t n_desc, void* P, const void* G, void* m, void* v,
                           const mfsdp_adamw_hparams_t* hp, void* cuda_stream);
@@ -445,8 +448,15 @@ int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void* W, const v
  * rows x out[4] bf16, out[6] elements apart), P_R (3 planes of cols x out[5] bf16, out[7] elements apart);
  * out[8] = byte offset in the workspace of D (rows x out[5] floats; MFSDP_SHAMPOO_KEEP_D only);
  * out[9] = byte offset in the workspace of the root control records of this matrix (L then R), out[10] bytes each:
- *   { double tr, fro2; float rho, z, x0, last_err; uint32 err_bits, iters, done (1 converged / stopped, 2 NaN), identity;
- *     float alpha_m, alpha_x; uint32 n_scaled, pad }. */
+ *   { double tr, fro2; float rho, z, x0, last_err; uint32 err_bits, iters, done, identity;
+ *     float alpha_m, alpha_x; uint32 n_scaled, pad }  with done = 1 converged (max |M - I| < root_tol, or at the fp32-class
+ *     noise floor), 2 the iteration met a NaN (S~ not positive definite in this arithmetic: the root was REPLACED by the
+ *     scalar (tr S / d + rho)^{-1/4} I), 3 max_root_iters reached first (P is the last iterate, not a converged root);
+ * out[11] = byte offset in the workspace of the status record of the last step that recomputed roots:
+ *   uint32 { converged, not_positive_definite, out_of_budget, roots } over the whole resident set.  mfsdp_shampoo_step
+ *   itself returns MFSDP_OK in all three cases (it never synchronises): a caller that must know whether the method's
+ *   own roots were used reads these 16 bytes after the step -- anything but {roots, 0, 0, roots} means some
+ *   preconditioner is a substitute. */
 int mfsdp_shampoo_view(const mfsdp_desc_t* desc, size_t n_desc, uint32_t flags, size_t index, size_t out[12]);
 
 /* Debug / test aid (HOST): byte offsets inside the workspace of the `index`-th matrix' NS buffers:

@@ -236,13 +236,29 @@ __global__ void k_sh_root_ctl(const RootInfo* roots, uint32_t n, ShCtl* ctl, flo
   // converged; or at the fp32-class noise floor (the error no longer falls); or not a number; or out of budget
   // (the stagnation rule only inside the quadratic regime: far from convergence the error sits just below 1 and
   // consecutive values may round to the same float)
-  if (!(e >= tol) || (e < 1e-2f && !(e < c->prev_err)) || c->iters >= max_iters) c->done = 1u;
+  if (!(e >= tol) || (e < 1e-2f && !(e < c->prev_err))) c->done = 1u;
+  else if (c->iters >= max_iters) c->done = 3u;     // out of budget: X is the best iterate so far, NOT a converged root
   if (!(e == e)) c->done = 2u;
   c->prev_err = e;
   c->err = 0u;
   const bool scale_next = c->iters + 1u <= c->n_scaled;      // the outputs of iteration iters + 1
   c->alpha_m = scale_next ? 2.5f : 1.f;
   c->alpha_x = scale_next ? 1.2574334f : 1.f;
+}
+
+// Status record of the last root refresh, behind the control block (mfsdp_shampoo_view out[11]): how many of the n
+// root problems ended converged (done == 1, identity problems included), not positive definite (2), out of budget (3).
+__global__ void __launch_bounds__(256) k_sh_status(const ShCtl* ctl, uint32_t n, uint32_t* status) {
+  __shared__ uint32_t cnt[4];
+  if (threadIdx.x < 4) cnt[threadIdx.x] = 0u;
+  __syncthreads();
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+    const uint32_t d = ctl[i].done;
+    atomicAdd(&cnt[d == 1u ? 0 : d == 2u ? 1 : d == 3u ? 2 : 3], 1u);      // [3]: still running (never after a refresh)
+  }
+  __syncthreads();
+  if (threadIdx.x < 3) status[threadIdx.x] = cnt[threadIdx.x];
+  if (threadIdx.x == 3) status[3] = n;
 }
 
 // P <- X[iters & 1].  A root whose iteration produced a NaN (done == 2: S + rho I was not positive definite in this
@@ -366,7 +382,7 @@ int build_sh_layout(const mfsdp_desc_t* desc, size_t n_desc, bool keep_d, ShLayo
   out.state_bytes = st;
   const uint64_t n_prob = 2 * out.mats.size();
   uint64_t ws = 0;
-  out.ctl_off = ws; ws = align_up_u64(ws + n_prob * sizeof(ShCtl), kBufAlign);
+  out.ctl_off = ws; ws = align_up_u64(ws + n_prob * sizeof(ShCtl) + 4 * sizeof(uint32_t), kBufAlign);   // + status record
   out.partial_off = ws; ws = align_up_u64(ws + n_prob * kRedBlocks * kPartWords * sizeof(double), kBufAlign);
   for (ShMat& m : out.mats) {
     if (!m.g_direct) { m.Gs_off = ws; ws = align_up_u64(ws + (uint64_t)m.g_terms * m.rows * m.pc * 2, kBufAlign); }
@@ -811,7 +827,7 @@ extern "C" int mfsdp_shampoo_view(const mfsdp_desc_t* desc, size_t n_desc, uint3
   out[8] = (flags & MFSDP_SHAMPOO_KEEP_D) ? m.D_off : 0;
   out[9] = lay.ctl_off + 2 * index * sizeof(ShCtl);
   out[10] = sizeof(ShCtl);
-  out[11] = 0;
+  out[11] = lay.ctl_off + 2 * lay.mats.size() * sizeof(ShCtl);
   return MFSDP_OK;
 }
 
@@ -836,9 +852,10 @@ extern "C" int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void*
   if (rc) return rc;
   if (state_bytes < pl->lay.state_bytes) return MFSDP_ECAP;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-  if (pl->W != W || pl->G != G) {
+  {                                       // the addresses the records point to are plan state: compare under the lock
     std::lock_guard<std::mutex> lock(plan_mutex());
-    if ((rc = repoint_sh_plan(*pl, reinterpret_cast<uint8_t*>(W), reinterpret_cast<const uint8_t*>(G), st))) return rc;
+    if (pl->W != W || pl->G != G)
+      if ((rc = repoint_sh_plan(*pl, reinterpret_cast<uint8_t*>(W), reinterpret_cast<const uint8_t*>(G), st))) return rc;
   }
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
   ShCtl* d_ctl = reinterpret_cast<ShCtl*>(ws + pl->lay.ctl_off);
@@ -882,6 +899,10 @@ extern "C" int mfsdp_shampoo_step(const mfsdp_desc_t* desc, size_t n_desc, void*
       count_launch();
       if ((rc = check_last_launch())) return rc;
     }
+    const uint32_t n_prob = 2u * (uint32_t)pl->lay.mats.size();
+    k_sh_status<<<1, 256, 0, st>>>(d_ctl, n_prob, reinterpret_cast<uint32_t*>(d_ctl + n_prob));
+    count_launch();
+    if ((rc = check_last_launch())) return rc;
   }
   if ((rc = sg_launch(*pl, pl->pre1, 1.f, 0.f, 0.f, 0.f, st))) return rc;
   const float decay = (float)(1.0 - hp->lr * hp->weight_decay);

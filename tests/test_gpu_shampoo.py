@@ -9,7 +9,11 @@ quarter of that.  With rho >= eps_floor ||S||_F = 2^-20 ||S||_F (reading S7) tha
 its largest (ridge) directions by 2^-22 / 2^-20 / 4 = 6e-2 per product; asserted: relF(P) <= 2e-2 (measured <= 5e-3
 where the ridge is at the floor, 1e-6 .. 1e-3 otherwise).  D = P_L G P_R sees those directions only through the part
 of G that lies in them: relF(D) <= 2e-3 with fresh roots (measured <= 2e-4), and with a 30 x larger ridge (eps = 1e-3)
-relF(P), relF(D) <= 2e-3 also for stale roots (measured 3e-4).  W is checked lock-step from the GPU's own D with the rule of reading
+relF(P), relF(D) <= 1e-3 also for stale roots (measured 3e-4).  Round 3: relF(D) <= 5e-4 with fresh
+roots on every set (measured <= 2e-4); relF(P) <= 2e-3 for every root whose ridge is NOT at the S7 floor (2e-2 only where
+it is); with eps_floor = 0 on full-rank square statistics -- reading S2 alone, the un-floored oracle -- relF(P) <= 5e-4
+and relF(D) <= 1e-4 (measured 1.5e-4 and 3.1e-5: the paper's own float32 figure is <= 4e-5 on loss trajectories,
+PAPER.md:182).  W is checked lock-step from the GPU's own D with the rule of reading
 U1, and against the oracle's W in norm.  Measured values are printed."""
 import numpy as np
 import pytest
@@ -100,13 +104,24 @@ class ShampooSession:
             ctl.append(dict(tr=tr, rho=rho, z=z, last_err=float(last), iters=int(iters), done=int(done), identity=int(ident)))
         return L, R, PL, PR, D, ctl
 
+    def status(self):
+        """{converged, not_positive_definite, out_of_budget, roots} of the last step that recomputed roots."""
+        off = self.view(0)[11]
+        return [int(x) for x in self.ws[off:off + 16].view(torch.int32).cpu().tolist()]
+
+
+P_TOL_UNFLOORED = 2e-3
+
 
 def _run_and_check(sess, steps, tol_p, tol_d, label):
     worst = dict(L=0.0, R=0.0, PL=0.0, PR=0.0, D=0.0)
+    floor_seen = {True: 0.0, False: 0.0}          # worst relF(P) of fresh roots with the ridge at / above the floor
     for t in range(1, steps + 1):
         W_old = [sess.seg64(sess.W, d) for d in sess.mats]
         sess.step(t)
         kw = sess.hp_kw
+        if (t - 1) % kw["root_every"] == 0:           # every root converged: none replaced (2), none out of budget (3)
+            assert sess.status() == [2 * len(sess.mats), 0, 0, 2 * len(sess.mats)], sess.status()
         for i, d in enumerate(sess.mats):
             G = sess.seg64(sess.hG, d)
             out = oshampoo.shampoo_step(W_old[i], G, sess.oL[i], sess.oR[i], sess.oPL[i], sess.oPR[i], t, lr=kw["lr"],
@@ -123,7 +138,14 @@ def _run_and_check(sess, steps, tol_p, tol_d, label):
                 worst[k] = max(worst[k], e[k])
             assert np.array_equal(L, L.T) and np.array_equal(R, R.T), "statistics must be bit-symmetric"
             assert e["L"] <= 1e-6 and e["R"] <= 1e-6, (label, t, i, e)
-            assert e["PL"] <= tol_p and e["PR"] <= tol_p, (label, t, i, e, ctl)
+            # a root whose ridge sits at the float32 floor (reading S7) is allowed tol_p; one whose ridge is the plain
+            # eps tr S / d of reading S2 must do better: P_TOL_UNFLOORED
+            for key, c, dim in (("PL", ctl[0], d.rows), ("PR", ctl[1], d.cols)):
+                at_floor = c["identity"] == 0 and c["rho"] > kw["eps"] * c["tr"] / dim * (1.0 + 1e-3)
+                lim = tol_p if at_floor else min(tol_p, P_TOL_UNFLOORED)
+                if (t - 1) % kw["root_every"] == 0:
+                    floor_seen[at_floor] = max(floor_seen[at_floor], e[key])
+                assert e[key] <= lim, (label, t, i, key, e, c, at_floor)
             assert e["D"] <= tol_d, (label, t, i, e)
             assert ctl[0]["done"] == 1 and ctl[1]["done"] == 1, ctl
             # lock-step update from the GPU's own D (reading U1): W = rn(decay W_old - lr D)
@@ -141,23 +163,53 @@ def _run_and_check(sess, steps, tol_p, tol_d, label):
             store = 2.0 ** -8 if d.dtype == mf.BF16 else 2.0 ** -23      # half an ulp relative to the value, at worst
             assert np.linalg.norm(got - out["W"]) <= (kw["lr"] * tol_d * np.linalg.norm(out["D"])
                                                       + store * np.linalg.norm(out["W"])), (label, t, i)
-    print(label, "worst", {k: "%.1e" % v for k, v in worst.items()})
+    print(label, "worst", {k: "%.1e" % v for k, v in worst.items()},
+          "relF(P) ridge at floor %.1e, above it %.1e" % (floor_seen[True], floor_seen[False]))
     return worst
 
 
 def test_shampoo_small_ragged_three_steps():
     sess = ShampooSession(workloads.small_ragged())
-    _run_and_check(sess, 3, 2e-2, 2e-3, "small")
+    _run_and_check(sess, 3, 2e-2, 5e-4, "small")
 
 
 def test_shampoo_medium_ragged_moving_average_stale_roots():
     sess = ShampooSession(workloads.medium_ragged(), beta2=0.99, root_every=2, eps=1e-3)
-    _run_and_check(sess, 3, 2e-3, 2e-3, "medium")
+    _run_and_check(sess, 3, 1e-3, 1e-3, "medium")
 
 
 def test_shampoo_fp32_storage():
     sess = ShampooSession(workloads.c1_tiny())
-    _run_and_check(sess, 2, 2e-2, 2e-3, "c1")
+    _run_and_check(sess, 2, 2e-2, 5e-4, "c1")
+
+
+@pytest.mark.parametrize("eps", [1e-3, 1e-4])
+def test_shampoo_unfloored_reading_on_full_rank_statistics(eps):
+    """Reading S2 alone (eps_floor = 0: rho = eps tr S / d, the oracle as first committed, before S7 existed) where it
+    is well posed in float32: square, full-rank Gaussian gradients without the per-row scale, so that both statistics
+    have every eigenvalue far above the 2^-22 ||S||_F rounding noise and the ridge is far above it too.  No floor is
+    involved on either side; the iteration must converge (status record: no substitute root, none out of budget)."""
+    shapes = [(130, 130), (384, 384), (768, 768)]
+    wl = workloads.Workload("square_full_rank", [(i, 2, r, c, workloads.BF16, 0) for i, (r, c) in enumerate(shapes)],
+                            seed=31, row_lognormal=False)
+    sess = ShampooSession(wl, eps=eps, eps_floor=0.0)
+    _run_and_check(sess, 2, 5e-4, 1e-4, "unfloored eps=%g" % eps)
+
+
+def test_shampoo_status_distinguishes_budget_exhaustion():
+    """done == 3 / the status record: a root that used up max_root_iters is reported as such, not as converged."""
+    sess = ShampooSession(workloads.small_ragged(), max_root_iters=2)
+    sess.step(1)
+    conv, notpd, budget, roots = sess.status()
+    assert roots == 2 * len(sess.mats) and notpd == 0 and budget > 0 and conv + budget == roots
+    seen = 0
+    for i in range(len(sess.mats)):
+        for c in sess.read_all(i)[5]:
+            assert c["done"] in (1, 3)
+            if c["done"] == 3:
+                assert c["iters"] == 2
+                seen += 1
+    assert seen == budget
 
 
 def test_shampoo_grouped_workspace_is_bit_identical():
@@ -220,7 +272,7 @@ def test_shampoo_c2_shapes_full_oracle():
     shapes = [(768, 2304), (768, 768), (768, 3072), (3072, 768)]
     wl = workloads.Workload("c2_shapes", [(i, 2, r, c, workloads.BF16, 0) for i, (r, c) in enumerate(shapes)], seed=1)
     sess = ShampooSession(wl)
-    _run_and_check(sess, 2, 2e-2, 2e-3, "c2shapes")
+    _run_and_check(sess, 2, 2e-2, 5e-4, "c2shapes")
 
 
 def test_shampoo_step_is_graph_capturable():
@@ -405,7 +457,7 @@ def test_shampoo_edge_shapes():
     """Degenerate and boundary shapes (scalars, single rows / columns, exact tile multiples and one past them, very thin
     matrices with a 4096-long statistic on the other side) against the oracle."""
     sess = ShampooSession(workloads.edge_shapes())
-    _run_and_check(sess, 2, 2e-2, 2e-3, "edge")
+    _run_and_check(sess, 2, 2e-2, 5e-4, "edge")
 
 
 def test_shampoo_ten_steps_free_running_statistics():
