@@ -174,7 +174,10 @@ def plan_for(wl, rank_override=None):
     return oplan.plan(wl.params, wl.world, wl.policy, wl.metric, r)
 
 
-ORACLE_BUDGET_FLOPS = 3.6e12      # dense fp64 flops per sample: about 12 s of dgemm on 16 host cores
+ORACLE_BUDGET_FLOPS = 2.6e13      # dense fp64 flops of the cpu_baseline sample: on the headline set that is every distinct
+                                  # shape, 1024 x 8192 and 8192 x 8192 for all five iterations and the dominant 28672 x 8192
+                                  # (79 % of the step's flops) for one whole iteration; about 40 s of dgemm on 16 host cores
+REFERENCE_TOTAL_FLOPS = 8.0e13    # --impl reference: budget of the whole run (all steps and the warm-up): a few minutes
 
 
 def oracle_sample(wl, desc, budget_flops=ORACLE_BUDGET_FLOPS):
@@ -233,12 +236,13 @@ def time_oracle(wl, sample, steps=1):
     return times, f_alg, cores
 
 
-def sample_text(wl, sample, skipped):
+def sample_text(wl, sample, skipped, budget=None):
+    budget = ORACLE_BUDGET_FLOPS if budget is None else budget
     K = wl.muon["ns_steps"]
     txt = "per-shape sampled, one matrix per distinct resident shape: " + ", ".join(
         "%dx%d (%d of %d NS iterations)" % (d["rows"], d["cols"], k, K) for d, k in sample)
     if skipped:
-        txt += "; not affordable within %.1e fp64 flops: " % ORACLE_BUDGET_FLOPS + ", ".join("%dx%d" % s for s in skipped)
+        txt += "; not affordable within %.1e fp64 flops: " % budget + ", ".join("%dx%d" % s for s in skipped)
     return txt
 
 
@@ -266,13 +270,15 @@ def run_reference(args):
     import workloads
     wl = apply_setting(workloads.get(args.config), args)
     pl = plan_for(wl)
-    sample, skipped = oracle_sample(wl, pl["desc"])
-    for _ in range(max(0, min(args.warmup, 1))):
+    n_warm = max(0, min(args.warmup, 1))
+    budget = min(ORACLE_BUDGET_FLOPS, REFERENCE_TOTAL_FLOPS / (max(1, args.steps) + n_warm))
+    sample, skipped = oracle_sample(wl, pl["desc"], budget)
+    for _ in range(n_warm):
         time_oracle(wl, sample, 1)
     times, f_alg, cores = time_oracle(wl, sample, max(1, args.steps))
     t = sum(times) / len(times)
     val = f_alg / t / 1e12
-    txt = sample_text(wl, sample, skipped)
+    txt = sample_text(wl, sample, skipped, budget)
     line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=t * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f64", data="synthetic (seeded, workloads/)", config=workload_config(wl, pl["desc"], pl["rank"]),
@@ -412,6 +418,23 @@ def passes_record(res, t, pk):
                             note="separate pass; mfsdp_muon_step applies the update in the last NS epilogue when "
                                  "the weights are bf16 and every cols % 8 == 0"),
                 adamw=dict(ms=t["adam"], gbs=gbs(b_adam, t["adam"])), ns=dict(ms=t["ns"]))
+
+
+def compact_config(rec, pk):
+    """One row of roofline.configs from a verbose other_configs record: the numbers the documents quote, nothing else."""
+    if "error" in rec:
+        return dict(workload=rec.get("workload"), error=rec["error"][:120])
+    if "refresh_step" in rec:           # Shampoo: the method's own work is fp32-class; three-term operands issue 6 x that in bf16
+        peak = pk["tc_sustained"] if rec["frac_of"].startswith("sustained") else pk["tc_burst"]
+        f32 = rec["refresh_step"]["f32_class_tflops"]
+        return dict(workload=rec["workload"] + "+shampoo", bound="tensor", unit="TFLOP/s (fp32-class)", achieved=f32,
+                    peak=peak / 6.0, frac=f32 / (peak / 6.0), frac_of=rec["frac_of"].split(" ")[0] + " bf16 peak / 6",
+                    issued_bf16_tflops=rec["refresh_step"]["umma_bf16_tflops"], refresh_ms=rec["refresh_step"]["ms"],
+                    stale_ms=rec["stale_step"]["ms"], root_iters_max=rec["refresh_step"]["root_iters_max"],
+                    sm_mhz=rec["clocks"]["sm_mhz"])
+    return dict(workload=rec["workload"], ms_per_step=rec["ms_per_step"], ns_ms=rec["ns_ms"], ns_tflops_alg=rec["ns_tflops_alg"],
+                ns_frac=rec["ns_frac"], frac_of=rec["ns_frac_of"].split(" ")[0], momentum_gbs=rec["momentum_gbs"],
+                update_gbs=rec["update_gbs"], launches_per_step=rec["launches_per_step"], sm_mhz=rec["clocks"]["sm_mhz"])
 
 
 def measure_other_config(torch, mf, name, pk, local, paper=False, reuse=None, precision=None):
@@ -637,7 +660,7 @@ def run_ours(args):
                             traffic_ratio=(traffic / min_bytes) if traffic else None, min_hbm_bytes=min_bytes,
                             peak_source=pk["src"] + ", sustained bf16", frac_of_burst=ns_tflops / pk["tc_burst"],
                             dense_equiv_tflops=res.f_dense / (t["ns"] * 1e-3) / 1e12, ms=t["ns"])
-    line["passes"] = passes_record(res, t, pk)
+    line["roofline"]["passes"] = passes_record(res, t, pk)      # the HBM-bound passes of the same step, against the copy peak
     if world > 1:
         pr = mf.mfsdp_plan(wl.params, wl.world, wl.policy, wl.metric, 0)
         planned = [pr.rank_load[r] for r in ranks_run]
@@ -684,12 +707,18 @@ def run_ours(args):
                 others.append(dict(workload=name + "+shampoo", error=repr(e)))
             torch.cuda.empty_cache()
         line["other_configs"] = others
+        line["roofline"]["configs"] = [compact_config(o, pk) for o in others]
     if not args.no_cpu_baseline and world == 1:
         desc_d = plan_for(wl, plan_rank)["desc"]
         sample, skipped = oracle_sample(wl, desc_d)
         times, fa, cores = time_oracle(wl, sample, 1)
         line["cpu_baseline"] = dict(value=fa / times[0] / 1e12, unit=UNIT, cores=cores, kind="oracle",
                                     sample=sample_text(wl, sample, skipped), seconds=times[0])
+    # key order: the verbose per-config records first, the compact blocks (roofline with its `configs` and `passes`,
+    # cpu_baseline, e2e) last, so that a consumer that keeps only the tail of the line still holds every quoted number
+    for key in ("e2e", "cpu_baseline", "roofline"):
+        if key in line:
+            line[key] = line.pop(key)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -56,9 +56,7 @@ constexpr uint32_t kABytes = 2 * kBoxBytes;    // 128 x 64
 constexpr uint32_t kBBytes = 4 * kBoxBytes;    // single CTA: 256 x 64; paired: 2 halves x (128 x 64)
 constexpr uint32_t kStageBytes = kABytes + kBBytes;   // 48 KB
 constexpr uint32_t kStages = 4;
-#ifndef MFSDP_NS_GROUP
-#define MFSDP_NS_GROUP 2
-#endif
+constexpr uint32_t kPairGroup = 2;             // CTA-pair class: ring stages consumed per accumulator visit
 constexpr uint32_t kThreads = 224;   // producer, UMMA issuer, 4 epilogue warps, tile scheduler
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kEpiBufBytes = 4096;        // one staging tile: 32 rows x 64 cols (or 64 x 32 transposed) bf16
@@ -204,7 +202,7 @@ struct Feed {
 
 template <int kCG>
 __global__ void __launch_bounds__(kThreads, 1) k_ns_tc(const TcParams p) {
-  constexpr uint32_t kGroup = kCG == 2 ? MFSDP_NS_GROUP : 1;   // ring stages per accumulator visit
+  constexpr uint32_t kGroup = kCG == 2 ? kPairGroup : 1;   // ring stages per accumulator visit
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   // [operand ring: kStages x 48 KB][epilogue staging: 4 warps x 2 x 4 KB][barriers]

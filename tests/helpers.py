@@ -1,4 +1,5 @@
-"""Comparison helpers for the tests (numpy only; no method arithmetic)."""
+"""Comparison helpers for the tests (numpy only).  No method arithmetic, with one labelled exception at the end: a
+model of WHERE the bf16 mode stores bf16, used to explain its error on ill-conditioned inputs."""
 import numpy as np
 
 
@@ -40,3 +41,23 @@ def bf16_ulp_distance(a, b):
         u = bf16_bits(x).astype(np.int32)
         return np.where(u & 0x8000, 0x8000 - u, u)
     return np.abs(key(a) - key(b))
+
+
+def ns_bf16_storage_model(U, steps, coeffs, eps):
+    """NOT the oracle and not a definition of anything: the north_star's iteration evaluated in fp64 with a rounding to
+    bf16 at the places where the bf16 mode keeps bf16 (the cast X~ = bf16(U); A, P and every X_k as stored operands of
+    the next product; the normalisation folded into the first iteration as include/mfsdp.h describes it).  It separates
+    "what storing bf16 costs on this input" (model vs oracle) from "what else the kernels do differently" (GPU vs
+    model: fp32 accumulation order).  DESIGN.md section 4, tolerance T-ill."""
+    a, b, c = coeffs
+    U = np.asarray(U, dtype=np.float64)
+    tall = U.shape[0] > U.shape[1]
+    X = bf16_rne(U.T if tall else U).astype(np.float64)
+    inv = 1.0 / max(np.sqrt(np.sum(U * U)), eps)
+    eye = np.eye(X.shape[0])
+    for k in range(steps):
+        s2, s1 = (inv * inv, inv) if k == 0 else (1.0, 1.0)
+        A = bf16_rne((X @ X.T) * s2).astype(np.float64)
+        P = bf16_rne(a * eye + b * A + c * (A @ A)).astype(np.float64)
+        X = bf16_rne((P @ X) * s1).astype(np.float64)
+    return X.T if tall else X

@@ -41,6 +41,7 @@ class Workload:
     precision: int = NS_BF16
     dtype: int = BF16
     row_lognormal: bool = True        # gradients carry a per-row lognormal(0, 0.5) scale
+    spectra: dict = field(default_factory=dict)   # tensor_id -> "inv" | "inv2" | "rank8": gradient with that singular spectrum
     muon: dict = field(default_factory=lambda: dict(lr=0.02, weight_decay=0.01, momentum=0.95, nesterov=1,
                                                     ns_steps=5, a=3.4445, b=-4.7750, c=2.0315, eps=1e-7,
                                                     scale_mode=0))
@@ -161,7 +162,6 @@ def fused2_shapes(seed=23, dtype=BF16, precision=NS_BF16):
     return Workload("fused2_shapes", params, seed=seed, precision=precision, dtype=dtype, row_lognormal=True)
 
 
-def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
 def fused8_shapes(seed=29, dtype=BF16, precision=NS_BF16):
     """Whole-matrix class (min(rows, cols) <= 128, padded X <= 128 KB) with EVERY column count a multiple of 8, so that
     the weight update runs inside that kernel's last epilogue (one odd column count anywhere in a table sends the whole
@@ -175,6 +175,7 @@ def fused8_shapes(seed=29, dtype=BF16, precision=NS_BF16):
     return Workload("fused8_shapes", params, seed=seed, precision=precision, dtype=dtype, row_lognormal=True)
 
 
+def vocab_embedding(seed=17, dtype=BF16, precision=NS_BF16):
     """The paper's convergence model puts the 50,257 x 768 embedding and the untied LM head on Muon (PAPER.md:121):
     a very tall matrix with an odd row count (GRAM k loop of 786 blocks) next to one ordinary matrix."""
     params = [(0, 2, 50257, 768, dtype, 0), (1, 2, 768, 3072, dtype, 0), (1, 1, 768, 1, dtype, 0)]
@@ -183,8 +184,8 @@ def fused8_shapes(seed=29, dtype=BF16, precision=NS_BF16):
 
 CONFIGS = {"paper16l": paper_qwen16l, "c1": c1_tiny, "c2": c2_gpt2_small, "c3": c3_ragged, "c4": c4_llama8b, "c5": c5_llama70b,
            "small": small_ragged, "medium": medium_ragged, "edge": edge_shapes, "fused": fused_shapes, "fused2": fused2_shapes,
-           "vocab": vocab_embedding}
            "fused8": fused8_shapes,
+           "vocab": vocab_embedding}
 
 
 def get(name):
@@ -207,11 +208,44 @@ def weight(wl, tensor_id, rows, cols):
 
 def gradient(wl, tensor_id, rows, cols, step, is_tail=False):
     """G ~ N(0, 1e-3), times exp(0.5 xi_row) per stored row when the workload says so (never for tails)."""
+    if not is_tail and tensor_id in wl.spectra:
+        return _spectral_gradient(wl, tensor_id, rows, cols, step, wl.spectra[tensor_id])
     g = (np.float32(1e-3) * _normal(wl.seed, tensor_id, KIND_G, step, rows * cols)).reshape(rows, cols)
     if wl.row_lognormal and not is_tail:
         xi = _normal(wl.seed, tensor_id, KIND_ROWSCALE, step, rows)
         g *= np.exp(np.float32(0.5) * xi)[:, None]
     return g
+
+
+def _spectral_gradient(wl, tensor_id, rows, cols, step, kind):
+    """G = U diag(sigma) V^T with seeded Haar-like orthonormal factors (QR of Gaussian matrices) and a prescribed
+    spectrum: "inv" sigma_i = 1/i, "inv2" sigma_i = 1/i^2, "rank8" eight equal singular values and zeros; scaled to the
+    Frobenius norm 1e-3 sqrt(rows cols) of the Gaussian sets.  Ill-conditioned inputs of the Newton-Schulz iteration:
+    singular values far below the top one are amplified by ~3.44 per step and never reach 1 within K = 5."""
+    d = min(rows, cols)
+    rng = _rng(wl.seed, tensor_id, KIND_G, step)
+    U, _ = np.linalg.qr(rng.standard_normal((rows, d)))
+    V, _ = np.linalg.qr(rng.standard_normal((cols, d)))
+    i = np.arange(1, d + 1, dtype=np.float64)
+    sig = {"inv": 1.0 / i, "inv2": 1.0 / i ** 2, "rank8": (i <= 8).astype(np.float64)}[kind]
+    g = (U * sig) @ V.T
+    g *= 1e-3 * np.sqrt(rows * cols) / np.linalg.norm(g)
+    return g.astype(np.float32)
+
+
+def illcond_shapes(seed=37, dtype=BF16, precision=NS_BF16):
+    """Ill-conditioned gradients for every Newton-Schulz kernel class: 256 x 1024 and 768 x 768 (tile kernels), 100 x 304
+    (whole-matrix class), 200 x 504 (second whole-matrix class), each with the spectra 1/i, 1/i^2 and rank 8."""
+    shapes = [(256, 1024), (768, 768), (100, 304), (200, 504)]
+    params, spectra = [], {}
+    for si, (r, c) in enumerate(shapes):
+        for kind in ("inv", "inv2", "rank8"):
+            spectra[len(params)] = kind
+            params.append((si, 2, r, c, dtype, 0))
+    return Workload("illcond_shapes", params, seed=seed, precision=precision, dtype=dtype, spectra=spectra)
+
+
+CONFIGS["illcond"] = illcond_shapes
 
 
 def _fields(d):
